@@ -1,0 +1,157 @@
+/* nb.h -- C-ABI of the B200-native direct-summation force library (libnb.so).
+ *
+ * What the library is: the "force library" layer of a direct N-body code as the paper states the
+ * problem (section III.A): j-particles exert a force, i-particles receive it; the
+ * library keeps the j-set on the GPU, can advance it to the current time with the Hermite
+ * predictor ("optional prediction step on the j particles"; "4th order
+ * Hermite predictor-corrector"), and returns acceleration, jerk and potential for the i-particles
+ * it is given (j split in blocks + partial-force reduction).
+ * The paper prints no formula; the readings taken are R1..R16 in DESIGN.md section 3.
+ *
+ * Conventions for every entry point
+ *   - returns NB_OK (0) or a negative nb_status; never throws, aborts or prints.
+ *   - "DEVICE" pointers are CUDA device memory on the context's device, "HOST" pointers are
+ *     ordinary host memory.  The caller owns every array it passes; the library owns only the
+ *     context and its internal buffers.  Inputs are read, outputs written, on the context's
+ *     stream: a call returns once the work is enqueued (DEVICE variants) and results are valid
+ *     after the stream, or nb_sync, completes.  *_host variants return after the copy back.
+ *   - vectors are SoA fp64; indices are int32 (N < 2^31); eps2 is the SQUARE of the softening.
+ *   - a context is not thread-safe; use one per host thread or lock around it.
+ *   - sm_100 (compute capability 10.x) only: nb_create fails with NB_ERR_ARCH elsewhere.  There is
+ *     no CPU or other-GPU fallback.
+ */
+#ifndef NB_H
+#define NB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nb_ctx nb_ctx;   /* opaque; one per j-set */
+
+typedef enum {
+    NB_OK = 0,
+    NB_ERR_ARG = -1,     /* NULL pointer, negative count, range beyond n_max / ni_max, bad eps2 / t */
+    NB_ERR_ALLOC = -2,   /* device or pinned allocation failed, or lent workspace too small        */
+    NB_ERR_CUDA = -3,    /* a CUDA runtime call or kernel launch failed                             */
+    NB_ERR_INDEX = -4,   /* an i_list / idx entry was outside [0, n) (reported by nb_sync)          */
+    NB_ERR_STATE = -5,   /* nb_force before any nb_predict, or workspace set too late               */
+    NB_ERR_ARCH = -6     /* device is not compute capability 10.x                                   */
+} nb_status;
+
+/* ---- lifetime --------------------------------------------------------------------------- */
+
+/* Create a context for up to n_max j-particles and up to ni_max i-particles per force call, on
+ * CUDA device `device`, enqueuing on `stream` (a cudaStream_t passed as void*; NULL = legacy
+ * default stream).  Internal buffers (j-store 112 B, predicted state 48 B, packed force record
+ * 48 B per particle, plus the partial-force buffer) are allocated on first use with cudaMalloc,
+ * unless nb_set_workspace lent memory before that. */
+int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* stream);
+int nb_destroy(nb_ctx* c);
+int nb_set_stream(nb_ctx* c, void* stream);
+
+/* Bytes of device memory a context of this size needs; and lending them (DEVICE pointer, 256-byte
+ * aligned, must outlive the context) so that the caller's allocator owns all device memory.
+ * nb_set_workspace must precede the first nb_set_j / nb_predict; NB_ERR_STATE afterwards. */
+size_t nb_workspace_bytes(int64_t n_max, int64_t ni_max);
+int nb_set_workspace(nb_ctx* c, void* dev_ptr, size_t bytes);
+
+/* ---- a0: the resident j-set (PAPER.md:49 "j particles, which exert a force"; PAPER.md:55, :83:
+ * keep it on the device, update it sparsely) ----------------------------------------------- */
+
+/* Load/replace particles [first, first+count).  14 DEVICE fp64 arrays of length count: mass,
+ * position, velocity, acceleration, jerk (the predictor's inputs, R1) and the time t the state
+ * refers to.  ax..jz and t may each be NULL (taken as 0).  n becomes max(n, first+count);
+ * particles never written have m = 0 at the origin and exert nothing. */
+int nb_set_j(nb_ctx* c, int64_t first, int64_t count, const double* m,
+             const double* x, const double* y, const double* z,
+             const double* vx, const double* vy, const double* vz,
+             const double* ax, const double* ay, const double* az,
+             const double* jx, const double* jy, const double* jz, const double* t);
+
+/* Scatter form used after a block step: element k replaces particle idx[k] (DEVICE int32, each
+ * in [0, n); out-of-range entries are skipped and latch NB_ERR_INDEX; with duplicates one of the
+ * writers wins).  Same 14 arrays, same NULL rule (NULL = leave that field unchanged here). */
+int nb_update_j(nb_ctx* c, const int32_t* idx, int64_t count, const double* m,
+                const double* x, const double* y, const double* z,
+                const double* vx, const double* vy, const double* vz,
+                const double* ax, const double* ay, const double* az,
+                const double* jx, const double* jy, const double* jz, const double* t);
+
+/* HOST-pointer form of nb_set_j (pageable or pinned host memory; staged through the context's
+ * pinned buffer with cudaMemcpyAsync).  Same argument rules. */
+int nb_set_j_host(nb_ctx* c, int64_t first, int64_t count, const double* m,
+                  const double* x, const double* y, const double* z,
+                  const double* vx, const double* vy, const double* vz,
+                  const double* ax, const double* ay, const double* az,
+                  const double* jx, const double* jy, const double* jz, const double* t);
+
+int nb_clear(nb_ctx* c);            /* n := 0, flags cleared, "predicted" state invalidated */
+int64_t nb_count(const nb_ctx* c);  /* current n (or a negative nb_status)                  */
+
+/* Mark particles whose MUTUAL pairs are unsoftened (R7: eps2_ij = 0 iff both carry bit 0; e.g.
+ * black holes).  idx, flags: HOST arrays of length count (the flagged set is
+ * small and changes rarely); replaces the flag of each listed particle.  At most NB_MAX_FLAGGED
+ * particles may carry the bit at one time (NB_ERR_ARG beyond). */
+#define NB_MAX_FLAGGED 1024
+int nb_set_flags(nb_ctx* c, const int32_t* idx, const uint8_t* flags, int64_t count);
+
+/* ---- a1: Hermite predictor (R1) --------------------------------------------- */
+
+/* For all n particles: dt = t - t_j; xp = x + v dt + a dt^2/2 + jerk dt^3/6; vp = v + a dt +
+ * jerk dt^2/2, in fp64, written to the internal predicted buffers (fp64 SoA, and the packed
+ * record the force kernel streams).  t must be finite. */
+int nb_predict(nb_ctx* c, double t);
+
+/* Copy predicted state of particles [first, first+count) to a DEVICE fp64 buffer laid out
+ * [6][count]: xp, yp, zp, vxp, vyp, vzp.  NB_ERR_STATE before the first nb_predict. */
+int nb_get_predicted(nb_ctx* c, int64_t first, int64_t count, double* out);
+
+/* ---- a2..a5: force call (R2..R9) ------------------------------ */
+
+/* acc, jerk, pot on particles i_list[0..ni) (DEVICE int32 indices into the j-set; duplicates are
+ * legal; unsorted is fine) from all n j-particles, both taken at their predicted state of the last
+ * nb_predict:
+ *     r = xp_j - xp_i, w = vp_j - vp_i, s = r.r + eps2_ij         (j != i by index, R5)
+ *     pot_i = - sum m_j s^-1/2 ;  acc_i = sum m_j r s^-3/2 ;
+ *     jrk_i = sum m_j ( w s^-3/2 - 3 (r.w) r s^-5/2 )             (s == 0 contributes nothing, R6)
+ * Outputs, DEVICE fp64, in i_list order: acc[0..ni) = ax, acc[ni..2ni) = ay, acc[2ni..3ni) = az;
+ * jrk likewise; pot[0..ni).  Precision: position differences carry >= 48 bits, pair terms are
+ * fp32, sums are fp64; results agree with exact summation to
+ * <= 1e-5 (acc, pot) and <= 1e-4 (jerk) relative per particle.  Deterministic run to run.
+ * eps2 must be finite and >= 0; ni in [0, ni_max].  An out-of-range i_list entry gets NaN
+ * outputs and latches NB_ERR_INDEX (returned by the next nb_sync). */
+int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
+             double* acc, double* jrk, double* pot);
+
+/* HOST-pointer form: i_list, acc, jrk, pot are host arrays; copies in, runs, copies back and
+ * synchronises the stream before returning (so it also returns latched errors). */
+int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
+                  double* acc, double* jrk, double* pot);
+
+/* ---- control ------------------------------------------------------------------------------ */
+
+/* Force-call tuning, for tests and experiments.  j_splits: 0 = let the dispatcher choose the
+ * number of j-subsets, >0 = use exactly this many (clamped to what the partial
+ * buffer holds).  reduce_mode: 0 = partial buffer + reduction kernel (deterministic;
+ * default), 1 = fp64 atomics into the output (sum order varies run to run). */
+int nb_set_tuning(nb_ctx* c, int j_splits, int reduce_mode);
+
+/* What the last nb_force launched: out[0] = j-splits used, out[1] = CTAs of the pair kernel,
+ * out[2] = kernels launched by the call, out[3] = kernel variant id.  HOST int64[4]. */
+int nb_last_launch(const nb_ctx* c, int64_t* out);
+
+/* Total kernels this context has launched since creation (bench.py's gpu_launches). */
+int64_t nb_launch_count(const nb_ctx* c);
+
+int nb_sync(nb_ctx* c);                 /* stream sync; returns and clears any latched error */
+const char* nb_strerror(int status);
+const char* nb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NB_H */
