@@ -1,0 +1,190 @@
+"""ctypes binding of libnb.so (include/nb.h): same names, argument marshalling only.
+
+torch supplies device memory (`tensor.data_ptr()`) and the stream; every step of the path runs in
+the library's sm_100a kernels.  There is no fallback: importing this module without a built
+libnb.so raises, and `nb_create` fails on anything that is not a compute-capability-10.x GPU.
+"""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnb.so")
+
+NB_OK, NB_ERR_ARG, NB_ERR_ALLOC, NB_ERR_CUDA = 0, -1, -2, -3
+NB_ERR_INDEX, NB_ERR_STATE, NB_ERR_ARCH = -4, -5, -6
+NB_MAX_FLAGGED = 1024
+
+EXPORTS = [
+    "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
+    "nb_set_j", "nb_update_j", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
+    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_host", "nb_set_tuning",
+    "nb_last_launch", "nb_launch_count", "nb_sync", "nb_strerror", "nb_version",
+]
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        "paper_1409_5474_b200/libnb.so is missing: build it with "
+        "`python -c 'import __graft_entry__ as g; g.build()'` (needs nvcc). There is no fallback.")
+
+lib = ctypes.CDLL(LIB_PATH)
+
+_vp, _i64, _i32, _dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+lib.nb_create.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _i32, _vp]
+lib.nb_destroy.argtypes = [_vp]
+lib.nb_set_stream.argtypes = [_vp, _vp]
+lib.nb_workspace_bytes.argtypes = [_i64, _i64]
+lib.nb_workspace_bytes.restype = ctypes.c_size_t
+lib.nb_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
+for _f in (lib.nb_set_j, lib.nb_set_j_host):
+    _f.argtypes = [_vp, _i64, _i64] + [_vp] * 14
+lib.nb_update_j.argtypes = [_vp, _vp, _i64] + [_vp] * 14
+lib.nb_clear.argtypes = [_vp]
+lib.nb_count.argtypes = [_vp]
+lib.nb_count.restype = _i64
+lib.nb_set_flags.argtypes = [_vp, _vp, _vp, _i64]
+lib.nb_predict.argtypes = [_vp, _dbl]
+lib.nb_get_predicted.argtypes = [_vp, _i64, _i64, _vp]
+for _f in (lib.nb_force, lib.nb_force_host):
+    _f.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _vp]
+lib.nb_set_tuning.argtypes = [_vp, _i32, _i32]
+lib.nb_last_launch.argtypes = [_vp, ctypes.POINTER(_i64)]
+lib.nb_launch_count.argtypes = [_vp]
+lib.nb_launch_count.restype = _i64
+lib.nb_sync.argtypes = [_vp]
+lib.nb_strerror.argtypes = [_i32]
+lib.nb_strerror.restype = ctypes.c_char_p
+lib.nb_version.restype = ctypes.c_char_p
+
+
+class NBError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__("%s: %s (%d)" % (where, lib.nb_strerror(status).decode(), status))
+
+
+def _check(status, where):
+    if status != NB_OK:
+        raise NBError(status, where)
+
+
+def _ptr(a):
+    """Address of a torch tensor / numpy array / None / int."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if hasattr(a, "data_ptr"):
+        return a.data_ptr()
+    return a.ctypes.data
+
+
+def nb_version():
+    return lib.nb_version().decode()
+
+
+def nb_strerror(status):
+    return lib.nb_strerror(status).decode()
+
+
+def nb_workspace_bytes(n_max, ni_max):
+    return int(lib.nb_workspace_bytes(n_max, ni_max))
+
+
+def nb_create(n_max, ni_max, device=0, stream=None):
+    h = _vp()
+    _check(lib.nb_create(ctypes.byref(h), n_max, ni_max, device, stream), "nb_create")
+    return h
+
+
+def nb_destroy(c):
+    _check(lib.nb_destroy(c), "nb_destroy")
+
+
+def nb_set_stream(c, stream):
+    _check(lib.nb_set_stream(c, stream), "nb_set_stream")
+
+
+def nb_set_workspace(c, dev_ptr, nbytes):
+    _check(lib.nb_set_workspace(c, _ptr(dev_ptr), nbytes), "nb_set_workspace")
+
+
+def _fields(m, x, v, a, j, t):
+    """14 pointers from m (N,), x, v, a, j (3, N) row-contiguous (or None), t (N,) (or None)."""
+    def rows(q):
+        if q is None:
+            return [None] * 3
+        assert q.shape[0] == 3 and _contig(q)
+        esz = q.element_size() if hasattr(q, "element_size") else q.itemsize
+        return [_ptr(q) + r * q.shape[1] * esz for r in range(3)]
+    return [_ptr(m)] + rows(x) + rows(v) + rows(a) + rows(j) + [_ptr(t)]
+
+
+def _contig(q):
+    return q.is_contiguous() if hasattr(q, "is_contiguous") else q.flags["C_CONTIGUOUS"]
+
+
+def nb_set_j(c, first, count, m, x, v, a=None, j=None, t=None):
+    """DEVICE tensors: m (count,), x, v, a, j (3, count) fp64 contiguous, t (count,)."""
+    _check(lib.nb_set_j(c, first, count, *_fields(m, x, v, a, j, t)), "nb_set_j")
+
+
+def nb_set_j_host(c, first, count, m, x, v, a=None, j=None, t=None):
+    """HOST arrays (numpy or CPU torch tensors, ideally pinned), same shapes as nb_set_j."""
+    _check(lib.nb_set_j_host(c, first, count, *_fields(m, x, v, a, j, t)), "nb_set_j_host")
+
+
+def nb_update_j(c, idx, count, m, x, v, a=None, j=None, t=None):
+    _check(lib.nb_update_j(c, _ptr(idx), count, *_fields(m, x, v, a, j, t)), "nb_update_j")
+
+
+def nb_clear(c):
+    _check(lib.nb_clear(c), "nb_clear")
+
+
+def nb_count(c):
+    return int(lib.nb_count(c))
+
+
+def nb_set_flags(c, idx, flags):
+    """idx: host int32 array, flags: host uint8 array (numpy)."""
+    import numpy as np
+    idx = np.ascontiguousarray(idx, np.int32)
+    flags = np.ascontiguousarray(flags, np.uint8)
+    assert idx.shape == flags.shape
+    _check(lib.nb_set_flags(c, idx.ctypes.data, flags.ctypes.data, idx.shape[0]), "nb_set_flags")
+
+
+def nb_predict(c, t):
+    _check(lib.nb_predict(c, float(t)), "nb_predict")
+
+
+def nb_get_predicted(c, first, count, out):
+    _check(lib.nb_get_predicted(c, first, count, _ptr(out)), "nb_get_predicted")
+
+
+def nb_force(c, i_list, ni, eps2, acc, jrk, pot):
+    """DEVICE: i_list int32 (ni,), acc, jrk fp64 (3, ni), pot fp64 (ni,) -- outputs."""
+    _check(lib.nb_force(c, _ptr(i_list), ni, float(eps2), _ptr(acc), _ptr(jrk), _ptr(pot)), "nb_force")
+
+
+def nb_force_host(c, i_list, ni, eps2, acc, jrk, pot):
+    _check(lib.nb_force_host(c, _ptr(i_list), ni, float(eps2), _ptr(acc), _ptr(jrk), _ptr(pot)),
+           "nb_force_host")
+
+
+def nb_set_tuning(c, j_splits=0, reduce_mode=0):
+    _check(lib.nb_set_tuning(c, j_splits, reduce_mode), "nb_set_tuning")
+
+
+def nb_last_launch(c):
+    out = (_i64 * 4)()
+    _check(lib.nb_last_launch(c, out), "nb_last_launch")
+    return {"j_splits": out[0], "ctas": out[1], "kernels": out[2], "variant": out[3]}
+
+
+def nb_launch_count(c):
+    return int(lib.nb_launch_count(c))
+
+
+def nb_sync(c):
+    _check(lib.nb_sync(c), "nb_sync")

@@ -1,0 +1,88 @@
+"""Convenience wrapper: one nb context + torch-allocated outputs.  Marshalling only."""
+import torch
+
+from . import binding as nb
+
+
+class Context:
+    def __init__(self, n_max, ni_max=None, device=0, stream=None):
+        self.device = torch.device("cuda", device)
+        self.n_max = int(n_max)
+        self.ni_max = int(ni_max if ni_max is not None else n_max)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        self.h = nb.nb_create(self.n_max, self.ni_max, device, stream)
+
+    def close(self):
+        if self.h is not None:
+            nb.nb_destroy(self.h)
+            self.h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- j-set ------------------------------------------------------------------------------
+    def _dev(self, q, dtype=torch.float64):
+        if q is None:
+            return None
+        return torch.as_tensor(q, dtype=dtype).to(self.device).contiguous()
+
+    def set_j(self, m, x, v, a=None, j=None, t=None, first=0):
+        """Arrays of any kind (numpy / torch, host or device); copied to the device by torch,
+        then handed to nb_set_j as device pointers."""
+        d = [self._dev(q) for q in (m, x, v, a, j, t)]
+        nb.nb_set_j(self.h, first, d[0].shape[0], *d)
+        self._keep = d   # alive until the stream has consumed them
+
+    def update_j(self, idx, m, x, v, a=None, j=None, t=None):
+        i = self._dev(idx, torch.int32)
+        d = [self._dev(q) for q in (m, x, v, a, j, t)]
+        nb.nb_update_j(self.h, i, i.shape[0], *d)
+        self._keep = [i] + d
+
+    def load_case(self, case):
+        self.set_j(case.m, case.x, case.v, case.a, case.j, case.t)
+        fl = case.flags.nonzero()[0]
+        if fl.size:
+            nb.nb_set_flags(self.h, fl, case.flags[fl])
+
+    def set_flags(self, idx, flags):
+        nb.nb_set_flags(self.h, idx, flags)
+
+    # -- predictor / force --------------------------------------------------------------------
+    def predict(self, t):
+        nb.nb_predict(self.h, t)
+
+    def predicted(self, first=0, count=None):
+        count = nb.nb_count(self.h) - first if count is None else count
+        out = torch.empty((6, count), dtype=torch.float64, device=self.device)
+        nb.nb_get_predicted(self.h, first, count, out)
+        return out[:3], out[3:]
+
+    def force(self, i_list, eps2):
+        il = self._dev(i_list, torch.int32)
+        ni = il.shape[0]
+        acc = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        jrk = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
+        nb.nb_force(self.h, il, ni, eps2, acc, jrk, pot)
+        self._keep_i = il
+        return acc, jrk, pot
+
+    def tuning(self, j_splits=0, reduce_mode=0):
+        nb.nb_set_tuning(self.h, j_splits, reduce_mode)
+
+    def last_launch(self):
+        return nb.nb_last_launch(self.h)
+
+    def sync(self):
+        nb.nb_sync(self.h)

@@ -1,0 +1,396 @@
+// force.cu -- a2..a5: i-gather, pair loop, j-split partials, reduction.
+//
+// Mapping.  A CTA of 128 threads owns ITILE = 256 active i-particles (two
+// per thread, held in registers as negated, lane-duplicated f32x2 values) and one of S j-subsets
+// (PAPER.md:51).  It streams its j-tiles (TJ = 128 particles, 5632 B, SoA inside the tile) from
+// L2/HBM into a 4-deep shared-memory ring with 1-D bulk async copies (TMA unit, cp.async.bulk)
+// completing on mbarriers; no thread spends issue slots on the copy.  Two consecutive j's form the
+// two lanes of every packed FP32 instruction (fma/add/mul .f32x2), so one issue slot serves two
+// pair interactions; per interaction the FP32 pipe executes 33 lane-ops (9 for the two-float
+// position difference) plus one MUFU.RSQ.  fp32 partial sums run over one tile (64
+// terms per lane) and are then flushed to fp64 registers.  The self pair and flagged-flagged pairs
+// are masked only in the tiles that contain them (warp-uniform slow path), so the common tile pays
+// nothing for R5/R7.  No tensor cores: the pair kernel with its reciprocal square root is not a
+// contraction.
+#include "nb_internal.h"
+
+namespace nb {
+
+namespace {
+
+// ---- PTX helpers: mbarrier + 1-D bulk async copy ---------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+        "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ float rsqrt_fast(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+struct IPart {            // one i-particle, negated and duplicated over both f32x2 lanes
+    float2 nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz;
+};
+struct Acc32 {            // per-tile fp32 sums, lane 0 = even j, lane 1 = odd j
+    float2 ax, ay, az, jx, jy, jz, p;
+};
+
+__device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
+
+// One i against one pair of j's: 13 FADD2 + 14 FFMA2 + 6 FMUL2 + 2 MUFU (R2, R17).
+__device__ __forceinline__ void pair2(const IPart& I, Acc32& A, float2 xh, float2 yh, float2 zh,
+                                      float2 xl, float2 yl, float2 zl, float2 vx, float2 vy,
+                                      float2 vz, float2 m, float2 eps2, float2 m3)
+{
+    const float2 dx = __fadd2_rn(__fadd2_rn(xh, I.nxh), __fadd2_rn(xl, I.nxl));
+    const float2 dy = __fadd2_rn(__fadd2_rn(yh, I.nyh), __fadd2_rn(yl, I.nyl));
+    const float2 dz = __fadd2_rn(__fadd2_rn(zh, I.nzh), __fadd2_rn(zl, I.nzl));
+    const float2 wx = __fadd2_rn(vx, I.nvx);
+    const float2 wy = __fadd2_rn(vy, I.nvy);
+    const float2 wz = __fadd2_rn(vz, I.nvz);
+    float2 r2 = __ffma2_rn(dx, dx, eps2);
+    r2 = __ffma2_rn(dy, dy, r2);
+    r2 = __ffma2_rn(dz, dz, r2);
+    float2 rinv;
+    rinv.x = rsqrt_fast(r2.x);
+    rinv.y = rsqrt_fast(r2.y);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 mr = __fmul2_rn(m, rinv);
+    const float2 mr3 = __fmul2_rn(mr, rinv2);
+    float2 rv = __fmul2_rn(dx, wx);
+    rv = __ffma2_rn(dy, wy, rv);
+    rv = __ffma2_rn(dz, wz, rv);
+    const float2 al = __fmul2_rn(__fmul2_rn(rinv2, m3), rv);      // -3 (r.w) / s
+    A.p = __fadd2_rn(A.p, mr);
+    A.ax = __ffma2_rn(mr3, dx, A.ax);
+    A.ay = __ffma2_rn(mr3, dy, A.ay);
+    A.az = __ffma2_rn(mr3, dz, A.az);
+    A.jx = __ffma2_rn(mr3, __ffma2_rn(al, dx, wx), A.jx);
+    A.jy = __ffma2_rn(mr3, __ffma2_rn(al, dy, wy), A.jy);
+    A.jz = __ffma2_rn(mr3, __ffma2_rn(al, dz, wz), A.jz);
+}
+
+// Masked scalar pair for the rare tiles that hold the i-particle itself, a flagged partner of a
+// flagged i, or when eps2 == 0 (R5, R6, R7): a skipped pair gets rinv = 0, i.e. contributes nothing.
+__device__ __forceinline__ void pair1_masked(const IPart& I, Acc32& A, const float* T, int p,
+                                             bool skip_self, bool iflag, float eps2)
+{
+    const float dx = (T[P_XH * TJ + p] + I.nxh.x) + (T[P_XL * TJ + p] + I.nxl.x);
+    const float dy = (T[P_YH * TJ + p] + I.nyh.x) + (T[P_YL * TJ + p] + I.nyl.x);
+    const float dz = (T[P_ZH * TJ + p] + I.nzh.x) + (T[P_ZL * TJ + p] + I.nzl.x);
+    const float wx = T[P_VX * TJ + p] + I.nvx.x;
+    const float wy = T[P_VY * TJ + p] + I.nvy.x;
+    const float wz = T[P_VZ * TJ + p] + I.nvz.x;
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+    const bool jflag = (__float_as_uint(T[P_FLAG * TJ + p]) & 1u) != 0;
+    const bool skip = skip_self || (iflag && jflag) || !(r2 > 0.0f);
+    const float rinv = skip ? 0.0f : rsqrt_fast(r2);
+    const float rinv2 = rinv * rinv;
+    const float mr = T[P_M * TJ + p] * rinv;
+    const float mr3 = mr * rinv2;
+    const float rv = fmaf(dz, wz, fmaf(dy, wy, dx * wx));
+    const float al = (rinv2 * -3.0f) * rv;
+    A.p.x += mr;
+    A.ax.x = fmaf(mr3, dx, A.ax.x);
+    A.ay.x = fmaf(mr3, dy, A.ay.x);
+    A.az.x = fmaf(mr3, dz, A.az.x);
+    A.jx.x = fmaf(mr3, fmaf(al, dx, wx), A.jx.x);
+    A.jy.x = fmaf(mr3, fmaf(al, dy, wy), A.jy.x);
+    A.jz.x = fmaf(mr3, fmaf(al, dz, wz), A.jz.x);
+}
+
+__device__ __forceinline__ void flush(Acc32& A, double* d)
+{
+    d[0] += (double)(A.ax.x + A.ax.y);
+    d[1] += (double)(A.ay.x + A.ay.y);
+    d[2] += (double)(A.az.x + A.az.y);
+    d[3] += (double)(A.jx.x + A.jx.y);
+    d[4] += (double)(A.jy.x + A.jy.y);
+    d[5] += (double)(A.jz.x + A.jz.y);
+    d[6] -= (double)(A.p.x + A.p.y);
+    A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.p = make_float2(0.f, 0.f);
+}
+
+template <bool ATOMIC>
+__global__ void __launch_bounds__(FORCE_THREADS, 3)
+force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
+             double* __restrict__ opot)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* tiles = reinterpret_cast<float*>(smem_raw);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STAGES * TILE_BYTES);
+
+    const int tid = threadIdx.x;
+    const int it = blockIdx.x % P.n_itiles;       // neighbouring CTAs share the j-subset (L2 reuse)
+    const int sp = blockIdx.x / P.n_itiles;
+    const int t0 = (int)(((int64_t)P.ntiles * sp) / P.splits);
+    const int t1 = (int)(((int64_t)P.ntiles * (sp + 1)) / P.splits);
+
+    // a4: the j-subset of this CTA is tiles [t0, t1).  Thread 0 runs the copy ring.
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&bars[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int s = 0; s < STAGES && t0 + s < t1; ++s) {
+            mbar_expect_tx(smem_u32(&bars[s]), TILE_BYTES);
+            bulk_g2s(smem_u32(tiles + s * TILE_FLOATS), P.pack + (int64_t)(t0 + s) * TILE_FLOATS,
+                     TILE_BYTES, smem_u32(&bars[s]));
+        }
+    }
+
+    // a2: i-gather from the pack (two-float position = 48 bits, fp32 velocity; R8, R17)
+    IPart I[IPT];
+    int idx[IPT];
+    bool iflag[IPT];
+    int k[IPT];
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        k[u] = it * ITILE + u * FORCE_THREADS + tid;
+        int q = (k[u] < P.ni) ? P.i_list[k[u]] : 0;
+        const bool bad = (q < 0) || (q >= P.n);
+        if (bad) {
+            atomicOr(P.err, 1);
+            q = 0;
+        }
+        idx[u] = (k[u] < P.ni && !bad) ? q : -1;
+        const float* b = P.pack + (int64_t)(q / TJ) * TILE_FLOATS + (q % TJ);
+        I[u].nxh = dup(-b[P_XH * TJ]); I[u].nyh = dup(-b[P_YH * TJ]); I[u].nzh = dup(-b[P_ZH * TJ]);
+        I[u].nxl = dup(-b[P_XL * TJ]); I[u].nyl = dup(-b[P_YL * TJ]); I[u].nzl = dup(-b[P_ZL * TJ]);
+        I[u].nvx = dup(-b[P_VX * TJ]); I[u].nvy = dup(-b[P_VY * TJ]); I[u].nvz = dup(-b[P_VZ * TJ]);
+        iflag[u] = P.any_flagged && (P.flags[q] & 1);
+    }
+
+    const float2 eps2 = dup(P.eps2);
+    const float2 m3 = dup(-3.0f);
+    const bool eps0 = !(P.eps2 > 0.0f);
+    Acc32 A[IPT];
+    double D[IPT][NOUT];
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < NOUT; ++c) D[u][c] = 0.0;
+    }
+    __syncthreads();   // barrier inits visible to all waiters
+
+    // a3: pair loop over the tiles of the subset
+    for (int t = t0; t < t1; ++t) {
+        const int st = (t - t0) % STAGES;
+        mbar_wait(smem_u32(&bars[st]), ((t - t0) / STAGES) & 1);
+        const float* T = tiles + st * TILE_FLOATS;
+
+        bool slow = eps0;
+#pragma unroll
+        for (int u = 0; u < IPT; ++u) {
+            slow |= (idx[u] >= t * TJ) && (idx[u] < (t + 1) * TJ);
+            if (iflag[u]) slow |= (P.tileflag[t >> 5] >> (t & 31)) & 1u;
+        }
+        if (!__any_sync(0xffffffffu, slow)) {
+#pragma unroll 2
+            for (int p = 0; p < TJ; p += 4) {
+                float4 f[10];
+#pragma unroll
+                for (int c = 0; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+                    pair2(I[u], A[u], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
+                          make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y),
+                          make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                          make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y),
+                          make_float2(f[8].x, f[8].y), make_float2(f[9].x, f[9].y), eps2, m3);
+                    pair2(I[u], A[u], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w),
+                          make_float2(f[2].z, f[2].w), make_float2(f[3].z, f[3].w),
+                          make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                          make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w),
+                          make_float2(f[8].z, f[8].w), make_float2(f[9].z, f[9].w), eps2, m3);
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int p = 0; p < TJ; ++p) {
+#pragma unroll
+                for (int u = 0; u < IPT; ++u)
+                    pair1_masked(I[u], A[u], T, p, idx[u] == t * TJ + p, iflag[u], P.eps2);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < IPT; ++u) flush(A[u], D[u]);
+
+        __syncthreads();   // every warp is done with this stage: refill it
+        if (tid == 0 && t + STAGES < t1) {
+            mbar_expect_tx(smem_u32(&bars[st]), TILE_BYTES);
+            bulk_g2s(smem_u32(tiles + st * TILE_FLOATS), P.pack + (int64_t)(t + STAGES) * TILE_FLOATS,
+                     TILE_BYTES, smem_u32(&bars[st]));
+        }
+    }
+
+    // a4: partial sums of this j-subset (second kernel adds them), or atomics (:63)
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        if (ATOMIC) {
+            if (idx[u] >= 0) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    atomicAdd(oacc + (int64_t)c * P.ni + k[u], D[u][c]);
+                    atomicAdd(ojrk + (int64_t)c * P.ni + k[u], D[u][3 + c]);
+                }
+                atomicAdd(opot + k[u], D[u][6]);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < NOUT; ++c)
+                P.part[((int64_t)sp * NOUT + c) * P.ni_pad + k[u]] = D[u][c];
+        }
+    }
+}
+
+// a4/a5: sum the S partials in a fixed order (deterministic), add the unsoftened flagged-flagged
+// pair terms in fp64 straight from the j-store (R7), NaN for rejected indices, store SoA.
+__global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= R.ni) return;
+    double o[NOUT];
+    if (R.atomic_mode) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            o[c] = R.acc[(int64_t)c * R.ni + k];
+            o[3 + c] = R.jrk[(int64_t)c * R.ni + k];
+        }
+        o[6] = R.pot[k];
+    } else {
+#pragma unroll
+        for (int c = 0; c < NOUT; ++c) o[c] = 0.0;
+        for (int s = 0; s < R.splits; ++s) {
+#pragma unroll
+            for (int c = 0; c < NOUT; ++c) o[c] += R.part[((int64_t)s * NOUT + c) * R.ni_pad + k];
+        }
+    }
+    const int i = R.i_list[k];
+    if (i < 0 || i >= R.n) {
+#pragma unroll
+        for (int c = 0; c < NOUT; ++c) o[c] = __longlong_as_double(0x7ff8000000000000LL);
+    } else if (R.nflag > 1 && (R.flags[i] & 1)) {
+        double xi[3], vi[3];
+        const double dti = R.t_pred - R.store.f[F_T][i];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            predict1(R.store.f[F_X + c][i], R.store.f[F_VX + c][i], R.store.f[F_AX + c][i],
+                     R.store.f[F_JX + c][i], dti, xi[c], vi[c]);
+        for (int q = 0; q < R.nflag; ++q) {
+            const int j = R.flag_list[q];
+            if (j == i) continue;
+            double r[3], w[3];
+            const double dtj = R.t_pred - R.store.f[F_T][j];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                double xj, vj;
+                predict1(R.store.f[F_X + c][j], R.store.f[F_VX + c][j], R.store.f[F_AX + c][j],
+                         R.store.f[F_JX + c][j], dtj, xj, vj);
+                r[c] = xj - xi[c];
+                w[c] = vj - vi[c];
+            }
+            const double s2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+            if (s2 == 0.0) continue;
+            const double rinv = 1.0 / sqrt(s2), rinv2 = rinv * rinv;
+            const double mr = R.store.f[F_M][j] * rinv, mr3 = mr * rinv2;
+            const double b = 3.0 * (r[0] * w[0] + r[1] * w[1] + r[2] * w[2]) * rinv2;
+            o[6] -= mr;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                o[c] += mr3 * r[c];
+                o[3 + c] += mr3 * (w[c] - b * r[c]);
+            }
+        }
+    } else if (R.atomic_mode) {
+        return;   // sums are already in place
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        R.acc[(int64_t)c * R.ni + k] = o[c];
+        R.jrk[(int64_t)c * R.ni + k] = o[3 + c];
+    }
+    R.pot[k] = o[6];
+}
+
+__global__ void __launch_bounds__(256) zero_out_kernel(double* acc, double* jrk, double* pot, int64_t ni)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= ni) return;
+    for (int c = 0; c < 3; ++c) {
+        acc[c * ni + k] = 0.0;
+        jrk[c * ni + k] = 0.0;
+    }
+    pot[k] = 0.0;
+}
+
+constexpr int FORCE_SMEM = STAGES * TILE_BYTES + STAGES * 8;
+
+}  // namespace
+
+cudaError_t force_kernel_setup(int* blocks_per_sm)
+{
+    cudaError_t e = cudaFuncSetAttribute(force_kernel<false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, FORCE_SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(force_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             FORCE_SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, force_kernel<false>,
+                                                         FORCE_THREADS, FORCE_SMEM);
+}
+
+cudaError_t launch_force(const ForceArgs& a, int atomic_mode, double* acc, double* jrk, double* pot,
+                         cudaStream_t s)
+{
+    const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
+    if (atomic_mode)
+        force_kernel<true><<<grid, FORCE_THREADS, FORCE_SMEM, s>>>(a, acc, jrk, pot);
+    else
+        force_kernel<false><<<grid, FORCE_THREADS, FORCE_SMEM, s>>>(a, acc, jrk, pot);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s)
+{
+    reduce_kernel<<<(a.ni + 127) / 128, 128, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s)
+{
+    zero_out_kernel<<<(unsigned)((ni + 255) / 256), 256, 0, s>>>(acc, jrk, pot, ni);
+    return cudaGetLastError();
+}
+
+}  // namespace nb

@@ -1,0 +1,533 @@
+// nb_api.cu -- the C-ABI of include/nb.h: context, argument checks, host dispatcher.
+#include <math.h>
+#include <new>
+#include <string.h>
+#include <vector>
+
+#include "nb_internal.h"
+
+using namespace nb;
+
+struct nb_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int64_t n_max = 0, ni_max = 0, n_cap = 0, n = 0;
+    int sm_count = 148, blocks_per_sm = 1;
+
+    // device memory: either one cudaMalloc'ed slab or the caller's workspace
+    bool allocated = false, own_slab = false;
+    unsigned char* slab = nullptr;
+    size_t lent_bytes = 0;
+    StorePtrs store{};
+    float* pack = nullptr;
+    uint8_t* flags = nullptr;
+    uint32_t* tileflag = nullptr;
+    int32_t* flag_list = nullptr;
+    double* part = nullptr;
+    size_t part_bytes = 0;
+    int* err = nullptr;
+    int32_t* h_ilist = nullptr;   // device staging for the *_host force call
+    double* h_out = nullptr;      // [7][ni_max]
+
+    int* err_pinned = nullptr;
+    std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
+
+    bool predicted = false;
+    double t_pred = 0.0;
+    int tune_splits = 0, tune_reduce = 0;
+    int64_t last[4] = {0, 0, 0, 0};
+    int64_t launches = 0;
+};
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t store, pack, flags, tileflag, flag_list, part, err, ilist, out, total;
+    size_t part_bytes;
+    int64_t n_cap;
+};
+
+Layout layout(int64_t n_max, int64_t ni_max)
+{
+    Layout L{};
+    L.n_cap = (int64_t)up((size_t)(n_max > 0 ? n_max : 1), 2 * TJ);
+    const int64_t ntiles = L.n_cap / TJ;
+    const int64_t ni_pad = (int64_t)up((size_t)(ni_max > 0 ? ni_max : 1), ITILE);
+    size_t off = 0;
+    L.store = off; off += up((size_t)NFIELD * L.n_cap * sizeof(double));
+    L.pack = off; off += up((size_t)ntiles * TILE_BYTES);
+    L.flags = off; off += up((size_t)L.n_cap);
+    L.tileflag = off; off += up((size_t)(ntiles + 31) / 32 * 4);
+    L.flag_list = off; off += up((size_t)NB_MAX_FLAGGED * 4);
+    // partial sums: S * 7 * ni_pad doubles.  S = 1 needs 56 B per i; small i-sets want many splits.
+    L.part_bytes = (size_t)NOUT * sizeof(double) * (size_t)ni_pad * 2;
+    if (L.part_bytes < ((size_t)32 << 20)) L.part_bytes = (size_t)32 << 20;
+    L.part = off; off += up(L.part_bytes);
+    L.err = off; off += up(sizeof(int));
+    L.ilist = off; off += up((size_t)ni_pad * 4);
+    L.out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
+    L.total = off;
+    return L;
+}
+
+int ensure_alloc(nb_ctx* c)
+{
+    if (c->allocated) return NB_OK;
+    const Layout L = layout(c->n_max, c->ni_max);
+    if (c->slab) {
+        if (c->lent_bytes < L.total) return NB_ERR_ALLOC;
+    } else {
+        if (cudaMalloc(&c->slab, L.total) != cudaSuccess) {
+            cudaGetLastError();
+            c->slab = nullptr;
+            return NB_ERR_ALLOC;
+        }
+        c->own_slab = true;
+    }
+    // zero the store (never-written particles are m = 0 at the origin), flags and the latch
+    if (cudaMemsetAsync(c->slab, 0, L.total, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    c->n_cap = L.n_cap;
+    for (int f = 0; f < NFIELD; ++f)
+        c->store.f[f] = reinterpret_cast<double*>(c->slab + L.store) + (size_t)f * L.n_cap;
+    c->pack = reinterpret_cast<float*>(c->slab + L.pack);
+    c->flags = c->slab + L.flags;
+    c->tileflag = reinterpret_cast<uint32_t*>(c->slab + L.tileflag);
+    c->flag_list = reinterpret_cast<int32_t*>(c->slab + L.flag_list);
+    c->part = reinterpret_cast<double*>(c->slab + L.part);
+    c->part_bytes = L.part_bytes;
+    c->err = reinterpret_cast<int*>(c->slab + L.err);
+    c->h_ilist = reinterpret_cast<int32_t*>(c->slab + L.ilist);
+    c->h_out = reinterpret_cast<double*>(c->slab + L.out);
+    c->allocated = true;
+    return NB_OK;
+}
+
+inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NB_OK : NB_ERR_CUDA; }
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        cudaGetDevice(&prev);
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+SrcPtrs make_src(const double* m, const double* x, const double* y, const double* z,
+                 const double* vx, const double* vy, const double* vz, const double* ax,
+                 const double* ay, const double* az, const double* jx, const double* jy,
+                 const double* jz, const double* t)
+{
+    SrcPtrs s;
+    const double* a[NFIELD] = {m, x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz, t};
+    for (int f = 0; f < NFIELD; ++f) s.f[f] = a[f];
+    return s;
+}
+
+// choose the number of j-subsets S so that (i-tiles x S) fills the chip.  Efficiency
+// of a choice = useful tile-passes / (waves x resident CTAs x tiles per CTA).
+int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad)
+{
+    const int64_t resident = (int64_t)c->sm_count * c->blocks_per_sm;
+    int64_t smax = (int64_t)(c->part_bytes / (NOUT * sizeof(double) * (size_t)ni_pad));
+    if (smax > ntiles) smax = ntiles;
+    if (smax > 4096) smax = 4096;
+    if (smax < 1) smax = 1;
+    if (c->tune_splits > 0) return (int)(c->tune_splits < smax ? c->tune_splits : smax);
+    int best = 1;
+    double best_eff = -1.0;
+    for (int64_t s = 1; s <= smax; ++s) {
+        const int64_t ctas = (int64_t)n_itiles * s;
+        const int64_t waves = (ctas + resident - 1) / resident;
+        const int64_t per = (ntiles + s - 1) / s;
+        // each CTA also pays a fixed cost of about two tiles (gather, pipeline fill, partial store)
+        const double eff = (double)n_itiles * ntiles / ((double)waves * resident * (per + 2));
+        if (eff > best_eff * 1.02) {   // prefer fewer splits unless clearly better
+            best_eff = eff;
+            best = (int)s;
+        }
+    }
+    return best;
+}
+
+int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc, double* jrk,
+               double* pot)
+{
+    if (!c->predicted) return NB_ERR_STATE;
+    c->last[0] = c->last[1] = c->last[2] = 0;
+    if (ni == 0) return NB_OK;
+    const int64_t n_launch = c->n > 0 ? c->n : 0;
+    ForceArgs a{};
+    a.pack = c->pack;
+    a.i_list = i_list;
+    a.part = c->part;
+    a.flags = c->flags;
+    a.tileflag = c->tileflag;
+    a.err = c->err;
+    a.ni = (int)ni;
+    a.n_itiles = (int)((ni + ITILE - 1) / ITILE);
+    a.ni_pad = a.n_itiles * ITILE;
+    a.n = (int)n_launch;
+    a.ntiles = (int)((n_launch + TJ - 1) / TJ);
+    a.eps2 = (float)eps2;
+    a.any_flagged = c->flagged.empty() ? 0 : 1;
+    const int mode = c->tune_reduce ? 1 : 0;
+    int launched = 0;
+    cudaError_t e = cudaSuccess;
+    if (a.ntiles > 0) {
+        a.splits = choose_splits(c, a.n_itiles, a.ntiles, a.ni_pad);
+        if (mode) {
+            e = launch_zero_out(acc, jrk, pot, ni, c->stream);
+            if (e != cudaSuccess) return NB_ERR_CUDA;
+            ++launched;
+        }
+        e = launch_force(a, mode, acc, jrk, pot, c->stream);
+        if (e != cudaSuccess) return NB_ERR_CUDA;
+        ++launched;
+    } else {
+        a.splits = 0;   // n == 0: the reduction of zero partials writes zeros
+    }
+    ReduceArgs r{};
+    r.part = c->part;
+    r.i_list = i_list;
+    r.acc = acc;
+    r.jrk = jrk;
+    r.pot = pot;
+    r.store = c->store;
+    r.flags = c->flags;
+    r.flag_list = c->flag_list;
+    r.nflag = (int)c->flagged.size();
+    r.ni = (int)ni;
+    r.ni_pad = a.ni_pad;
+    r.splits = a.splits;
+    r.n = (int)n_launch;
+    r.t_pred = c->t_pred;
+    r.atomic_mode = (mode && a.ntiles > 0) ? 1 : 0;
+    e = launch_reduce(r, c->stream);
+    if (e != cudaSuccess) return NB_ERR_CUDA;
+    ++launched;
+    c->last[0] = a.splits;
+    c->last[1] = (int64_t)a.n_itiles * a.splits;
+    c->last[2] = launched;
+    c->last[3] = mode;
+    c->launches += launched;
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* nb_version(void) { return "nb 0.1 (sm_100a)"; }
+
+const char* nb_strerror(int status)
+{
+    switch (status) {
+        case NB_OK: return "ok";
+        case NB_ERR_ARG: return "invalid argument";
+        case NB_ERR_ALLOC: return "allocation failed or workspace too small";
+        case NB_ERR_CUDA: return "CUDA error";
+        case NB_ERR_INDEX: return "particle index out of range";
+        case NB_ERR_STATE: return "call out of order (predict before force; workspace before data)";
+        case NB_ERR_ARCH: return "device is not compute capability 10.x";
+        default: return "unknown status";
+    }
+}
+
+size_t nb_workspace_bytes(int64_t n_max, int64_t ni_max)
+{
+    if (n_max < 0 || ni_max < 0) return 0;
+    return layout(n_max, ni_max).total;
+}
+
+int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* stream)
+{
+    if (!out) return NB_ERR_ARG;
+    *out = nullptr;
+    if (n_max < 1 || ni_max < 1 || n_max >= ((int64_t)1 << 31) - 4 * TJ ||
+        ni_max >= ((int64_t)1 << 31) - 4 * ITILE)
+        return NB_ERR_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return NB_ERR_CUDA;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NB_ERR_CUDA;
+    if (prop.major != 10) return NB_ERR_ARCH;
+    nb_ctx* c = new (std::nothrow) nb_ctx();
+    if (!c) return NB_ERR_ALLOC;
+    c->device = device;
+    c->stream = (cudaStream_t)stream;
+    c->n_max = n_max;
+    c->ni_max = ni_max;
+    c->sm_count = prop.multiProcessorCount;
+    DeviceGuard g(device);
+    if (force_kernel_setup(&c->blocks_per_sm) != cudaSuccess || c->blocks_per_sm < 1) {
+        cudaGetLastError();
+        delete c;
+        return NB_ERR_CUDA;
+    }
+    if (cudaMallocHost(&c->err_pinned, sizeof(int)) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return NB_ERR_ALLOC;
+    }
+    *out = c;
+    return NB_OK;
+}
+
+int nb_destroy(nb_ctx* c)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    cudaStreamSynchronize(c->stream);
+    if (c->own_slab && c->slab) cudaFree(c->slab);
+    if (c->err_pinned) cudaFreeHost(c->err_pinned);
+    delete c;
+    return NB_OK;
+}
+
+int nb_set_stream(nb_ctx* c, void* stream)
+{
+    if (!c) return NB_ERR_ARG;
+    c->stream = (cudaStream_t)stream;
+    return NB_OK;
+}
+
+int nb_set_workspace(nb_ctx* c, void* dev_ptr, size_t bytes)
+{
+    if (!c || !dev_ptr || ((uintptr_t)dev_ptr % ALIGN) != 0) return NB_ERR_ARG;
+    if (c->allocated) return NB_ERR_STATE;
+    if (bytes < layout(c->n_max, c->ni_max).total) return NB_ERR_ALLOC;
+    c->slab = static_cast<unsigned char*>(dev_ptr);
+    c->lent_bytes = bytes;
+    c->own_slab = false;
+    return NB_OK;
+}
+
+static int set_j_common(nb_ctx* c, int64_t first, int64_t count, const SrcPtrs& src, bool host)
+{
+    if (!c || first < 0 || count < 0 || first + count > c->n_max) return NB_ERR_ARG;
+    for (int f = F_M; f <= F_VZ; ++f)
+        if (!src.f[f] && count > 0) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (host) {
+        for (int f = 0; f < NFIELD && count > 0; ++f) {
+            cudaError_t e = src.f[f]
+                ? cudaMemcpyAsync(c->store.f[f] + first, src.f[f], (size_t)count * sizeof(double),
+                                  cudaMemcpyHostToDevice, c->stream)
+                : cudaMemsetAsync(c->store.f[f] + first, 0, (size_t)count * sizeof(double), c->stream);
+            if (e != cudaSuccess) return NB_ERR_CUDA;
+        }
+    } else {
+        if (launch_set_j(c->store, src, first, count, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+        if (count > 0) c->launches += 1;
+    }
+    if (first + count > c->n) c->n = first + count;
+    c->predicted = false;
+    return NB_OK;
+}
+
+int nb_set_j(nb_ctx* c, int64_t first, int64_t count, const double* m, const double* x,
+             const double* y, const double* z, const double* vx, const double* vy, const double* vz,
+             const double* ax, const double* ay, const double* az, const double* jx,
+             const double* jy, const double* jz, const double* t)
+{
+    return set_j_common(c, first, count, make_src(m, x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz, t),
+                        false);
+}
+
+int nb_set_j_host(nb_ctx* c, int64_t first, int64_t count, const double* m, const double* x,
+                  const double* y, const double* z, const double* vx, const double* vy,
+                  const double* vz, const double* ax, const double* ay, const double* az,
+                  const double* jx, const double* jy, const double* jz, const double* t)
+{
+    return set_j_common(c, first, count, make_src(m, x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz, t),
+                        true);
+}
+
+int nb_update_j(nb_ctx* c, const int32_t* idx, int64_t count, const double* m, const double* x,
+                const double* y, const double* z, const double* vx, const double* vy,
+                const double* vz, const double* ax, const double* ay, const double* az,
+                const double* jx, const double* jy, const double* jz, const double* t)
+{
+    if (!c || count < 0 || (count > 0 && !idx)) return NB_ERR_ARG;
+    if (count == 0) return NB_OK;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    const SrcPtrs src = make_src(m, x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz, t);
+    if (launch_update_j(c->store, src, idx, count, c->n, c->err, c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    c->launches += 1;
+    c->predicted = false;
+    return NB_OK;
+}
+
+int nb_clear(nb_ctx* c)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    if (c->allocated) {
+        const Layout L = layout(c->n_max, c->ni_max);
+        if (cudaMemsetAsync(c->slab, 0, L.part, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    }
+    c->n = 0;
+    c->flagged.clear();
+    c->predicted = false;
+    return NB_OK;
+}
+
+int64_t nb_count(const nb_ctx* c) { return c ? c->n : (int64_t)NB_ERR_ARG; }
+
+int nb_set_flags(nb_ctx* c, const int32_t* idx, const uint8_t* flags, int64_t count)
+{
+    if (!c || count < 0 || (count > 0 && (!idx || !flags))) return NB_ERR_ARG;
+    if (count == 0) return NB_OK;
+    std::vector<int32_t> next = c->flagged;
+    for (int64_t k = 0; k < count; ++k) {
+        if (idx[k] < 0 || idx[k] >= c->n_max) return NB_ERR_INDEX;
+        size_t pos = 0;
+        bool have = false;
+        for (; pos < next.size(); ++pos)
+            if (next[pos] == idx[k]) { have = true; break; }
+        if ((flags[k] & 1) && !have) next.push_back(idx[k]);
+        if (!(flags[k] & 1) && have) next.erase(next.begin() + pos);
+    }
+    if (next.size() > NB_MAX_FLAGGED) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    // rewrite the flag bytes of the old and new sets, the tile bitmap and the flagged list
+    const int64_t ntiles = c->n_cap / TJ;
+    std::vector<uint32_t> tf((size_t)(ntiles + 31) / 32, 0u);
+    const uint8_t zero = 0, one = 1;
+    for (int32_t i : c->flagged)
+        if (cudaMemcpyAsync(c->flags + i, &zero, 1, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+    for (int32_t i : next) {
+        if (cudaMemcpyAsync(c->flags + i, &one, 1, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        tf[(size_t)(i / TJ) >> 5] |= 1u << ((i / TJ) & 31);
+    }
+    if (cudaMemcpyAsync(c->tileflag, tf.data(), tf.size() * 4, cudaMemcpyHostToDevice, c->stream) !=
+        cudaSuccess)
+        return NB_ERR_CUDA;
+    if (!next.empty() &&
+        cudaMemcpyAsync(c->flag_list, next.data(), next.size() * 4, cudaMemcpyHostToDevice,
+                        c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    // the sources above are pageable host memory: the copies are staged before the calls return
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    c->flagged.swap(next);
+    c->predicted = false;   // the pack carries the flag word
+    return NB_OK;
+}
+
+int nb_predict(nb_ctx* c, double t)
+{
+    if (!c || !isfinite(t)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (launch_predict(c->store, c->flags, c->pack, c->n, t, c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    if (c->n > 0) c->launches += 1;
+    c->predicted = true;
+    c->t_pred = t;
+    return NB_OK;
+}
+
+int nb_get_predicted(nb_ctx* c, int64_t first, int64_t count, double* out)
+{
+    if (!c || first < 0 || count < 0 || first + count > c->n || (count > 0 && !out)) return NB_ERR_ARG;
+    if (!c->predicted) return NB_ERR_STATE;
+    DeviceGuard g(c->device);
+    if (launch_get_predicted(c->store, first, count, c->t_pred, out, c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    if (count > 0) c->launches += 1;
+    return NB_OK;
+}
+
+int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc, double* jrk,
+             double* pot)
+{
+    if (!c || ni < 0 || ni > c->ni_max || !isfinite(eps2) || eps2 < 0.0) return NB_ERR_ARG;
+    if (ni > 0 && (!i_list || !acc || !jrk || !pot)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    return force_impl(c, i_list, ni, eps2, acc, jrk, pot);
+}
+
+int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc,
+                  double* jrk, double* pot)
+{
+    if (!c || ni < 0 || ni > c->ni_max || !isfinite(eps2) || eps2 < 0.0) return NB_ERR_ARG;
+    if (ni > 0 && (!i_list || !acc || !jrk || !pot)) return NB_ERR_ARG;
+    if (!c->predicted) return NB_ERR_STATE;
+    if (ni == 0) return nb_sync(c);
+    DeviceGuard g(c->device);
+    if (cudaMemcpyAsync(c->h_ilist, i_list, (size_t)ni * 4, cudaMemcpyHostToDevice, c->stream) !=
+        cudaSuccess)
+        return NB_ERR_CUDA;
+    double* d_acc = c->h_out;
+    double* d_jrk = c->h_out + 3 * ni;
+    double* d_pot = c->h_out + 6 * ni;
+    int rc = force_impl(c, c->h_ilist, ni, eps2, d_acc, d_jrk, d_pot);
+    if (rc != NB_OK) return rc;
+    const size_t b = (size_t)ni * sizeof(double);
+    if (cudaMemcpyAsync(acc, d_acc, 3 * b, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(jrk, d_jrk, 3 * b, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(pot, d_pot, b, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    return nb_sync(c);
+}
+
+int nb_set_tuning(nb_ctx* c, int j_splits, int reduce_mode)
+{
+    if (!c || j_splits < 0 || reduce_mode < 0 || reduce_mode > 1) return NB_ERR_ARG;
+    c->tune_splits = j_splits;
+    c->tune_reduce = reduce_mode;
+    return NB_OK;
+}
+
+int nb_last_launch(const nb_ctx* c, int64_t* out)
+{
+    if (!c || !out) return NB_ERR_ARG;
+    memcpy(out, c->last, sizeof(c->last));
+    return NB_OK;
+}
+
+int64_t nb_launch_count(const nb_ctx* c) { return c ? c->launches : (int64_t)NB_ERR_ARG; }
+
+int nb_sync(nb_ctx* c)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    if (c->allocated) {
+        if (cudaMemcpyAsync(c->err_pinned, c->err, sizeof(int), cudaMemcpyDeviceToHost, c->stream) !=
+            cudaSuccess)
+            return NB_ERR_CUDA;
+    } else {
+        *c->err_pinned = 0;
+    }
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    if (*c->err_pinned) {
+        *c->err_pinned = 0;
+        if (cudaMemsetAsync(c->err, 0, sizeof(int), c->stream) != cudaSuccess) return NB_ERR_CUDA;
+        return NB_ERR_INDEX;
+    }
+    return NB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,93 @@
+// nb_internal.h -- shared declarations of libnb.so (context, device layouts, kernel launchers).
+// Product code: nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/nb.h"
+
+namespace nb {
+
+// ---- device data layout ------------------------------------------------
+// j-store: 14 fp64 arrays of stride n_cap (SoA): m, x,y,z, vx,vy,vz, ax,ay,az, jx,jy,jz, t.
+enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F_JY, F_JZ, F_T, NFIELD };
+
+// pack: the force-ready predicted j-set, written by the predictor, streamed by the pair kernel.
+// Tiles of TJ particles, SoA inside a tile: NPF float arrays of TJ entries, so that one tile is one
+// contiguous 1-D bulk copy and two consecutive j's form an f32x2 operand pair.
+constexpr int TJ = 128;                       // j-particles per tile
+enum PackField { P_XH = 0, P_YH, P_ZH, P_XL, P_YL, P_ZL, P_VX, P_VY, P_VZ, P_M, P_FLAG, NPF };
+constexpr int TILE_FLOATS = TJ * NPF;         // 1408
+constexpr int TILE_BYTES = TILE_FLOATS * 4;   // 5632 (multiple of 16: legal bulk-copy size)
+
+// pair kernel shape
+constexpr int FORCE_THREADS = 128;
+constexpr int IPT = 2;                        // i-particles per thread
+constexpr int ITILE = FORCE_THREADS * IPT;    // i-particles per CTA
+constexpr int STAGES = 4;                     // j-tile ring depth
+constexpr int NOUT = 7;                       // ax ay az jx jy jz pot
+
+constexpr float PAD_POS = 1.0e10f;            // where the m = 0 padding records of the last tile sit
+
+struct StorePtrs {
+    double* f[NFIELD];
+};
+
+struct SrcPtrs {
+    const double* f[NFIELD];
+};
+
+struct ForceArgs {
+    const float* pack;        // [ntiles][NPF][TJ]
+    const int32_t* i_list;    // [ni]
+    double* part;             // [S][NOUT][ni_pad] partial sums (reduce_mode 0)
+    const uint8_t* flags;     // [n_cap] bit 0: unsoftened among flagged
+    const uint32_t* tileflag; // bit t: tile t holds a flagged particle
+    int* err;                 // device error latch
+    int ni, ni_pad, n_itiles;
+    int n, ntiles, splits;
+    float eps2;
+    int any_flagged;
+};
+
+struct ReduceArgs {
+    const double* part;
+    const int32_t* i_list;
+    double *acc, *jrk, *pot;
+    StorePtrs store;          // for the fp64 flagged-pair terms
+    const uint8_t* flags;
+    const int32_t* flag_list; // indices of flagged particles
+    int nflag;
+    int ni, ni_pad, splits, n;
+    double t_pred;
+    int atomic_mode;          // 1: acc/jrk/pot already hold the sums (atomics); only fix-ups here
+};
+
+// kernel launchers (each returns the cudaError of the launch)
+cudaError_t launch_set_j(const StorePtrs& dst, const SrcPtrs& src, int64_t first, int64_t count,
+                         cudaStream_t s);
+cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int32_t* idx,
+                            int64_t count, int64_t n, int* err, cudaStream_t s);
+cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, int64_t n,
+                           double t, cudaStream_t s);
+cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
+                                 double* out, cudaStream_t s);
+cudaError_t force_kernel_setup(int* blocks_per_sm);
+cudaError_t launch_force(const ForceArgs& a, int atomic_mode, double* acc, double* jrk, double* pot,
+                         cudaStream_t s);
+cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);
+cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
+
+// Hermite predictor of one component (R1), shared by predict / get_predicted / the flagged-pair
+// fix-up so that all three see the same fp64 state.
+__device__ __forceinline__ void predict1(double x, double v, double a, double j, double dt,
+                                         double& xp, double& vp)
+{
+    const double h = 0.5 * dt, s = dt * (1.0 / 3.0);
+    // xp = x + dt (v + dt/2 (a + dt/3 j)) ; vp = v + dt (a + dt/2 j)
+    xp = fma(dt, fma(h, fma(s, j, a), v), x);
+    vp = fma(dt, fma(h, j, a), v);
+}
+
+}  // namespace nb

@@ -1,0 +1,154 @@
+// predict.cu -- a0 (j-store load / scatter) and a1 (Hermite predictor) kernels.
+//
+// The predictor ("optional prediction step on the j particles"; reading
+// R1 in DESIGN.md) is bandwidth-bound: per particle it reads the 14 fp64 fields of the j-store
+// (112 B) and writes one 44-byte force-ready record (two-float position, fp32 velocity and mass,
+// flag word) into the tiled pack the pair kernel streams.  All accesses are unit-stride across
+// the warp; each thread handles two particles so that loads are 128-bit and stores 64-bit.
+#include "nb_internal.h"
+
+namespace nb {
+
+namespace {
+
+__global__ void __launch_bounds__(256) set_j_kernel(StorePtrs dst, SrcPtrs src, int64_t first,
+                                                    int64_t count)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < count; p += stride) {
+#pragma unroll
+        for (int f = 0; f < NFIELD; ++f)
+            dst.f[f][first + p] = src.f[f] ? src.f[f][p] : 0.0;
+    }
+}
+
+__global__ void __launch_bounds__(256) update_j_kernel(StorePtrs dst, SrcPtrs src,
+                                                       const int32_t* __restrict__ idx,
+                                                       int64_t count, int64_t n, int* err)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < count; p += stride) {
+        const int64_t q = idx[p];
+        if (q < 0 || q >= n) {
+            atomicOr(err, 1);
+            continue;
+        }
+#pragma unroll
+        for (int f = 0; f < NFIELD; ++f)
+            if (src.f[f]) dst.f[f][q] = src.f[f][p];
+    }
+}
+
+__device__ __forceinline__ double2 ld2(const double* p, int64_t i)
+{
+    return __ldg(reinterpret_cast<const double2*>(p + i));
+}
+
+// split a double into hi + lo floats (hi = nearest float, lo = nearest float of the remainder):
+// hi + lo carries >= 48 bits of x (emulated double for the inter-particle distance).
+__device__ __forceinline__ void split(double x, float& hi, float& lo)
+{
+    hi = __double2float_rn(x);
+    lo = __double2float_rn(x - (double)hi);
+}
+
+// One thread = particles 2q, 2q+1.  n_pad = ntiles * TJ; particles in [n, n_pad) become m = 0
+// padding records far away.  Store arrays are n_cap >= n_pad long, so loads never leave them.
+__global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_t* __restrict__ flags,
+                                                      float* __restrict__ pack, int64_t n,
+                                                      int64_t n_pad, double t)
+{
+    const int64_t p = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+    if (p >= n_pad) return;
+    const double2 tj = ld2(st.f[F_T], p);
+    const double dt0 = t - tj.x, dt1 = t - tj.y;
+    float2 out[NPF];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double2 x = ld2(st.f[F_X + c], p), v = ld2(st.f[F_VX + c], p);
+        const double2 a = ld2(st.f[F_AX + c], p), j = ld2(st.f[F_JX + c], p);
+        double xp0, vp0, xp1, vp1;
+        predict1(x.x, v.x, a.x, j.x, dt0, xp0, vp0);
+        predict1(x.y, v.y, a.y, j.y, dt1, xp1, vp1);
+        split(xp0, out[P_XH + c].x, out[P_XL + c].x);
+        split(xp1, out[P_XH + c].y, out[P_XL + c].y);
+        out[P_VX + c] = make_float2(__double2float_rn(vp0), __double2float_rn(vp1));
+    }
+    const double2 m = ld2(st.f[F_M], p);
+    out[P_M] = make_float2(__double2float_rn(m.x), __double2float_rn(m.y));
+    const uchar2 fl = *reinterpret_cast<const uchar2*>(flags + p);
+    out[P_FLAG] = make_float2(__uint_as_float(fl.x & 1u), __uint_as_float(fl.y & 1u));
+    if (p >= n || p + 1 >= n) {
+#pragma unroll
+        for (int f = 0; f < NPF; ++f) {
+            const float pad = (f <= P_ZH) ? PAD_POS : 0.0f;
+            if (p >= n) out[f].x = pad;
+            if (p + 1 >= n) out[f].y = pad;
+        }
+    }
+    float* base = pack + (p / TJ) * TILE_FLOATS + (p % TJ);
+#pragma unroll
+    for (int f = 0; f < NPF; ++f) *reinterpret_cast<float2*>(base + f * TJ) = out[f];
+}
+
+__global__ void __launch_bounds__(256) get_predicted_kernel(StorePtrs st, int64_t first,
+                                                            int64_t count, double t, double* out)
+{
+    const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= count) return;
+    const int64_t p = first + q;
+    const double dt = t - st.f[F_T][p];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double xp, vp;
+        predict1(st.f[F_X + c][p], st.f[F_VX + c][p], st.f[F_AX + c][p], st.f[F_JX + c][p], dt, xp, vp);
+        out[(int64_t)c * count + q] = xp;
+        out[(int64_t)(3 + c) * count + q] = vp;
+    }
+}
+
+inline int grid_for(int64_t work, int block, int cap)
+{
+    int64_t g = (work + block - 1) / block;
+    if (g < 1) g = 1;
+    if (g > cap) g = cap;
+    return (int)g;
+}
+
+}  // namespace
+
+cudaError_t launch_set_j(const StorePtrs& dst, const SrcPtrs& src, int64_t first, int64_t count,
+                         cudaStream_t s)
+{
+    if (count == 0) return cudaSuccess;
+    set_j_kernel<<<grid_for(count, 256, 148 * 16), 256, 0, s>>>(dst, src, first, count);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int32_t* idx,
+                            int64_t count, int64_t n, int* err, cudaStream_t s)
+{
+    if (count == 0) return cudaSuccess;
+    update_j_kernel<<<grid_for(count, 256, 148 * 16), 256, 0, s>>>(dst, src, idx, count, n, err);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, int64_t n,
+                           double t, cudaStream_t s)
+{
+    if (n == 0) return cudaSuccess;
+    const int64_t n_pad = (n + TJ - 1) / TJ * TJ;
+    const int64_t threads = n_pad / 2;
+    predict_kernel<<<(unsigned)((threads + 127) / 128), 128, 0, s>>>(store, flags, pack, n, n_pad, t);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
+                                 double* out, cudaStream_t s)
+{
+    if (count == 0) return cudaSuccess;
+    get_predicted_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(store, first, count, t, out);
+    return cudaGetLastError();
+}
+
+}  // namespace nb

@@ -1,0 +1,130 @@
+"""-m gpu: BASELINE.json's configs 2-5 at full size, in the launch configuration bench.py times
+(dispatcher-chosen j-splits), checked on every i (config 2) or on the sampled set C of DESIGN.md
+(configs 3-5): seed-sampled active i, all flagged particles, the active i with the smallest and
+largest |a_gpu| (worst relative error sits at small |a|), and the index-edge cases."""
+import numpy as np
+import pytest
+
+import nbgen
+import oracle
+from util import check_parity
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def nbmod():
+    import __graft_entry__ as g
+    g.build()
+    import paper_1409_5474_b200 as nbm
+    return nbm
+
+
+def _np(ts):
+    return [q.cpu().numpy() for q in ts]
+
+
+def check_set(case, il, a_gpu, n_sample, seed):
+    """Positions k into il to verify (set C)."""
+    ni = len(il)
+    pos = [nbgen.sample_positions(seed, ni, n_sample)]
+    if ni > n_sample:
+        an = np.sqrt((a_gpu ** 2).sum(0))
+        order = np.argsort(an)
+        pos += [order[:64], order[-64:]]
+        where = {int(v): k for k, v in enumerate(il)} if ni <= 1 << 16 else None
+        edges = [0, 1, 127, 128, 255, 256, case.n - 129, case.n - 2, case.n - 1] + \
+            np.flatnonzero(case.flags).tolist()
+        if where is None:
+            hit = np.flatnonzero(np.isin(il, edges))
+        else:
+            hit = np.array([where[e] for e in edges if e in where], dtype=np.int64)
+        pos.append(hit)
+    return np.unique(np.concatenate([np.asarray(p, dtype=np.int64) for p in pos]))
+
+
+def sampled_parity(ctx, case, il, t, n_sample, seed):
+    got = _np(ctx.force(il, case.eps2))
+    info = ctx.last_launch()
+    ctx.sync()
+    pos = check_set(case, il, got[0], n_sample, seed)
+    xp, vp = oracle.predict(t, case.x, case.v, case.a, case.j, case.t)
+    fl = case.flags if case.flags.any() else None
+    ref = oracle.force(case.m, xp, vp, il[pos], case.eps2, fl)
+    errs = check_parity([got[0][:, pos], got[1][:, pos], got[2][pos]], ref)
+    assert all(np.isfinite(g).all() for g in got)
+    return errs, info, len(pos)
+
+
+def hermite_correct(x0, v0, a0, j0, a1, j1, dt):
+    """R12: one P(EC) pass with a shared step (harness code, fp64)."""
+    v1 = v0 + (a0 + a1) * (dt / 2) + (j0 - j1) * (dt * dt / 12)
+    x1 = x0 + (v0 + v1) * (dt / 2) + (a0 - a1) * (dt * dt / 12)
+    return x1, v1
+
+
+def test_config2_hermite_steps(nbmod):
+    """Predictor + force over 10 shared steps.  The trajectory is driven by the ORACLE's forces;
+    at each step the GPU gets the same stored state and must reproduce predictor and forces."""
+    c = nbgen.config2()
+    il = c.i_lists[0]
+    with nbmod.Context(c.n) as ctx:
+        ctx.load_case(c)
+        ra, rj, rp = oracle.force(c.m, c.x, c.v, il, c.eps2)          # step 0: (a0, j0)
+        ctx.predict(0.0)
+        print("cfg2 step 0", check_parity(_np(ctx.force(il, c.eps2)), (ra, rj, rp)))
+        c.a, c.j = ra, rj
+        e0 = 0.5 * (c.m * (c.v ** 2).sum(0)).sum() + 0.5 * (c.m * rp).sum()
+        for step in range(1, c.steps + 1):
+            t = step * c.dt
+            ctx.update_j(il, c.m, c.x, c.v, c.a, c.j, c.t)
+            ctx.predict(t)
+            gx, gv = _np(ctx.predicted())
+            got = _np(ctx.force(il, c.eps2))
+            ctx.sync()
+            xp, vp = oracle.predict(t, c.x, c.v, c.a, c.j, c.t)
+            ra, rj, rp = oracle.force(c.m, xp, vp, il, c.eps2)
+            assert np.abs(gx - xp).max() < 1e-14 and np.abs(gv - vp).max() < 1e-14
+            errs = check_parity(got, (ra, rj, rp))
+            c.x, c.v = hermite_correct(c.x, c.v, c.a, c.j, ra, rj, c.dt)
+            c.a, c.j, c.t = ra, rj, np.full(c.n, t)
+        print("cfg2 step", step, errs)
+        # the corrector is 4th order: energy drifts little over 10 steps (informational pin P11)
+        ra, rj, rp = oracle.force(c.m, c.x, c.v, il, c.eps2)
+        e1 = 0.5 * (c.m * (c.v ** 2).sum(0)).sum() + 0.5 * (c.m * rp).sum()
+        assert abs(e1 - e0) < 1e-5 * abs(e0)
+
+
+def test_config3_block_step_subsets(nbmod):
+    c = nbgen.config3()
+    with nbmod.Context(c.n) as ctx:
+        ctx.load_case(c)
+        ctx.predict(c.t_now)
+        gx, gv = _np(ctx.predicted(0, 4096))
+        xp, vp = oracle.predict(c.t_now, c.x, c.v, c.a, c.j, c.t)
+        assert np.abs(gx - xp[:, :4096]).max() < 1e-14 and np.abs(gv - vp[:, :4096]).max() < 1e-14
+        for il in c.i_lists:
+            ns = 4096 if len(il) > 1024 else len(il)
+            errs, info, nchk = sampled_parity(ctx, c, il, c.t_now, ns, nbgen.SEED0 * 100 + 3)
+            print("cfg3 ni=%d checked=%d" % (len(il), nchk), errs, info)
+
+
+def test_config4_merger_with_black_holes(nbmod):
+    c = nbgen.config4()
+    with nbmod.Context(c.n) as ctx:
+        ctx.load_case(c)
+        ctx.predict(0.0)
+        errs, info, nchk = sampled_parity(ctx, c, c.i_lists[0], 0.0, 4096, nbgen.SEED0 * 100 + 4)
+        print("cfg4 checked=%d" % nchk, errs, info)
+
+
+def test_config5_group(nbmod):
+    c = nbgen.config5()
+    il = c.i_lists[0]
+    with nbmod.Context(c.n, len(il)) as ctx:
+        ctx.load_case(c)
+        ctx.predict(0.0)
+        errs, info, nchk = sampled_parity(ctx, c, il, 0.0, 4096, nbgen.SEED0 * 100 + 5)
+        print("cfg5 checked=%d" % nchk, errs, info)
