@@ -147,6 +147,14 @@ int nb_last_launch(const nb_ctx* c, int64_t* out);
 /* Total kernels this context has launched since creation (bench.py's gpu_launches). */
 int64_t nb_launch_count(const nb_ctx* c);
 
+/* Per-kernel device timing for the roofline report.  With profiling on,
+ * nb_predict and nb_force record CUDA events on the context's stream around their kernels;
+ * nb_kernel_times synchronises the stream and writes, to HOST double[3], the duration in ms of
+ * the last predictor kernel, the last pair kernel and the last reduction kernel (-1 where none
+ * ran since profiling was switched on).  NB_ERR_STATE if profiling is off. */
+int nb_set_profiling(nb_ctx* c, int on);
+int nb_kernel_times(nb_ctx* c, double* out_ms);
+
 int nb_sync(nb_ctx* c);                 /* stream sync; returns and clears any latched error */
 const char* nb_strerror(int status);
 const char* nb_version(void);

@@ -7,5 +7,6 @@ libnb.so's sm_100a kernels (csrc/).  Importing fails loudly if the library has n
 from . import binding
 from .binding import *  # noqa: F401,F403  (the nb_* functions and status codes)
 from .context import Context
+from . import sharding
 
-__all__ = ["binding", "Context"] + [n for n in dir(binding) if n.startswith(("nb_", "NB"))]
+__all__ = ["binding", "Context", "sharding"] + [n for n in dir(binding) if n.startswith(("nb_", "NB"))]

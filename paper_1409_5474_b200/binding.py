@@ -18,7 +18,7 @@ EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_host", "nb_set_tuning",
-    "nb_last_launch", "nb_launch_count", "nb_sync", "nb_strerror", "nb_version",
+    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync", "nb_strerror", "nb_version",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -50,6 +50,8 @@ lib.nb_set_tuning.argtypes = [_vp, _i32, _i32]
 lib.nb_last_launch.argtypes = [_vp, ctypes.POINTER(_i64)]
 lib.nb_launch_count.argtypes = [_vp]
 lib.nb_launch_count.restype = _i64
+lib.nb_set_profiling.argtypes = [_vp, _i32]
+lib.nb_kernel_times.argtypes = [_vp, ctypes.POINTER(_dbl)]
 lib.nb_sync.argtypes = [_vp]
 lib.nb_strerror.argtypes = [_i32]
 lib.nb_strerror.restype = ctypes.c_char_p
@@ -184,6 +186,17 @@ def nb_last_launch(c):
 
 def nb_launch_count(c):
     return int(lib.nb_launch_count(c))
+
+
+def nb_set_profiling(c, on=True):
+    _check(lib.nb_set_profiling(c, 1 if on else 0), "nb_set_profiling")
+
+
+def nb_kernel_times(c):
+    """ms of the last predictor / pair / reduction kernels (after a stream sync)."""
+    out = (_dbl * 3)()
+    _check(lib.nb_kernel_times(c, out), "nb_kernel_times")
+    return {"predict_ms": out[0], "pair_ms": out[1], "reduce_ms": out[2]}
 
 
 def nb_sync(c):

@@ -86,3 +86,23 @@ class Context:
 
     def sync(self):
         nb.nb_sync(self.h)
+
+    # -- host-buffer entry points (the end-to-end path: copies are part of the call) ----------
+    def set_j_host(self, m, x, v, a=None, j=None, t=None, first=0):
+        """HOST arrays (numpy or pinned CPU tensors), fp64 contiguous; staged by the library."""
+        nb.nb_set_j_host(self.h, first, m.shape[0], m, x, v, a, j, t)
+
+    def force_host(self, i_list, eps2, acc, jrk, pot):
+        """HOST int32 i_list and HOST fp64 outputs acc, jrk (3, ni), pot (ni,); returns after
+        the results are back on the host."""
+        nb.nb_force_host(self.h, i_list, i_list.shape[0], eps2, acc, jrk, pot)
+
+    # -- measurement --------------------------------------------------------------------------
+    def profiling(self, on=True):
+        nb.nb_set_profiling(self.h, on)
+
+    def kernel_times(self):
+        return nb.nb_kernel_times(self.h)
+
+    def launch_count(self):
+        return nb.nb_launch_count(self.h)

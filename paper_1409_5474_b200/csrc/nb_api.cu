@@ -37,6 +37,11 @@ struct nb_ctx {
     int tune_splits = 0, tune_reduce = 0;
     int64_t last[4] = {0, 0, 0, 0};
     int64_t launches = 0;
+
+    // optional per-kernel timing (nb_set_profiling): events recorded on the context's stream
+    bool prof = false;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // predict [0,1], pair [2,3], reduce [3,4]
+    bool ev_predict = false, ev_force = false;
 };
 
 namespace {
@@ -189,8 +194,10 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             if (e != cudaSuccess) return NB_ERR_CUDA;
             ++launched;
         }
+        if (c->prof) cudaEventRecord(c->ev[2], c->stream);
         e = launch_force(a, mode, acc, jrk, pot, c->stream);
         if (e != cudaSuccess) return NB_ERR_CUDA;
+        if (c->prof) cudaEventRecord(c->ev[3], c->stream);
         ++launched;
     } else {
         a.splits = 0;   // n == 0: the reduction of zero partials writes zeros
@@ -213,6 +220,10 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     r.atomic_mode = (mode && a.ntiles > 0) ? 1 : 0;
     e = launch_reduce(r, c->stream);
     if (e != cudaSuccess) return NB_ERR_CUDA;
+    if (c->prof && a.ntiles > 0) {
+        cudaEventRecord(c->ev[4], c->stream);
+        c->ev_force = true;
+    }
     ++launched;
     c->last[0] = a.splits;
     c->last[1] = (int64_t)a.n_itiles * a.splits;
@@ -292,6 +303,8 @@ int nb_destroy(nb_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->own_slab && c->slab) cudaFree(c->slab);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
+    for (cudaEvent_t e : c->ev)
+        if (e) cudaEventDestroy(e);
     delete c;
     return NB_OK;
 }
@@ -441,8 +454,13 @@ int nb_predict(nb_ctx* c, double t)
     DeviceGuard g(c->device);
     int rc = ensure_alloc(c);
     if (rc != NB_OK) return rc;
+    if (c->prof) cudaEventRecord(c->ev[0], c->stream);
     if (launch_predict(c->store, c->flags, c->pack, c->n, t, c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
+    if (c->prof) {
+        cudaEventRecord(c->ev[1], c->stream);
+        c->ev_predict = true;
+    }
     if (c->n > 0) c->launches += 1;
     c->predicted = true;
     c->t_pred = t;
@@ -509,6 +527,40 @@ int nb_last_launch(const nb_ctx* c, int64_t* out)
 }
 
 int64_t nb_launch_count(const nb_ctx* c) { return c ? c->launches : (int64_t)NB_ERR_ARG; }
+
+int nb_set_profiling(nb_ctx* c, int on)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    if (on && !c->ev[0]) {
+        for (cudaEvent_t& e : c->ev)
+            if (cudaEventCreate(&e) != cudaSuccess) return NB_ERR_CUDA;
+    }
+    c->prof = on != 0;
+    c->ev_predict = c->ev_force = false;
+    return NB_OK;
+}
+
+int nb_kernel_times(nb_ctx* c, double* out_ms)
+{
+    if (!c || !out_ms) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    out_ms[0] = out_ms[1] = out_ms[2] = -1.0;
+    if (!c->prof) return NB_ERR_STATE;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    float ms = 0.f;
+    if (c->ev_predict) {
+        if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) != cudaSuccess) return NB_ERR_CUDA;
+        out_ms[0] = ms;
+    }
+    if (c->ev_force) {
+        if (cudaEventElapsedTime(&ms, c->ev[2], c->ev[3]) != cudaSuccess) return NB_ERR_CUDA;
+        out_ms[1] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[3], c->ev[4]) != cudaSuccess) return NB_ERR_CUDA;
+        out_ms[2] = ms;
+    }
+    return NB_OK;
+}
 
 int nb_sync(nb_ctx* c)
 {

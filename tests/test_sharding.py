@@ -1,0 +1,77 @@
+"""-m "not gpu": host logic of the multi-GPU decomposition (paper_1409_5474_b200/sharding.py),
+world_size 2 over gloo on the CPU.  Each rank's "force call" here is the ORACLE on its i-slice
+(tests may call the oracle); what is tested is the slicing and the assembly in i_list order, i.e.
+that sharded == unsharded exactly (the i-particles are independent)."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+torch = pytest.importorskip("torch")
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def test_shard_bounds_cover_without_overlap():
+    import __graft_entry__ as g
+    g.build()
+    from paper_1409_5474_b200 import sharding
+    for ni in (0, 1, 2, 7, 256, 1000, 1 << 20):
+        for world in (1, 2, 3, 8):
+            cuts = [sharding.shard_bounds(ni, r, world) for r in range(world)]
+            assert cuts[0][0] == 0 and cuts[-1][1] == ni
+            assert all(cuts[r][1] == cuts[r + 1][0] for r in range(world - 1))
+            sizes = [b - a for a, b in cuts]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        sharding.shard_bounds(10, 2, 2)
+
+
+def _worker(rank, world, port, ni, out_q):
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch.distributed as dist
+    import nbgen
+    import oracle
+    from paper_1409_5474_b200 import sharding
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        c = nbgen.config1(512)
+        il = nbgen.permutation(5, c.n)[:ni]
+        mine = sharding.shard_i_list(il, rank, world)
+        a, j, p = oracle.force(c.m, c.x, c.v, mine, c.eps2)
+        acc, jrk, pot = sharding.gather_forces(torch.from_numpy(a), torch.from_numpy(j),
+                                               torch.from_numpy(p), len(il))
+        ra, rj, rp = oracle.force(c.m, c.x, c.v, il, c.eps2)
+        ok = (acc.numpy() == ra).all() and (jrk.numpy() == rj).all() and (pot.numpy() == rp).all()
+        out_q.put((rank, bool(ok), tuple(acc.shape)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("ni", [301, 2, 1])
+def test_gather_forces_world2_gloo(ni):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, ni, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [0, 1]
+    assert all(r[1] for r in res)
+    assert all(r[2] == (3, ni) for r in res)
