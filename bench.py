@@ -1,0 +1,401 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the driver (contract: the task prompt's section 4).
+
+A "step" is one pass of the whole hot path (rows a0..a5) over config 3's
+headline call (BASELINE.json configs[2], the one north_star's target is quoted on): Plummer sphere
+N = 2^20 in the synthetic block-time-step state, all 2^20 particles active:
+    nb_update_j(active)  ->  nb_predict(t)  ->  nb_force(i_list, eps2)  [gather, pairs, reduce]
+`value` = interactions/s (N_i x N per call, self pair counted, 60 flop each; R11) with
+all inputs resident in HBM; `e2e` = the same step through the host-buffer entry points of the
+C-ABI (pinned host arrays in, host arrays out, copies inside the timed region).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg3|cfg2|cfg4|cfg5|small] [--no-cpu-baseline] [--no-e2e]
+
+N > 1 (torchrun, one rank per GPU): the active list is sharded over the ranks (i-particles are
+independent), every rank holds all j; the per-rank results are assembled with one
+all_gather (paper_1409_5474_b200/sharding.py).  Total work is fixed: "scaling": "strong".
+
+--impl reference: there is no reference code (the paper ships none); this arm times the fp64
+oracle, as it stands, on the host cores, each step a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_INTERACTION = 60.0
+# "alu" roofline denominator: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x
+# clocks.max.sm 1.965 GHz (B200_PROFILING.md unit counts and clocks) = 74.45 Tflop/s.
+FP32_LANES_PER_SM = 128
+PREDICT_BYTES_PER_PARTICLE = 152.0     # 104 B read + 48 B written
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg2", "cfg4", "cfg5", "small"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0,
+                    help="target duration of the cpu_baseline sample")
+    return ap.parse_args()
+
+
+def make_case(name):
+    """Returns (case, i_list, t, workload string).  Seeded synthetic input (nbgen, DESIGN.md
+    section 5): stands in for the paper's own particle sets, which are not available."""
+    import nbgen
+    if name == "cfg3":
+        c = nbgen.config3()
+        return c, c.i_lists[-1], c.t_now, "cfg3_plummer_N1048576_blockstep_all_active"
+    if name == "cfg2":
+        c = nbgen.config2()
+        c.a, c.j = nbgen.mean_field(c.x, c.v)
+        return c, c.i_lists[0], c.dt, "cfg2_plummer_N65536_hermite_step"
+    if name == "cfg4":
+        c = nbgen.config4()
+        return c, c.i_lists[0], 0.0, "cfg4_merger_N1048578_all_active"
+    if name == "cfg5":
+        c = nbgen.config5()
+        return c, c.i_lists[0], 0.0, "cfg5_group_N4194315_Ni1048576"
+    c = nbgen.config3(n=1 << 14, sizes=(1 << 14,))
+    return c, c.i_lists[-1], c.t_now, "small_plummer_N16384_all_active"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.path = "/tmp/nb_bench_clocks_%d_%d.csv" % (os.getpid(), index)
+
+    def start(self):
+        try:
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=self.fh, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return None
+        self.proc.terminate()          # the exact PID started above
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.fh.close()
+        sm, mx, pw, reasons = [], [], [], set()
+        with open(self.path) as f:
+            for line in f:
+                p = [q.strip() for q in line.split(",")]
+                if len(p) < 7:
+                    continue
+                try:
+                    sm.append(float(p[0])); mx.append(float(p[1])); pw.append(float(p[2]))
+                except ValueError:
+                    continue
+                for name, val in zip(self.NAMES, p[3:7]):
+                    if val == "Active":
+                        reasons.add(name)
+        try:
+            os.remove(self.path)
+        except OSError:
+            pass
+        if not sm:
+            return None
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(case, il, t, seconds):
+    """Time the oracle, as it stands, on a bounded sample of the workload: the predictor on all N
+    (once) and the force on the first `ni_s` entries of the active list against all N j.  ni_s is
+    calibrated so that the force leg takes about `seconds`."""
+    import numpy as np
+    import oracle
+    fl = case.flags if case.flags.any() else None
+    t0 = time.perf_counter()
+    xp, vp = oracle.predict(t, case.x, case.v, case.a, case.j, case.t)
+    t_pred = time.perf_counter() - t0
+    n = case.n
+    ni_c = max(1, min(len(il), (1 << 29) // n))           # calibration: ~5.4e8 pairs
+    t0 = time.perf_counter()
+    oracle.force(case.m, xp, vp, il[:ni_c], case.eps2, fl)
+    rate = ni_c * n / (time.perf_counter() - t0)
+    ni_s = int(max(1, min(len(il), rate * seconds / n)))
+    t0 = time.perf_counter()
+    oracle.force(case.m, xp, vp, il[:ni_s], case.eps2, fl)
+    dt = time.perf_counter() - t0
+    return {"value": ni_s * n / dt, "unit": "interactions/s", "cores": oracle.threads(),
+            "kind": "oracle",
+            "sample": "first %d of %d active i against all %d j (%.3g interactions, %.1f s); "
+                      "predictor on all j took %.3f s" % (ni_s, len(il), n, ni_s * float(n), dt, t_pred),
+            "gflops": ni_s * n / dt * FLOP_PER_INTERACTION / 1e9}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (no reference code exists)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    import oracle
+    case, il, t, workload = make_case(args.workload)
+    n = case.n
+    fl = case.flags if case.flags.any() else None
+    # bounded sample per step: ~1.5 s of force work
+    xp, vp = oracle.predict(t, case.x, case.v, case.a, case.j, case.t)
+    ni_c = max(1, min(len(il), (1 << 29) // n))
+    t0 = time.perf_counter()
+    oracle.force(case.m, xp, vp, il[:ni_c], case.eps2, fl)
+    rate = ni_c * n / (time.perf_counter() - t0)
+    ni_s = int(max(1, min(len(il), rate * 1.5 / n)))
+    sub = np.ascontiguousarray(il[:ni_s])
+
+    def step():
+        xp, vp = oracle.predict(t, case.x, case.v, case.a, case.j, case.t)
+        return oracle.force(case.m, xp, vp, sub, case.eps2, fl)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = ni_s * n * args.steps / dt
+    sample = "each step: oracle predictor on all %d j + oracle force on the first %d of %d active i" % (
+        n, ni_s, len(il))
+    line = {
+        "impl": "reference", "metric": "interactions/s", "value": val, "unit": "interactions/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "gflops": val * FLOP_PER_INTERACTION / 1e9,
+        "config": {"workload": workload, "n_j": n, "n_i": int(len(il)), "eps2": case.eps2,
+                   "note": "no reference code exists (paper only); this arm is the fp64 oracle on host cores"},
+        "cpu_baseline": {"value": val, "unit": "interactions/s", "cores": oracle.threads(),
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "interactions/s", "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def measured_peaks():
+    """MEASURED_PEAKS.json (driver-written) or the profiling recipe's stated fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
+                "source": "measured"}
+    except (OSError, ValueError, KeyError):
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload,
+# from the committed `ncu --set full` capture (profiles/r1_force_full.md); None until captured.
+FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": None}
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as g
+    g.build()
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import binding as nb, sharding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: there is no CPU fallback (use --impl reference "
+                         "for the oracle on host cores)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    case, il, t, workload = make_case(args.workload)
+    n, ni = case.n, len(il)
+    lo, hi = sharding.shard_bounds(ni, rank, world)
+    il_loc = np.ascontiguousarray(il[lo:hi])
+    ni_loc = hi - lo
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ctx = nbm.Context(n, max(ni, 1), device=local)
+    ctx.load_case(case)
+    h = ctx.h
+    # device-resident step inputs: the active list and the active particles' corrected state (here:
+    # their stored state again -- a real integrator writes the corrector's output into these)
+    d_il_full = torch.from_numpy(np.ascontiguousarray(il)).to(dev)
+    d_il = torch.from_numpy(il_loc).to(dev)
+    upd = [torch.from_numpy(np.ascontiguousarray(q[..., il])).to(dev)
+           for q in (case.m, case.x, case.v, case.a, case.j, case.t)]
+    acc = torch.empty((3, ni_loc), dtype=torch.float64, device=dev)
+    jrk = torch.empty((3, ni_loc), dtype=torch.float64, device=dev)
+    pot = torch.empty((ni_loc,), dtype=torch.float64, device=dev)
+
+    def step():
+        nb.nb_update_j(h, d_il_full, ni, *upd)                     # a0
+        nb.nb_predict(h, t)                                        # a1
+        nb.nb_force(h, d_il, ni_loc, case.eps2, acc, jrk, pot)     # a2..a5
+        if world > 1:
+            return sharding.gather_forces(acc, jrk, pot, ni)
+        return acc, jrk, pot
+
+    def timed(fn, k):
+        """k calls of fn between barrier + synchronize, CUDA events on the launching stream."""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(k):
+            fn()
+        e1.record()
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+    for attempt in range(2):
+        ctx.profiling(True)
+        l0 = ctx.launch_count()
+        sampler = ClockSampler(local)
+        sampler.start()
+        ms = timed(step, args.steps)
+        clocks = sampler.stop()
+        launches = ctx.launch_count() - l0
+        kt = ctx.kernel_times()
+        ctx.profiling(False)
+        if clocks is None or not (bad & set(clocks["reasons"])):
+            break
+    nb.nb_sync(h)
+    assert bool(torch.isfinite(pot).all()), "non-finite potential"
+    value = float(ni) * n * args.steps / (ms * 1e-3)
+
+    # ---- e2e: the same step through the HOST-buffer entry points of the C-ABI -----------------
+    e2e = None
+    if not args.no_e2e:
+        def pin(a):
+            return torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h_il_full, h_il = pin(il), pin(il_loc)
+        h_upd = [pin(q[..., il]) for q in (case.m, case.x, case.v, case.a, case.j, case.t)]
+        h_acc = torch.empty((3, ni_loc), dtype=torch.float64).pin_memory()
+        h_jrk = torch.empty((3, ni_loc), dtype=torch.float64).pin_memory()
+        h_pot = torch.empty((ni_loc,), dtype=torch.float64).pin_memory()
+        h2d = ni * 4 + sum(q.numel() * 8 for q in h_upd) + ni_loc * 4
+        d2h = (h_acc.numel() + h_jrk.numel() + h_pot.numel()) * 8
+
+        def step_host():
+            nb.nb_update_j_host(h, h_il_full, ni, *h_upd)
+            nb.nb_predict(h, t)
+            nb.nb_force_host(h, h_il, ni_loc, case.eps2, h_acc, h_jrk, h_pot)   # returns synced
+
+        step_host()
+        barrier()
+        w0 = time.perf_counter()
+        ms_h = timed(step_host, args.steps)
+        wall = time.perf_counter() - w0
+        assert bool(torch.isfinite(h_pot).all())
+        e2e = {"value": float(ni) * n * args.steps / (ms_h * 1e-3), "unit": "interactions/s",
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": ms_h / args.steps, "wall_ms_per_step": wall / args.steps * 1e3,
+               "api": "nb_update_j_host + nb_predict + nb_force_host (pinned host buffers)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peaks = measured_peaks()
+    props = torch.cuda.get_device_properties(dev)
+    sm_max = clocks["sm_max_mhz"] if clocks else peaks["sm_max_mhz"]
+    fp32_peak_tflops = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    pair_ms = kt["pair_ms"] / max(kt["n_pair"], 1)
+    pred_ms = kt["predict_ms"] / max(kt["n_predict"], 1)
+    red_ms = kt["reduce_ms"] / max(kt["n_reduce"], 1)
+    ach = FLOP_PER_INTERACTION * ni_loc * n / (pair_ms * 1e-3) / 1e12
+    roofline = {"kernel": "force_kernel", "bound": "alu", "achieved": ach, "peak": fp32_peak_tflops,
+                "unit": "TFLOP/s", "frac": ach / fp32_peak_tflops,
+                "traffic": FORCE_KERNEL_DRAM_TRAFFIC.get(args.workload),
+                "peak_source": "derived: %d SMs x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm)" % (
+                    props.multi_processor_count, sm_max),
+                "ms_per_launch": pair_ms, "launches_timed": kt["n_pair"],
+                "share_of_step": kt["pair_ms"] / ms}
+    if clocks:
+        obs = props.multi_processor_count * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12
+        roofline["frac_at_observed_clock"] = ach / obs
+    pred_gbs = PREDICT_BYTES_PER_PARTICLE * n / (pred_ms * 1e-3) / 1e9
+    roofline_predict = {"kernel": "predict_kernel", "bound": "hbm", "achieved": pred_gbs,
+                        "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_gbs / peaks["hbm_gbs"],
+                        "traffic": None, "peak_source": peaks["source"], "ms_per_launch": pred_ms,
+                        "bytes_per_particle": PREDICT_BYTES_PER_PARTICLE}
+    line = {
+        "metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "gflops": value * FLOP_PER_INTERACTION / 1e9,
+        "config": {"workload": workload, "n_j": n, "n_i": ni, "eps2": case.eps2,
+                   "step": "nb_update_j(active) + nb_predict + nb_force (gather, pairs, reduce)",
+                   "parallelism": "i-sharded x%d, j replicated" % world,
+                   "l2": "no flush: per-step working set (j-store %.0f MB + pack %.0f MB + outputs "
+                         "%.0f MB) exceeds the L2" % (112e-6 * n, 44e-6 * n, 56e-6 * ni),
+                   "arithmetic": "two-float (48-bit) position differences, fp32 pair terms, "
+                                 "fp32 per-tile sums flushed to fp64"},
+        "clocks": ({"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"],
+                    "reasons": clocks["reasons"], "power_w_max": clocks["power_w_max"],
+                    "samples": clocks["samples"]} if clocks else None),
+        "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roofline, "roofline_predict": roofline_predict,
+        "kernels_ms": {"predict": pred_ms, "pair": pair_ms, "reduce": red_ms},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = oracle_sample(case, il, t, args.cpu_seconds)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

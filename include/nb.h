@@ -81,6 +81,16 @@ int nb_update_j(nb_ctx* c, const int32_t* idx, int64_t count, const double* m,
                 const double* ax, const double* ay, const double* az,
                 const double* jx, const double* jy, const double* jz, const double* t);
 
+/* nb_update_j from HOST memory (idx and the 14 arrays are HOST pointers, ideally pinned): staged
+ * through the context's own device buffers on its stream, then scattered.  count <= ni_max
+ * (the staging area is sized by it), else NB_ERR_ARG.  The host arrays must stay valid until the
+ * stream has consumed them (nb_sync). */
+int nb_update_j_host(nb_ctx* c, const int32_t* idx, int64_t count, const double* m,
+                const double* x, const double* y, const double* z,
+                const double* vx, const double* vy, const double* vz,
+                const double* ax, const double* ay, const double* az,
+                const double* jx, const double* jy, const double* jz, const double* t);
+
 /* HOST-pointer form of nb_set_j (pageable or pinned host memory; staged through the context's
  * pinned buffer with cudaMemcpyAsync).  Same argument rules. */
 int nb_set_j_host(nb_ctx* c, int64_t first, int64_t count, const double* m,
@@ -148,10 +158,11 @@ int nb_last_launch(const nb_ctx* c, int64_t* out);
 int64_t nb_launch_count(const nb_ctx* c);
 
 /* Per-kernel device timing for the roofline report.  With profiling on,
- * nb_predict and nb_force record CUDA events on the context's stream around their kernels;
- * nb_kernel_times synchronises the stream and writes, to HOST double[3], the duration in ms of
- * the last predictor kernel, the last pair kernel and the last reduction kernel (-1 where none
- * ran since profiling was switched on).  NB_ERR_STATE if profiling is off. */
+ * nb_predict and nb_force record CUDA events on the context's stream around their kernels.
+ * nb_kernel_times synchronises the stream and writes, to HOST double[6], the running totals
+ * since profiling was switched on: [0..2] = summed duration in ms of the predictor kernels, the
+ * pair kernels and the reduction kernels, [3..5] = how many of each were timed.
+ * nb_set_profiling(on) resets the totals.  NB_ERR_STATE if profiling is off. */
 int nb_set_profiling(nb_ctx* c, int on);
 int nb_kernel_times(nb_ctx* c, double* out_ms);
 

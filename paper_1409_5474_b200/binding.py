@@ -16,7 +16,7 @@ NB_MAX_FLAGGED = 1024
 
 EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
-    "nb_set_j", "nb_update_j", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
+    "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_host", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync", "nb_strerror", "nb_version",
 ]
@@ -38,6 +38,7 @@ lib.nb_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
 for _f in (lib.nb_set_j, lib.nb_set_j_host):
     _f.argtypes = [_vp, _i64, _i64] + [_vp] * 14
 lib.nb_update_j.argtypes = [_vp, _vp, _i64] + [_vp] * 14
+lib.nb_update_j_host.argtypes = [_vp, _vp, _i64] + [_vp] * 14
 lib.nb_clear.argtypes = [_vp]
 lib.nb_count.argtypes = [_vp]
 lib.nb_count.restype = _i64
@@ -139,6 +140,11 @@ def nb_update_j(c, idx, count, m, x, v, a=None, j=None, t=None):
     _check(lib.nb_update_j(c, _ptr(idx), count, *_fields(m, x, v, a, j, t)), "nb_update_j")
 
 
+def nb_update_j_host(c, idx, count, m, x, v, a=None, j=None, t=None):
+    """HOST idx (int32) and arrays; count <= ni_max."""
+    _check(lib.nb_update_j_host(c, _ptr(idx), count, *_fields(m, x, v, a, j, t)), "nb_update_j_host")
+
+
 def nb_clear(c):
     _check(lib.nb_clear(c), "nb_clear")
 
@@ -193,10 +199,12 @@ def nb_set_profiling(c, on=True):
 
 
 def nb_kernel_times(c):
-    """ms of the last predictor / pair / reduction kernels (after a stream sync)."""
-    out = (_dbl * 3)()
+    """Totals since profiling was switched on (after a stream sync): summed ms and launch counts
+    of the predictor / pair / reduction kernels."""
+    out = (_dbl * 6)()
     _check(lib.nb_kernel_times(c, out), "nb_kernel_times")
-    return {"predict_ms": out[0], "pair_ms": out[1], "reduce_ms": out[2]}
+    return {"predict_ms": out[0], "pair_ms": out[1], "reduce_ms": out[2],
+            "n_predict": int(out[3]), "n_pair": int(out[4]), "n_reduce": int(out[5])}
 
 
 def nb_sync(c):

@@ -92,6 +92,10 @@ class Context:
         """HOST arrays (numpy or pinned CPU tensors), fp64 contiguous; staged by the library."""
         nb.nb_set_j_host(self.h, first, m.shape[0], m, x, v, a, j, t)
 
+    def update_j_host(self, idx, m, x, v, a=None, j=None, t=None):
+        """HOST int32 idx and HOST fp64 arrays of the idx.shape[0] updated particles."""
+        nb.nb_update_j_host(self.h, idx, idx.shape[0], m, x, v, a, j, t)
+
     def force_host(self, i_list, eps2, acc, jrk, pot):
         """HOST int32 i_list and HOST fp64 outputs acc, jrk (3, ni), pot (ni,); returns after
         the results are back on the host."""

@@ -28,6 +28,8 @@ struct nb_ctx {
     int* err = nullptr;
     int32_t* h_ilist = nullptr;   // device staging for the *_host force call
     double* h_out = nullptr;      // [7][ni_max]
+    double* h_in = nullptr;       // [14][ni_pad] staging of nb_update_j_host
+    int64_t ni_pad = 0;
 
     int* err_pinned = nullptr;
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
@@ -38,10 +40,17 @@ struct nb_ctx {
     int64_t last[4] = {0, 0, 0, 0};
     int64_t launches = 0;
 
-    // optional per-kernel timing (nb_set_profiling): events recorded on the context's stream
+    // optional per-kernel timing (nb_set_profiling): a ring of event records on the context's
+    // stream, drained into running sums by nb_kernel_times (or when the ring is full)
     bool prof = false;
-    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // predict [0,1], pair [2,3], reduce [3,4]
-    bool ev_predict = false, ev_force = false;
+    struct Rec {
+        cudaEvent_t e[3] = {nullptr, nullptr, nullptr};   // kind 0: predict [0,1]; kind 1: pair [0,1], reduce [1,2]
+        int kind = -1;
+    };
+    std::vector<Rec> ring;
+    size_t ring_used = 0;
+    double prof_ms[3] = {0, 0, 0};
+    int64_t prof_n[3] = {0, 0, 0};
 };
 
 namespace {
@@ -50,7 +59,8 @@ constexpr size_t ALIGN = 256;
 inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t store, pack, flags, tileflag, flag_list, part, err, ilist, out, total;
+    size_t store, pack, flags, tileflag, flag_list, part, err, ilist, out, in, total;
+    int64_t ni_pad;
     size_t part_bytes;
     int64_t n_cap;
 };
@@ -74,6 +84,8 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.err = off; off += up(sizeof(int));
     L.ilist = off; off += up((size_t)ni_pad * 4);
     L.out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
+    L.in = off; off += up((size_t)NFIELD * ni_pad * sizeof(double));
+    L.ni_pad = ni_pad;
     L.total = off;
     return L;
 }
@@ -106,11 +118,11 @@ int ensure_alloc(nb_ctx* c)
     c->err = reinterpret_cast<int*>(c->slab + L.err);
     c->h_ilist = reinterpret_cast<int32_t*>(c->slab + L.ilist);
     c->h_out = reinterpret_cast<double*>(c->slab + L.out);
+    c->h_in = reinterpret_cast<double*>(c->slab + L.in);
+    c->ni_pad = L.ni_pad;
     c->allocated = true;
     return NB_OK;
 }
-
-inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NB_OK : NB_ERR_CUDA; }
 
 struct DeviceGuard {
     int prev = -1;
@@ -125,6 +137,38 @@ struct DeviceGuard {
         if (prev >= 0) cudaSetDevice(prev);
     }
 };
+
+constexpr size_t PROF_RING = 256;
+
+// Sum the finished records into prof_ms / prof_n (synchronises the stream).
+int prof_drain(nb_ctx* c)
+{
+    if (c->ring_used == 0) return NB_OK;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    for (size_t r = 0; r < c->ring_used; ++r) {
+        nb_ctx::Rec& R = c->ring[r];
+        float ms = 0.f;
+        if (R.kind == 0) {
+            if (cudaEventElapsedTime(&ms, R.e[0], R.e[1]) != cudaSuccess) return NB_ERR_CUDA;
+            c->prof_ms[0] += ms; c->prof_n[0] += 1;
+        } else if (R.kind == 1) {
+            if (cudaEventElapsedTime(&ms, R.e[0], R.e[1]) != cudaSuccess) return NB_ERR_CUDA;
+            c->prof_ms[1] += ms; c->prof_n[1] += 1;
+            if (cudaEventElapsedTime(&ms, R.e[1], R.e[2]) != cudaSuccess) return NB_ERR_CUDA;
+            c->prof_ms[2] += ms; c->prof_n[2] += 1;
+        }
+        R.kind = -1;
+    }
+    c->ring_used = 0;
+    return NB_OK;
+}
+
+nb_ctx::Rec* prof_next(nb_ctx* c)
+{
+    if (!c->prof) return nullptr;
+    if (c->ring_used == c->ring.size() && prof_drain(c) != NB_OK) return nullptr;
+    return &c->ring[c->ring_used];
+}
 
 SrcPtrs make_src(const double* m, const double* x, const double* y, const double* z,
                  const double* vx, const double* vy, const double* vz, const double* ax,
@@ -187,6 +231,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     const int mode = c->tune_reduce ? 1 : 0;
     int launched = 0;
     cudaError_t e = cudaSuccess;
+    nb_ctx::Rec* rec = nullptr;
     if (a.ntiles > 0) {
         a.splits = choose_splits(c, a.n_itiles, a.ntiles, a.ni_pad);
         if (mode) {
@@ -194,10 +239,11 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             if (e != cudaSuccess) return NB_ERR_CUDA;
             ++launched;
         }
-        if (c->prof) cudaEventRecord(c->ev[2], c->stream);
+        rec = prof_next(c);
+        if (rec) cudaEventRecord(rec->e[0], c->stream);
         e = launch_force(a, mode, acc, jrk, pot, c->stream);
         if (e != cudaSuccess) return NB_ERR_CUDA;
-        if (c->prof) cudaEventRecord(c->ev[3], c->stream);
+        if (rec) cudaEventRecord(rec->e[1], c->stream);
         ++launched;
     } else {
         a.splits = 0;   // n == 0: the reduction of zero partials writes zeros
@@ -220,9 +266,10 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     r.atomic_mode = (mode && a.ntiles > 0) ? 1 : 0;
     e = launch_reduce(r, c->stream);
     if (e != cudaSuccess) return NB_ERR_CUDA;
-    if (c->prof && a.ntiles > 0) {
-        cudaEventRecord(c->ev[4], c->stream);
-        c->ev_force = true;
+    if (rec) {
+        cudaEventRecord(rec->e[2], c->stream);
+        rec->kind = 1;
+        c->ring_used += 1;
     }
     ++launched;
     c->last[0] = a.splits;
@@ -303,8 +350,9 @@ int nb_destroy(nb_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->own_slab && c->slab) cudaFree(c->slab);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
-    for (cudaEvent_t e : c->ev)
-        if (e) cudaEventDestroy(e);
+    for (nb_ctx::Rec& R : c->ring)
+        for (cudaEvent_t e : R.e)
+            if (e) cudaEventDestroy(e);
     delete c;
     return NB_OK;
 }
@@ -388,6 +436,37 @@ int nb_update_j(nb_ctx* c, const int32_t* idx, int64_t count, const double* m, c
     return NB_OK;
 }
 
+int nb_update_j_host(nb_ctx* c, const int32_t* idx, int64_t count, const double* m, const double* x,
+                     const double* y, const double* z, const double* vx, const double* vy,
+                     const double* vz, const double* ax, const double* ay, const double* az,
+                     const double* jx, const double* jy, const double* jz, const double* t)
+{
+    if (!c || count < 0 || count > c->ni_max || (count > 0 && !idx)) return NB_ERR_ARG;
+    if (count == 0) return NB_OK;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    const SrcPtrs host = make_src(m, x, y, z, vx, vy, vz, ax, ay, az, jx, jy, jz, t);
+    SrcPtrs dev{};
+    if (cudaMemcpyAsync(c->h_ilist, idx, (size_t)count * 4, cudaMemcpyHostToDevice, c->stream) !=
+        cudaSuccess)
+        return NB_ERR_CUDA;
+    for (int f = 0; f < NFIELD; ++f) {
+        dev.f[f] = nullptr;
+        if (!host.f[f]) continue;
+        double* stage = c->h_in + (size_t)f * c->ni_pad;
+        if (cudaMemcpyAsync(stage, host.f[f], (size_t)count * sizeof(double), cudaMemcpyHostToDevice,
+                            c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        dev.f[f] = stage;
+    }
+    if (launch_update_j(c->store, dev, c->h_ilist, count, c->n, c->err, c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    c->launches += 1;
+    c->predicted = false;
+    return NB_OK;
+}
+
 int nb_clear(nb_ctx* c)
 {
     if (!c) return NB_ERR_ARG;
@@ -454,12 +533,14 @@ int nb_predict(nb_ctx* c, double t)
     DeviceGuard g(c->device);
     int rc = ensure_alloc(c);
     if (rc != NB_OK) return rc;
-    if (c->prof) cudaEventRecord(c->ev[0], c->stream);
+    nb_ctx::Rec* rec = c->n > 0 ? prof_next(c) : nullptr;
+    if (rec) cudaEventRecord(rec->e[0], c->stream);
     if (launch_predict(c->store, c->flags, c->pack, c->n, t, c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
-    if (c->prof) {
-        cudaEventRecord(c->ev[1], c->stream);
-        c->ev_predict = true;
+    if (rec) {
+        cudaEventRecord(rec->e[1], c->stream);
+        rec->kind = 0;
+        c->ring_used += 1;
     }
     if (c->n > 0) c->launches += 1;
     c->predicted = true;
@@ -532,32 +613,35 @@ int nb_set_profiling(nb_ctx* c, int on)
 {
     if (!c) return NB_ERR_ARG;
     DeviceGuard g(c->device);
-    if (on && !c->ev[0]) {
-        for (cudaEvent_t& e : c->ev)
-            if (cudaEventCreate(&e) != cudaSuccess) return NB_ERR_CUDA;
+    if (c->prof) {
+        int rc = prof_drain(c);
+        if (rc != NB_OK) return rc;
+    }
+    if (on && c->ring.empty()) {
+        c->ring.resize(PROF_RING);
+        for (nb_ctx::Rec& R : c->ring)
+            for (cudaEvent_t& e : R.e)
+                if (cudaEventCreate(&e) != cudaSuccess) return NB_ERR_CUDA;
     }
     c->prof = on != 0;
-    c->ev_predict = c->ev_force = false;
+    for (int k = 0; k < 3; ++k) {
+        c->prof_ms[k] = 0.0;
+        c->prof_n[k] = 0;
+    }
     return NB_OK;
 }
 
-int nb_kernel_times(nb_ctx* c, double* out_ms)
+int nb_kernel_times(nb_ctx* c, double* out)
 {
-    if (!c || !out_ms) return NB_ERR_ARG;
+    if (!c || !out) return NB_ERR_ARG;
     DeviceGuard g(c->device);
-    out_ms[0] = out_ms[1] = out_ms[2] = -1.0;
+    for (int k = 0; k < 6; ++k) out[k] = 0.0;
     if (!c->prof) return NB_ERR_STATE;
-    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
-    float ms = 0.f;
-    if (c->ev_predict) {
-        if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) != cudaSuccess) return NB_ERR_CUDA;
-        out_ms[0] = ms;
-    }
-    if (c->ev_force) {
-        if (cudaEventElapsedTime(&ms, c->ev[2], c->ev[3]) != cudaSuccess) return NB_ERR_CUDA;
-        out_ms[1] = ms;
-        if (cudaEventElapsedTime(&ms, c->ev[3], c->ev[4]) != cudaSuccess) return NB_ERR_CUDA;
-        out_ms[2] = ms;
+    int rc = prof_drain(c);
+    if (rc != NB_OK) return rc;
+    for (int k = 0; k < 3; ++k) {
+        out[k] = c->prof_ms[k];
+        out[3 + k] = (double)c->prof_n[k];
     }
     return NB_OK;
 }
