@@ -150,6 +150,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STAGES * TILE_BYTES);
+    int* rel = reinterpret_cast<int*>(smem_raw + STAGES * TILE_BYTES + STAGES * 8);
 
     const int tid = threadIdx.x;
     const int it = blockIdx.x % P.n_itiles;       // neighbouring CTAs share the j-subset (L2 reuse)
@@ -159,7 +160,10 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 
     // a4: the j-subset of this CTA is tiles [t0, t1).  Thread 0 runs the copy ring.
     if (tid == 0) {
-        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&bars[s]), 1);
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(smem_u32(&bars[s]), 1);
+            rel[s] = 0;
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         for (int s = 0; s < STAGES && t0 + s < t1; ++s) {
             mbar_expect_tx(smem_u32(&bars[s]), TILE_BYTES);
@@ -172,6 +176,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
     IPart I[IPT];
     int idx[IPT];
     bool iflag[IPT];
+    float mi[IPT];
     int k[IPT];
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
@@ -187,6 +192,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         I[u].nxh = dup(-b[P_XH * TJ]); I[u].nyh = dup(-b[P_YH * TJ]); I[u].nzh = dup(-b[P_ZH * TJ]);
         I[u].nxl = dup(-b[P_XL * TJ]); I[u].nyl = dup(-b[P_YL * TJ]); I[u].nzl = dup(-b[P_ZL * TJ]);
         I[u].nvx = dup(-b[P_VX * TJ]); I[u].nvy = dup(-b[P_VY * TJ]); I[u].nvz = dup(-b[P_VZ * TJ]);
+        mi[u] = b[P_M * TJ];
         iflag[u] = P.any_flagged && (P.flags[q] & 1);
     }
 
@@ -201,20 +207,23 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 #pragma unroll
         for (int c = 0; c < NOUT; ++c) D[u][c] = 0.0;
     }
-    __syncthreads();   // barrier inits visible to all waiters
+    __syncthreads();   // barrier inits and the zeroed release counters visible to all warps
 
-    // a3: pair loop over the tiles of the subset
+    // a3: pair loop over the tiles of the subset.  No CTA-wide barrier inside: a warp that is done
+    // with a stage bumps the stage's release counter, and the warp that brings it to a multiple of
+    // NWARPS (the last one out) refills the stage, so warps drift up to STAGES-1 tiles apart.
     for (int t = t0; t < t1; ++t) {
         const int st = (t - t0) % STAGES;
         mbar_wait(smem_u32(&bars[st]), ((t - t0) / STAGES) & 1);
         const float* T = tiles + st * TILE_FLOATS;
 
+        // The self pair needs no mask when eps2 > 0 (r = w = 0 exactly: it adds nothing to acc and
+        // jerk, and m_i/eps to pot, which the tail takes back); only eps2 == 0 and flagged-flagged
+        // pairs (R6, R7) go through the masked path.
         bool slow = eps0;
 #pragma unroll
-        for (int u = 0; u < IPT; ++u) {
-            slow |= (idx[u] >= t * TJ) && (idx[u] < (t + 1) * TJ);
+        for (int u = 0; u < IPT; ++u)
             if (iflag[u]) slow |= (P.tileflag[t >> 5] >> (t & 31)) & 1u;
-        }
         if (!__any_sync(0xffffffffu, slow)) {
 #pragma unroll 2
             for (int p = 0; p < TJ; p += 4) {
@@ -240,18 +249,31 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
             for (int p = 0; p < TJ; ++p) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)
-                    pair1_masked(I[u], A[u], T, p, idx[u] == t * TJ + p, iflag[u], P.eps2);
+                    pair1_masked(I[u], A[u], T, p, (eps0 || iflag[u]) && idx[u] == t * TJ + p,
+                                 iflag[u], P.eps2);
             }
         }
 #pragma unroll
         for (int u = 0; u < IPT; ++u) flush(A[u], D[u]);
 
-        __syncthreads();   // every warp is done with this stage: refill it
-        if (tid == 0 && t + STAGES < t1) {
-            mbar_expect_tx(smem_u32(&bars[st]), TILE_BYTES);
-            bulk_g2s(smem_u32(tiles + st * TILE_FLOATS), P.pack + (int64_t)(t + STAGES) * TILE_FLOATS,
-                     TILE_BYTES, smem_u32(&bars[st]));
+        // release the stage; the last warp out refills it with tile t + STAGES
+        __syncwarp();
+        if ((tid & 31) == 0) {
+            const int old = atomicAdd(&rel[st], 1);
+            if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STAGES < t1) {
+                mbar_expect_tx(smem_u32(&bars[st]), TILE_BYTES);
+                bulk_g2s(smem_u32(tiles + st * TILE_FLOATS),
+                         P.pack + (int64_t)(t + STAGES) * TILE_FLOATS, TILE_BYTES, smem_u32(&bars[st]));
+            }
         }
+    }
+
+    // a5 (first half): take back the self term of pot where the unmasked path included it
+    if (!eps0) {
+        const float rinv_e = rsqrt_fast(P.eps2);
+#pragma unroll
+        for (int u = 0; u < IPT; ++u)
+            if (!iflag[u] && idx[u] >= t0 * TJ && idx[u] < t1 * TJ) D[u][6] += (double)(mi[u] * rinv_e);
     }
 
     // a4: partial sums of this j-subset (second kernel adds them), or atomics (:63)
@@ -354,7 +376,9 @@ __global__ void __launch_bounds__(256) zero_out_kernel(double* acc, double* jrk,
     pot[k] = 0.0;
 }
 
-constexpr int FORCE_SMEM = STAGES * TILE_BYTES + STAGES * 8;
+constexpr int NWARPS_CHECK = FORCE_THREADS / 32;
+static_assert((NWARPS_CHECK & (NWARPS_CHECK - 1)) == 0, "warps per CTA must be a power of two");
+constexpr int FORCE_SMEM = STAGES * TILE_BYTES + STAGES * 8 + STAGES * 4;
 
 }  // namespace
 

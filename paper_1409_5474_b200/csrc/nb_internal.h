@@ -23,6 +23,7 @@ constexpr int TILE_BYTES = TILE_FLOATS * 4;   // 5632 (multiple of 16: legal bul
 
 // pair kernel shape
 constexpr int FORCE_THREADS = 128;
+constexpr int NWARPS = FORCE_THREADS / 32;
 constexpr int IPT = 2;                        // i-particles per thread
 constexpr int ITILE = FORCE_THREADS * IPT;    // i-particles per CTA
 constexpr int STAGES = 4;                     // j-tile ring depth
