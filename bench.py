@@ -46,6 +46,9 @@ def parse():
     ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg2", "cfg4", "cfg5", "small"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="also time nb_force alone on every active-subset size of the workload "
+                         "(config 3: 1, 1024, 16384, 262144, 2^20) and add it as \"sweep\"")
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target duration of the cpu_baseline sample")
     return ap.parse_args()
@@ -334,6 +337,36 @@ def run_ours(args):
                "ms_per_step": ms_h / args.steps, "wall_ms_per_step": wall / args.steps * 1e3,
                "api": "nb_update_j_host + nb_predict + nb_force_host (pinned host buffers)"}
 
+    sweep = None
+    if args.sweep and world == 1:
+        # force call alone (gather + pairs + reduce), device-resident, per active-subset size:
+        # the few-i regime is bound by streaming the packed j-set (44 B per j), not by FP32
+        sweep = []
+        for sub in case.i_lists:
+            ns = len(sub)
+            d_sub = torch.from_numpy(np.ascontiguousarray(sub)).to(dev)
+            o = [torch.empty((3, ns), dtype=torch.float64, device=dev),
+                 torch.empty((3, ns), dtype=torch.float64, device=dev),
+                 torch.empty((ns,), dtype=torch.float64, device=dev)]
+            reps = 3 if ns * n > 1e11 else (20 if ns * n > 1e9 else 200)
+
+            def call():
+                nb.nb_force(h, d_sub, ns, case.eps2, *o)
+            for _ in range(3):
+                call()
+            best = min(timed(lambda: [call() for _ in range(reps)], 1) for _ in range(3)) / reps
+            info = ctx.last_launch()
+            ctx.profiling(True)
+            for _ in range(min(reps, 50)):
+                call()
+            kts = ctx.kernel_times()
+            ctx.profiling(False)
+            sweep.append({"n_i": ns, "ms_per_call": best, "interactions_per_s": ns * n / (best * 1e-3),
+                          "frac_fp32_peak": None, "pack_gbs": 44.0 * n / (best * 1e-3) / 1e9,
+                          "j_splits": int(info["j_splits"]), "ctas": int(info["ctas"]),
+                          "pair_ms": kts["pair_ms"] / max(kts["n_pair"], 1),
+                          "reduce_ms": kts["reduce_ms"] / max(kts["n_reduce"], 1)})
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -381,6 +414,10 @@ def run_ours(args):
         "roofline": roofline, "roofline_predict": roofline_predict,
         "kernels_ms": {"predict": pred_ms, "pair": pair_ms, "reduce": red_ms},
     }
+    if sweep is not None:
+        for q in sweep:
+            q["frac_fp32_peak"] = q["interactions_per_s"] * FLOP_PER_INTERACTION / 1e12 / fp32_peak_tflops
+        line["sweep"] = sweep
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = oracle_sample(case, il, t, args.cpu_seconds)
     ctx.close()

@@ -150,8 +150,10 @@ int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
  * default), 1 = fp64 atomics into the output (sum order varies run to run). */
 int nb_set_tuning(nb_ctx* c, int j_splits, int reduce_mode);
 
-/* What the last nb_force launched: out[0] = j-splits used, out[1] = CTAs of the pair kernel,
- * out[2] = kernels launched by the call, out[3] = kernel variant id.  HOST int64[4]. */
+/* What the last nb_force launched: out[0] = j-splits used (when the active list is cut in a
+ * whole-wave segment with one j-subset and a remainder segment with several, the remainder's
+ * count), out[1] = CTAs of the pair kernel launches together, out[2] = kernels launched by the
+ * call, out[3] = reduce mode.  HOST int64[4]. */
 int nb_last_launch(const nb_ctx* c, int64_t* out);
 
 /* Total kernels this context has launched since creation (bench.py's gpu_launches). */

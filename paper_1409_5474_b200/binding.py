@@ -8,7 +8,7 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libnb.so")
+LIB_PATH = os.environ.get("NB_LIBRARY") or os.path.join(_HERE, "libnb.so")   # NB_LIBRARY: another build
 
 NB_OK, NB_ERR_ARG, NB_ERR_ALLOC, NB_ERR_CUDA = 0, -1, -2, -3
 NB_ERR_INDEX, NB_ERR_STATE, NB_ERR_ARCH = -4, -5, -6

@@ -142,15 +142,23 @@ __device__ __forceinline__ void flush(Acc32& A, double* d)
     A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.p = make_float2(0.f, 0.f);
 }
 
-template <bool ATOMIC>
-__global__ void __launch_bounds__(FORCE_THREADS, 3)
+// JL = threads that share one i-particle ("split the j-particles in subsets" when few
+// i are active; here inside the CTA).  The 256 i-slots of a CTA then hold ITILE / JL particles, lane
+// jl of an i covers TJ / JL consecutive j of every tile, and the JL partial sums meet in a shuffle
+// butterfly before the CTA's partial is written.  JL = 1 is the all-i kernel.
+// ring depth: the few-i variants do little arithmetic per tile and live on bytes in flight
+__host__ __device__ constexpr int stages_for(int jl) { return jl == 1 ? STAGES : 2 * STAGES; }
+
+template <bool ATOMIC, int JL>
+__global__ void __launch_bounds__(FORCE_THREADS, NB_MINB)
 force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
              double* __restrict__ opot)
 {
+    constexpr int STG = stages_for(JL);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STAGES * TILE_BYTES);
-    int* rel = reinterpret_cast<int*>(smem_raw + STAGES * TILE_BYTES + STAGES * 8);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG * TILE_BYTES);
+    int* rel = reinterpret_cast<int*>(smem_raw + STG * TILE_BYTES + STG * 8);
 
     const int tid = threadIdx.x;
     const int it = blockIdx.x % P.n_itiles;       // neighbouring CTAs share the j-subset (L2 reuse)
@@ -160,12 +168,12 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 
     // a4: the j-subset of this CTA is tiles [t0, t1).  Thread 0 runs the copy ring.
     if (tid == 0) {
-        for (int s = 0; s < STAGES; ++s) {
+        for (int s = 0; s < STG; ++s) {
             mbar_init(smem_u32(&bars[s]), 1);
             rel[s] = 0;
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        for (int s = 0; s < STAGES && t0 + s < t1; ++s) {
+        for (int s = 0; s < STG && t0 + s < t1; ++s) {
             mbar_expect_tx(smem_u32(&bars[s]), TILE_BYTES);
             bulk_g2s(smem_u32(tiles + s * TILE_FLOATS), P.pack + (int64_t)(t0 + s) * TILE_FLOATS,
                      TILE_BYTES, smem_u32(&bars[s]));
@@ -180,14 +188,14 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
     int k[IPT];
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
-        k[u] = it * ITILE + u * FORCE_THREADS + tid;
-        int q = (k[u] < P.ni) ? P.i_list[k[u]] : 0;
+        k[u] = it * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;   // position inside the segment
+        int q = (P.k0 + k[u] < P.ni) ? P.i_list[P.k0 + k[u]] : 0;
         const bool bad = (q < 0) || (q >= P.n);
         if (bad) {
             atomicOr(P.err, 1);
             q = 0;
         }
-        idx[u] = (k[u] < P.ni && !bad) ? q : -1;
+        idx[u] = (P.k0 + k[u] < P.ni && !bad) ? q : -1;
         const float* b = P.pack + (int64_t)(q / TJ) * TILE_FLOATS + (q % TJ);
         I[u].nxh = dup(-b[P_XH * TJ]); I[u].nyh = dup(-b[P_YH * TJ]); I[u].nzh = dup(-b[P_ZH * TJ]);
         I[u].nxl = dup(-b[P_XL * TJ]); I[u].nyl = dup(-b[P_YL * TJ]); I[u].nzl = dup(-b[P_ZL * TJ]);
@@ -211,10 +219,10 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 
     // a3: pair loop over the tiles of the subset.  No CTA-wide barrier inside: a warp that is done
     // with a stage bumps the stage's release counter, and the warp that brings it to a multiple of
-    // NWARPS (the last one out) refills the stage, so warps drift up to STAGES-1 tiles apart.
+    // NWARPS (the last one out) refills the stage, so warps drift up to STG-1 tiles apart.
     for (int t = t0; t < t1; ++t) {
-        const int st = (t - t0) % STAGES;
-        mbar_wait(smem_u32(&bars[st]), ((t - t0) / STAGES) & 1);
+        const int st = (t - t0) % STG;
+        mbar_wait(smem_u32(&bars[st]), ((t - t0) / STG) & 1);
         const float* T = tiles + st * TILE_FLOATS;
 
         // The self pair needs no mask when eps2 > 0 (r = w = 0 exactly: it adds nothing to acc and
@@ -224,9 +232,12 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 #pragma unroll
         for (int u = 0; u < IPT; ++u)
             if (iflag[u]) slow |= (P.tileflag[t >> 5] >> (t & 31)) & 1u;
+        constexpr int JPT = TJ / JL;              // j per thread per tile
+        constexpr int UNROLL_Q = NB_UNROLL;       // j-quads per trip of the pair loop
+        const int p0 = (tid % JL) * JPT;
         if (!__any_sync(0xffffffffu, slow)) {
-#pragma unroll 2
-            for (int p = 0; p < TJ; p += 4) {
+#pragma unroll UNROLL_Q
+            for (int p = p0; p < p0 + JPT; p += 4) {
                 float4 f[10];
 #pragma unroll
                 for (int c = 0; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
@@ -246,26 +257,41 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
             }
         } else {
 #pragma unroll 1
-            for (int p = 0; p < TJ; ++p) {
+            for (int p = p0; p < p0 + JPT; ++p) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)
                     pair1_masked(I[u], A[u], T, p, (eps0 || iflag[u]) && idx[u] == t * TJ + p,
                                  iflag[u], P.eps2);
             }
         }
+        // fp32 sums stay short (R17: 64 terms per lane) before they move to fp64
+        constexpr int FLUSH_EVERY = 2 * 64 / JPT > 1 ? 2 * 64 / JPT : 1;
+        if (FLUSH_EVERY == 1 || (t - t0) % FLUSH_EVERY == FLUSH_EVERY - 1 || t == t1 - 1) {
 #pragma unroll
-        for (int u = 0; u < IPT; ++u) flush(A[u], D[u]);
+            for (int u = 0; u < IPT; ++u) flush(A[u], D[u]);
+        }
 
-        // release the stage; the last warp out refills it with tile t + STAGES
+        // release the stage; the last warp out refills it with tile t + STG
         __syncwarp();
         if ((tid & 31) == 0) {
             const int old = atomicAdd(&rel[st], 1);
-            if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STAGES < t1) {
+            if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STG < t1) {
                 mbar_expect_tx(smem_u32(&bars[st]), TILE_BYTES);
                 bulk_g2s(smem_u32(tiles + st * TILE_FLOATS),
-                         P.pack + (int64_t)(t + STAGES) * TILE_FLOATS, TILE_BYTES, smem_u32(&bars[st]));
+                         P.pack + (int64_t)(t + STG) * TILE_FLOATS, TILE_BYTES, smem_u32(&bars[st]));
             }
         }
+    }
+
+    // a4 inside the CTA: the JL lanes of one i add their sums (fixed butterfly: deterministic)
+    if (JL > 1) {
+#pragma unroll
+        for (int u = 0; u < IPT; ++u)
+#pragma unroll
+            for (int c = 0; c < NOUT; ++c)
+#pragma unroll
+                for (int w = 1; w < JL; w <<= 1) D[u][c] += __shfl_xor_sync(0xffffffffu, D[u][c], w);
+        if (tid % JL != 0) return;
     }
 
     // a5 (first half): take back the self term of pot where the unmasked path included it
@@ -283,10 +309,10 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
             if (idx[u] >= 0) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    atomicAdd(oacc + (int64_t)c * P.ni + k[u], D[u][c]);
-                    atomicAdd(ojrk + (int64_t)c * P.ni + k[u], D[u][3 + c]);
+                    atomicAdd(oacc + (int64_t)c * P.ni + P.k0 + k[u], D[u][c]);
+                    atomicAdd(ojrk + (int64_t)c * P.ni + P.k0 + k[u], D[u][3 + c]);
                 }
-                atomicAdd(opot + k[u], D[u][6]);
+                atomicAdd(opot + P.k0 + k[u], D[u][6]);
             }
         } else {
 #pragma unroll
@@ -298,9 +324,14 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 
 // a4/a5: sum the S partials in a fixed order (deterministic), add the unsoftened flagged-flagged
 // pair terms in fp64 straight from the j-store (R7), NaN for rejected indices, store SoA.
+// WARP = one warp per i (lanes stride over the partials, fixed butterfly) for the few-i calls whose
+// many j-subsets would otherwise be summed by one thread; else one thread per i.
+template <bool WARP>
 __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = WARP ? gt / 32 : gt;
+    const int lane = threadIdx.x & 31;
     if (k >= R.ni) return;
     double o[NOUT];
     if (R.atomic_mode) {
@@ -313,11 +344,22 @@ __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
     } else {
 #pragma unroll
         for (int c = 0; c < NOUT; ++c) o[c] = 0.0;
-        for (int s = 0; s < R.splits; ++s) {
+        const bool in_b = k >= R.kA;
+        const double* part = in_b ? R.part_b : R.part;
+        const int64_t stride = in_b ? R.ni_pad_b : R.ni_pad;
+        const int kl = in_b ? k - R.kA : k, ns = in_b ? R.splits_b : R.splits;
+        for (int s = WARP ? lane : 0; s < ns; s += WARP ? 32 : 1) {
 #pragma unroll
-            for (int c = 0; c < NOUT; ++c) o[c] += R.part[((int64_t)s * NOUT + c) * R.ni_pad + k];
+            for (int c = 0; c < NOUT; ++c) o[c] += part[((int64_t)s * NOUT + c) * stride + kl];
+        }
+        if (WARP) {
+#pragma unroll
+            for (int c = 0; c < NOUT; ++c)
+#pragma unroll
+                for (int w = 16; w >= 1; w >>= 1) o[c] += __shfl_xor_sync(0xffffffffu, o[c], w);
         }
     }
+    if (WARP && lane != 0) return;
     const int i = R.i_list[k];
     if (i < 0 || i >= R.n) {
 #pragma unroll
@@ -378,36 +420,59 @@ __global__ void __launch_bounds__(256) zero_out_kernel(double* acc, double* jrk,
 
 constexpr int NWARPS_CHECK = FORCE_THREADS / 32;
 static_assert((NWARPS_CHECK & (NWARPS_CHECK - 1)) == 0, "warps per CTA must be a power of two");
-constexpr int FORCE_SMEM = STAGES * TILE_BYTES + STAGES * 8 + STAGES * 4;
+__host__ __device__ constexpr int force_smem(int jl) { return stages_for(jl) * (TILE_BYTES + 8 + 4); }
 
 }  // namespace
 
-cudaError_t force_kernel_setup(int* blocks_per_sm)
+template <int JL>
+cudaError_t setup_one(int* blocks)
 {
-    cudaError_t e = cudaFuncSetAttribute(force_kernel<false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, FORCE_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(force_kernel<false, JL>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, force_smem(JL));
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(force_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             FORCE_SMEM);
+    e = cudaFuncSetAttribute(force_kernel<true, JL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             force_smem(JL));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, force_kernel<false>,
-                                                         FORCE_THREADS, FORCE_SMEM);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks, force_kernel<false, JL>,
+                                                         FORCE_THREADS, force_smem(JL));
 }
 
-cudaError_t launch_force(const ForceArgs& a, int atomic_mode, double* acc, double* jrk, double* pot,
-                         cudaStream_t s)
+cudaError_t force_kernel_setup(int* blocks_per_sm)
+{
+    int b = 0;
+    cudaError_t e = setup_one<JL_MID>(&b);
+    if (e != cudaSuccess) return e;
+    e = setup_one<JL_MAX>(&b);
+    if (e != cudaSuccess) return e;
+    return setup_one<1>(blocks_per_sm);
+}
+
+template <int JL>
+void launch_one(const ForceArgs& a, int atomic_mode, double* acc, double* jrk, double* pot,
+                cudaStream_t s)
 {
     const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
     if (atomic_mode)
-        force_kernel<true><<<grid, FORCE_THREADS, FORCE_SMEM, s>>>(a, acc, jrk, pot);
+        force_kernel<true, JL><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
     else
-        force_kernel<false><<<grid, FORCE_THREADS, FORCE_SMEM, s>>>(a, acc, jrk, pot);
-    return cudaGetLastError();
+        force_kernel<false, JL><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
 }
 
+cudaError_t launch_force(const ForceArgs& a, int jl, int atomic_mode, double* acc, double* jrk,
+                         double* pot, cudaStream_t s)
+{
+    if (jl == JL_MAX) launch_one<JL_MAX>(a, atomic_mode, acc, jrk, pot, s);
+    else if (jl == JL_MID) launch_one<JL_MID>(a, atomic_mode, acc, jrk, pot, s);
+    else launch_one<1>(a, atomic_mode, acc, jrk, pot, s);
+    return cudaGetLastError();
+}
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s)
 {
-    reduce_kernel<<<(a.ni + 127) / 128, 128, 0, s>>>(a);
+    const int most = a.splits > a.splits_b ? a.splits : a.splits_b;
+    if (!a.atomic_mode && most > 8 && a.ni <= 4096)
+        reduce_kernel<true><<<(a.ni + 3) / 4, 128, 0, s>>>(a);
+    else
+        reduce_kernel<false><<<(a.ni + 127) / 128, 128, 0, s>>>(a);
     return cudaGetLastError();
 }
 

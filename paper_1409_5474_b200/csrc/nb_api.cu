@@ -183,10 +183,10 @@ SrcPtrs make_src(const double* m, const double* x, const double* y, const double
 
 // choose the number of j-subsets S so that (i-tiles x S) fills the chip.  Efficiency
 // of a choice = useful tile-passes / (waves x resident CTAs x tiles per CTA).
-int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad)
+int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t part_bytes)
 {
     const int64_t resident = (int64_t)c->sm_count * c->blocks_per_sm;
-    int64_t smax = (int64_t)(c->part_bytes / (NOUT * sizeof(double) * (size_t)ni_pad));
+    int64_t smax = (int64_t)(part_bytes / (NOUT * sizeof(double) * (size_t)ni_pad));
     if (smax > ntiles) smax = ntiles;
     if (smax > 4096) smax = 4096;
     if (smax < 1) smax = 1;
@@ -217,39 +217,70 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     ForceArgs a{};
     a.pack = c->pack;
     a.i_list = i_list;
-    a.part = c->part;
     a.flags = c->flags;
     a.tileflag = c->tileflag;
     a.err = c->err;
     a.ni = (int)ni;
-    a.n_itiles = (int)((ni + ITILE - 1) / ITILE);
-    a.ni_pad = a.n_itiles * ITILE;
     a.n = (int)n_launch;
     a.ntiles = (int)((n_launch + TJ - 1) / TJ);
     a.eps2 = (float)eps2;
     a.any_flagged = c->flagged.empty() ? 0 : 1;
     const int mode = c->tune_reduce ? 1 : 0;
+    // few active i: several threads share one i-particle and split the j of a tile
+    const int jl = ni <= ITILE / JL_MAX ? JL_MAX : (ni <= ITILE / JL_MID ? JL_MID : 1);
+    const int itile = ITILE / jl;
+    const int n_itiles = (int)((ni + itile - 1) / itile);
+    const int resident = c->sm_count * c->blocks_per_sm;
+
+    // the i-tiles are cut in two segments.  A = the largest multiple of the resident CTA
+    // count, one j-subset each (whole waves of equal CTAs); B = the rest, whose j is split in S
+    // subsets so that its CTAs fill the chip once more instead of leaving a ragged last wave.
+    int tiles_a = (c->tune_splits > 0) ? 0 : (n_itiles / resident) * resident;
+    int tiles_b = n_itiles - tiles_a;
+    int splits_a = tiles_a > 0 ? 1 : 0, splits_b = 0;
+    const int64_t pad_a = (int64_t)tiles_a * itile, pad_b = (int64_t)tiles_b * itile;
+    double* part_b = c->part + (size_t)NOUT * pad_a;
     int launched = 0;
-    cudaError_t e = cudaSuccess;
     nb_ctx::Rec* rec = nullptr;
     if (a.ntiles > 0) {
-        a.splits = choose_splits(c, a.n_itiles, a.ntiles, a.ni_pad);
+        if (tiles_b > 0) {
+            const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a;
+            splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left);
+        }
         if (mode) {
-            e = launch_zero_out(acc, jrk, pot, ni, c->stream);
-            if (e != cudaSuccess) return NB_ERR_CUDA;
+            if (launch_zero_out(acc, jrk, pot, ni, c->stream) != cudaSuccess) return NB_ERR_CUDA;
             ++launched;
         }
         rec = prof_next(c);
         if (rec) cudaEventRecord(rec->e[0], c->stream);
-        e = launch_force(a, mode, acc, jrk, pot, c->stream);
-        if (e != cudaSuccess) return NB_ERR_CUDA;
+        if (tiles_a > 0) {
+            a.k0 = 0;
+            a.n_itiles = tiles_a;
+            a.ni_pad = (int)pad_a;
+            a.splits = 1;
+            a.part = c->part;
+            if (launch_force(a, jl, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            ++launched;
+        }
+        if (tiles_b > 0) {
+            a.k0 = (int)pad_a;
+            a.n_itiles = tiles_b;
+            a.ni_pad = (int)pad_b;
+            a.splits = splits_b;
+            a.part = part_b;
+            if (launch_force(a, jl, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            ++launched;
+        }
         if (rec) cudaEventRecord(rec->e[1], c->stream);
-        ++launched;
     } else {
-        a.splits = 0;   // n == 0: the reduction of zero partials writes zeros
+        splits_a = splits_b = 0;   // n == 0: the reduction of zero partials writes zeros
     }
     ReduceArgs r{};
     r.part = c->part;
+    r.part_b = part_b;
+    r.kA = (int)pad_a;
+    r.ni_pad_b = (int)pad_b;
+    r.splits_b = splits_b;
     r.i_list = i_list;
     r.acc = acc;
     r.jrk = jrk;
@@ -259,21 +290,20 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     r.flag_list = c->flag_list;
     r.nflag = (int)c->flagged.size();
     r.ni = (int)ni;
-    r.ni_pad = a.ni_pad;
-    r.splits = a.splits;
+    r.ni_pad = (int)pad_a;
+    r.splits = splits_a;
     r.n = (int)n_launch;
     r.t_pred = c->t_pred;
     r.atomic_mode = (mode && a.ntiles > 0) ? 1 : 0;
-    e = launch_reduce(r, c->stream);
-    if (e != cudaSuccess) return NB_ERR_CUDA;
+    if (launch_reduce(r, c->stream) != cudaSuccess) return NB_ERR_CUDA;
     if (rec) {
         cudaEventRecord(rec->e[2], c->stream);
         rec->kind = 1;
         c->ring_used += 1;
     }
     ++launched;
-    c->last[0] = a.splits;
-    c->last[1] = (int64_t)a.n_itiles * a.splits;
+    c->last[0] = tiles_b > 0 ? splits_b : splits_a;
+    c->last[1] = (int64_t)tiles_a * splits_a + (int64_t)tiles_b * splits_b;
     c->last[2] = launched;
     c->last[3] = mode;
     c->launches += launched;

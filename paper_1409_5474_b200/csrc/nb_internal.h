@@ -16,7 +16,19 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 // pack: the force-ready predicted j-set, written by the predictor, streamed by the pair kernel.
 // Tiles of TJ particles, SoA inside a tile: NPF float arrays of TJ entries, so that one tile is one
 // contiguous 1-D bulk copy and two consecutive j's form an f32x2 operand pair.
-constexpr int TJ = 128;                       // j-particles per tile
+#ifndef NB_TJ
+#define NB_TJ 128
+#endif
+#ifndef NB_STAGES
+#define NB_STAGES 4
+#endif
+#ifndef NB_MINB
+#define NB_MINB 3
+#endif
+#ifndef NB_UNROLL
+#define NB_UNROLL 2
+#endif
+constexpr int TJ = NB_TJ;                     // j-particles per tile
 enum PackField { P_XH = 0, P_YH, P_ZH, P_XL, P_YL, P_ZL, P_VX, P_VY, P_VZ, P_M, P_FLAG, NPF };
 constexpr int TILE_FLOATS = TJ * NPF;         // 1408
 constexpr int TILE_BYTES = TILE_FLOATS * 4;   // 5632 (multiple of 16: legal bulk-copy size)
@@ -25,8 +37,9 @@ constexpr int TILE_BYTES = TILE_FLOATS * 4;   // 5632 (multiple of 16: legal bul
 constexpr int FORCE_THREADS = 128;
 constexpr int NWARPS = FORCE_THREADS / 32;
 constexpr int IPT = 2;                        // i-particles per thread
-constexpr int ITILE = FORCE_THREADS * IPT;    // i-particles per CTA
-constexpr int STAGES = 4;                     // j-tile ring depth
+constexpr int ITILE = FORCE_THREADS * IPT;    // i-slots per CTA (= i-particles when JL = 1)
+constexpr int JL_MID = 4, JL_MAX = 32;        // threads per i in the few-i variants (force.cu)
+constexpr int STAGES = NB_STAGES;             // j-tile ring depth
 constexpr int NOUT = 7;                       // ax ay az jx jy jz pot
 
 constexpr float PAD_POS = 1.0e10f;            // where the m = 0 padding records of the last tile sit
@@ -46,14 +59,18 @@ struct ForceArgs {
     const uint8_t* flags;     // [n_cap] bit 0: unsoftened among flagged
     const uint32_t* tileflag; // bit t: tile t holds a flagged particle
     int* err;                 // device error latch
-    int ni, ni_pad, n_itiles;
+    int ni;                   // length of i_list (bounds, output stride)
+    int k0;                   // first i_list position of this launch (segment), multiple of ITILE
+    int ni_pad, n_itiles;     // padded length and i-tiles of the segment
     int n, ntiles, splits;
     float eps2;
     int any_flagged;
 };
 
 struct ReduceArgs {
-    const double* part;
+    const double* part;       // segment A: [splits][NOUT][ni_pad], positions [0, kA)
+    const double* part_b;     // segment B: [splits_b][NOUT][ni_pad_b], positions [kA, ni)
+    int kA, ni_pad_b, splits_b;
     const int32_t* i_list;
     double *acc, *jrk, *pot;
     StorePtrs store;          // for the fp64 flagged-pair terms
@@ -75,8 +92,8 @@ cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* 
 cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
                                  double* out, cudaStream_t s);
 cudaError_t force_kernel_setup(int* blocks_per_sm);
-cudaError_t launch_force(const ForceArgs& a, int atomic_mode, double* acc, double* jrk, double* pot,
-                         cudaStream_t s);
+cudaError_t launch_force(const ForceArgs& a, int jl, int atomic_mode, double* acc, double* jrk,
+                         double* pot, cudaStream_t s);
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 

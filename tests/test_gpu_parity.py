@@ -172,6 +172,39 @@ def test_j_split_variants_agree(nbmod):
     assert all((p == q).all() for p, q in zip(again, outs[2]))    # deterministic (R9)
 
 
+@pytest.mark.parametrize("ni", [1, 3, 8, 9, 64, 65, 200])
+def test_few_active_i_share_threads(nbmod, ni):
+    """few i active -> several threads per i split the j of a tile (32 threads per i
+    up to 8 i, 4 up to 64), shuffle butterfly, warp-per-i reduction.  Includes a flagged i, its own
+    tile, and the self pair of every i."""
+    c = _random_case(6000, 94, eps2=2.0 ** -14)
+    c.flags[[11, 4000]] = 1
+    il = nbgen.permutation(95, c.n)[:ni].astype(np.int32)
+    il[0] = 11
+    ref = _oracle_force(c, 0.3, il)
+    for splits, mode in [(0, 0), (1, 0), (5, 0), (0, 1)]:
+        got, info = _gpu_force(nbmod, c, 0.3, il, splits=splits, mode=mode)
+        check_parity(got, ref)
+    got0, _ = _gpu_force(nbmod, c, 0.3, il, eps2=0.0)
+    check_parity(got0, _oracle_force(c, 0.3, il, eps2=0.0))
+
+
+def test_whole_wave_segment_plus_remainder(nbmod):
+    """More i-tiles than resident CTAs: the dispatcher runs whole waves with one j-subset and the
+    remainder with a split j (two pair-kernel launches, one reduction).  Duplicates keep N small."""
+    c = _random_case(3000, 92, eps2=2.0 ** -18)
+    c.flags[[7, 2999]] = 1
+    ni = 148 * 3 * 256 + 1234                                     # > 444 full i-tiles + a ragged one
+    il = (nbgen.permutation(93, ni) % c.n).astype(np.int32)
+    got, info = _gpu_force(nbmod, c, 0.1, il)
+    assert info["kernels"] >= 3 and info["ctas"] > 444
+    ref_all = _oracle_force(c, 0.1, np.arange(c.n, dtype=np.int32))
+    ref = [ref_all[0][:, il], ref_all[1][:, il], ref_all[2][il]]
+    check_parity(got, ref)
+    atom, _ = _gpu_force(nbmod, c, 0.1, il, mode=1)
+    check_parity(atom, ref)
+
+
 def test_i_subsets_duplicates_and_order(nbmod):
     c = _random_case(2048, 95)
     full, _ = _gpu_force(nbmod, c, 0.0, np.arange(c.n))
