@@ -130,15 +130,18 @@ __device__ __forceinline__ void pair1_masked(const IPart& I, Acc32& A, const flo
     A.jz.x = fmaf(mr3, fmaf(al, dz, wz), A.jz.x);
 }
 
+// S = distance between the 7 sums of one i: 1 when they sit in registers, FORCE_THREADS when they
+// sit in shared memory (the all-i kernel keeps them there: 28 registers fewer, no spill in the loop)
+template <int S>
 __device__ __forceinline__ void flush(Acc32& A, double* d)
 {
-    d[0] += (double)(A.ax.x + A.ax.y);
-    d[1] += (double)(A.ay.x + A.ay.y);
-    d[2] += (double)(A.az.x + A.az.y);
-    d[3] += (double)(A.jx.x + A.jx.y);
-    d[4] += (double)(A.jy.x + A.jy.y);
-    d[5] += (double)(A.jz.x + A.jz.y);
-    d[6] -= (double)(A.p.x + A.p.y);
+    d[0 * S] += (double)(A.ax.x + A.ax.y);
+    d[1 * S] += (double)(A.ay.x + A.ay.y);
+    d[2 * S] += (double)(A.az.x + A.az.y);
+    d[3 * S] += (double)(A.jx.x + A.jx.y);
+    d[4 * S] += (double)(A.jy.x + A.jy.y);
+    d[5 * S] += (double)(A.jz.x + A.jz.y);
+    d[6 * S] -= (double)(A.p.x + A.p.y);
     A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.p = make_float2(0.f, 0.f);
 }
 
@@ -159,6 +162,12 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
     float* tiles = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG * TILE_BYTES);
     int* rel = reinterpret_cast<int*>(smem_raw + STG * TILE_BYTES + STG * 8);
+    // JL == 1: the fp64 sums live in shared memory ([u][c][thread], touched once per tile)
+    constexpr bool DSM = (JL == 1);
+    double* sd = reinterpret_cast<double*>(smem_raw + STG * (TILE_BYTES + 16)) + threadIdx.x;
+    // index of each i (or -1), only needed in the masked path and in the tail: kept out of registers
+    int* sidx = reinterpret_cast<int*>(smem_raw + STG * (TILE_BYTES + 16) +
+                                       (DSM ? IPT * NOUT * FORCE_THREADS * 8 : 0)) + threadIdx.x;
 
     const int tid = threadIdx.x;
     const int it = blockIdx.x % P.n_itiles;       // neighbouring CTAs share the j-subset (L2 reuse)
@@ -182,38 +191,37 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 
     // a2: i-gather from the pack (two-float position = 48 bits, fp32 velocity; R8, R17)
     IPart I[IPT];
-    int idx[IPT];
-    bool iflag[IPT];
-    float mi[IPT];
-    int k[IPT];
+    unsigned iflags = 0;      // bit u: i-particle u carries the unsoftened flag (R7)
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
-        k[u] = it * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;   // position inside the segment
-        int q = (P.k0 + k[u] < P.ni) ? P.i_list[P.k0 + k[u]] : 0;
+        const int ku = it * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;   // position inside the segment
+        int q = (P.k0 + ku < P.ni) ? P.i_list[P.k0 + ku] : 0;
         const bool bad = (q < 0) || (q >= P.n);
         if (bad) {
             atomicOr(P.err, 1);
             q = 0;
         }
-        idx[u] = (P.k0 + k[u] < P.ni && !bad) ? q : -1;
+        sidx[u * FORCE_THREADS] = (P.k0 + ku < P.ni && !bad) ? q : -1;
         const float* b = P.pack + (int64_t)(q / TJ) * TILE_FLOATS + (q % TJ);
         I[u].nxh = dup(-b[P_XH * TJ]); I[u].nyh = dup(-b[P_YH * TJ]); I[u].nzh = dup(-b[P_ZH * TJ]);
         I[u].nxl = dup(-b[P_XL * TJ]); I[u].nyl = dup(-b[P_YL * TJ]); I[u].nzl = dup(-b[P_ZL * TJ]);
         I[u].nvx = dup(-b[P_VX * TJ]); I[u].nvy = dup(-b[P_VY * TJ]); I[u].nvz = dup(-b[P_VZ * TJ]);
-        mi[u] = b[P_M * TJ];
-        iflag[u] = P.any_flagged && (P.flags[q] & 1);
+        if (P.any_flagged && (P.flags[q] & 1)) iflags |= 1u << u;
     }
 
     const float2 eps2 = dup(P.eps2);
     const float2 m3 = dup(-3.0f);
     const bool eps0 = !(P.eps2 > 0.0f);
     Acc32 A[IPT];
-    double D[IPT][NOUT];
+    double D[DSM ? 1 : IPT][NOUT];
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
         A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
 #pragma unroll
-        for (int c = 0; c < NOUT; ++c) D[u][c] = 0.0;
+        for (int c = 0; c < NOUT; ++c) {
+            if (DSM) sd[(u * NOUT + c) * FORCE_THREADS] = 0.0;
+            else D[u][c] = 0.0;
+        }
     }
     __syncthreads();   // barrier inits and the zeroed release counters visible to all warps
 
@@ -229,9 +237,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         // jerk, and m_i/eps to pot, which the tail takes back); only eps2 == 0 and flagged-flagged
         // pairs (R6, R7) go through the masked path.
         bool slow = eps0;
-#pragma unroll
-        for (int u = 0; u < IPT; ++u)
-            if (iflag[u]) slow |= (P.tileflag[t >> 5] >> (t & 31)) & 1u;
+        if (iflags) slow |= (P.tileflag[t >> 5] >> (t & 31)) & 1u;
         constexpr int JPT = TJ / JL;              // j per thread per tile
         constexpr int UNROLL_Q = NB_UNROLL;       // j-quads per trip of the pair loop
         const int p0 = (tid % JL) * JPT;
@@ -260,15 +266,19 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
             for (int p = p0; p < p0 + JPT; ++p) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)
-                    pair1_masked(I[u], A[u], T, p, (eps0 || iflag[u]) && idx[u] == t * TJ + p,
-                                 iflag[u], P.eps2);
+                    pair1_masked(I[u], A[u], T, p,
+                                 (eps0 || ((iflags >> u) & 1u)) && sidx[u * FORCE_THREADS] == t * TJ + p,
+                                 (iflags >> u) & 1u, P.eps2);
             }
         }
         // fp32 sums stay short (R17: 64 terms per lane) before they move to fp64
         constexpr int FLUSH_EVERY = 2 * 64 / JPT > 1 ? 2 * 64 / JPT : 1;
         if (FLUSH_EVERY == 1 || (t - t0) % FLUSH_EVERY == FLUSH_EVERY - 1 || t == t1 - 1) {
 #pragma unroll
-            for (int u = 0; u < IPT; ++u) flush(A[u], D[u]);
+            for (int u = 0; u < IPT; ++u) {
+                if (DSM) flush<FORCE_THREADS>(A[u], sd + u * NOUT * FORCE_THREADS);
+                else flush<1>(A[u], D[DSM ? 0 : u]);
+            }
         }
 
         // release the stage; the last warp out refills it with tile t + STG
@@ -290,34 +300,46 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 #pragma unroll
             for (int c = 0; c < NOUT; ++c)
 #pragma unroll
-                for (int w = 1; w < JL; w <<= 1) D[u][c] += __shfl_xor_sync(0xffffffffu, D[u][c], w);
+                for (int w = 1; w < JL; w <<= 1)
+                    D[DSM ? 0 : u][c] += __shfl_xor_sync(0xffffffffu, D[DSM ? 0 : u][c], w);
         if (tid % JL != 0) return;
     }
 
     // a5 (first half): take back the self term of pot where the unmasked path included it
-    if (!eps0) {
-        const float rinv_e = rsqrt_fast(P.eps2);
-#pragma unroll
-        for (int u = 0; u < IPT; ++u)
-            if (!iflag[u] && idx[u] >= t0 * TJ && idx[u] < t1 * TJ) D[u][6] += (double)(mi[u] * rinv_e);
-    }
+    const float rinv_e = eps0 ? 0.0f : rsqrt_fast(P.eps2);
+    // the CTA's place in the grid is read again here, so that it does not hold registers through
+    // the pair loop (the all-i kernel then needs 130 registers and nothing spills)
+    unsigned bid;
+    asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(bid));
+    const int it2 = bid % P.n_itiles, sp2 = bid / P.n_itiles;
+    const int u0 = (int)(((int64_t)P.ntiles * sp2) / P.splits) * TJ;
+    const int u1 = (int)(((int64_t)P.ntiles * (sp2 + 1)) / P.splits) * TJ;
 
     // a4: partial sums of this j-subset (second kernel adds them), or atomics (:63)
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
+        double o[NOUT];
+#pragma unroll
+        for (int c = 0; c < NOUT; ++c) o[c] = DSM ? sd[(u * NOUT + c) * FORCE_THREADS] : D[DSM ? 0 : u][c];
+        const int ku = it2 * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;
+        const int q = sidx[u * FORCE_THREADS];
+        if (!eps0 && !((iflags >> u) & 1u) && q >= u0 && q < u1) {
+            const float mi = P.pack[(int64_t)(q / TJ) * TILE_FLOATS + P_M * TJ + (q % TJ)];
+            o[6] += (double)(mi * rinv_e);
+        }
         if (ATOMIC) {
-            if (idx[u] >= 0) {
+            if (q >= 0) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    atomicAdd(oacc + (int64_t)c * P.ni + P.k0 + k[u], D[u][c]);
-                    atomicAdd(ojrk + (int64_t)c * P.ni + P.k0 + k[u], D[u][3 + c]);
+                    atomicAdd(oacc + (int64_t)c * P.ni + P.k0 + ku, o[c]);
+                    atomicAdd(ojrk + (int64_t)c * P.ni + P.k0 + ku, o[3 + c]);
                 }
-                atomicAdd(opot + P.k0 + k[u], D[u][6]);
+                atomicAdd(opot + P.k0 + ku, o[6]);
             }
         } else {
 #pragma unroll
             for (int c = 0; c < NOUT; ++c)
-                P.part[((int64_t)sp * NOUT + c) * P.ni_pad + k[u]] = D[u][c];
+                P.part[((int64_t)sp2 * NOUT + c) * P.ni_pad + ku] = o[c];
         }
     }
 }
@@ -420,7 +442,11 @@ __global__ void __launch_bounds__(256) zero_out_kernel(double* acc, double* jrk,
 
 constexpr int NWARPS_CHECK = FORCE_THREADS / 32;
 static_assert((NWARPS_CHECK & (NWARPS_CHECK - 1)) == 0, "warps per CTA must be a power of two");
-__host__ __device__ constexpr int force_smem(int jl) { return stages_for(jl) * (TILE_BYTES + 8 + 4); }
+__host__ __device__ constexpr int force_smem(int jl)
+{
+    return stages_for(jl) * (TILE_BYTES + 16) + (jl == 1 ? IPT * NOUT * FORCE_THREADS * 8 : 0) +
+           IPT * FORCE_THREADS * 4;
+}
 
 }  // namespace
 
