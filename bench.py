@@ -387,6 +387,14 @@ def run_ours(args):
                     props.multi_processor_count, sm_max),
                 "ms_per_launch": pair_ms, "launches_timed": kt["n_pair"],
                 "share_of_step": kt["pair_ms"] / ms}
+    # what the FMA pipe sustains on this device with the pair kernel's instruction kinds
+    # (nb_probe_fp32: register-only full-chip kernels, outside the timed region)
+    rate_ffma, rate_ffma2 = ctx.probe_fp32(0), ctx.probe_fp32(1)
+    roofline["fma_probe"] = {
+        "ffma_tflops": 2 * rate_ffma / 1e12, "ffma2_tflops": 2 * rate_ffma2 / 1e12,
+        "frac_of_ffma2_rate": (ach * 1e12 / FLOP_PER_INTERACTION * 33.0) / rate_ffma2,
+        "note": "the pair body executes 33 FP32 lane-ops per interaction (DESIGN.md 7.2); "
+                "frac_of_ffma2_rate = executed lane-ops/s over the measured packed-FMA rate"}
     if clocks:
         obs = props.multi_processor_count * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12
         roofline["frac_at_observed_clock"] = ach / obs

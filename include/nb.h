@@ -168,6 +168,14 @@ int64_t nb_launch_count(const nb_ctx* c);
 int nb_set_profiling(nb_ctx* c, int on);
 int nb_kernel_times(nb_ctx* c, double* out_ms);
 
+/* Measure what the FP32 FMA pipe of this device sustains, with the instruction kinds the pair
+ * kernel is built from: kind 0 = scalar FFMA, kind 1 = packed FFMA2
+ * (fma.rn.f32x2).  Runs a short full-chip register-only kernel four times on the context's stream
+ * (synchronises it) and writes the best rate, in fused multiply-adds per second summed over all
+ * lanes, to HOST *lane_ops_per_s (nominal: SMs x 128 x clock).  Diagnostic for the roofline
+ * report, not part of the force path. */
+int nb_probe_fp32(nb_ctx* c, int kind, double* lane_ops_per_s);
+
 int nb_sync(nb_ctx* c);                 /* stream sync; returns and clears any latched error */
 const char* nb_strerror(int status);
 const char* nb_version(void);

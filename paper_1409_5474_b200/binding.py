@@ -18,7 +18,7 @@ EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_host", "nb_set_tuning",
-    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync", "nb_strerror", "nb_version",
+    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_probe_fp32", "nb_sync", "nb_strerror", "nb_version",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -56,6 +56,7 @@ lib.nb_kernel_times.argtypes = [_vp, ctypes.POINTER(_dbl)]
 lib.nb_sync.argtypes = [_vp]
 lib.nb_strerror.argtypes = [_i32]
 lib.nb_strerror.restype = ctypes.c_char_p
+lib.nb_probe_fp32.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(_dbl)]
 lib.nb_version.restype = ctypes.c_char_p
 
 
@@ -196,6 +197,13 @@ def nb_launch_count(c):
 
 def nb_set_profiling(c, on=True):
     _check(lib.nb_set_profiling(c, 1 if on else 0), "nb_set_profiling")
+
+
+def nb_probe_fp32(c, kind):
+    """FMA lane-operations per second the device sustains (kind 0 = FFMA, 1 = FFMA2)."""
+    out = _dbl(0.0)
+    _check(lib.nb_probe_fp32(c, int(kind), ctypes.byref(out)), "nb_probe_fp32")
+    return out.value
 
 
 def nb_kernel_times(c):

@@ -108,5 +108,9 @@ class Context:
     def kernel_times(self):
         return nb.nb_kernel_times(self.h)
 
+    def probe_fp32(self, kind):
+        """Sustained FMA lane-operations/s of the device (0 = FFMA, 1 = FFMA2)."""
+        return nb.nb_probe_fp32(self.h, kind)
+
     def launch_count(self):
         return nb.nb_launch_count(self.h)

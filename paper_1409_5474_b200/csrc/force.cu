@@ -131,7 +131,7 @@ __device__ __forceinline__ void pair1_masked(const IPart& I, Acc32& A, const flo
 }
 
 // S = distance between the 7 sums of one i: 1 when they sit in registers, FORCE_THREADS when they
-// sit in shared memory (the all-i kernel keeps them there: 28 registers fewer, no spill in the loop)
+// sit in shared memory (the all-i kernel keeps them there: 28 registers fewer, 4 CTAs per SM)
 template <int S>
 __device__ __forceinline__ void flush(Acc32& A, double* d)
 {
@@ -308,7 +308,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
     // a5 (first half): take back the self term of pot where the unmasked path included it
     const float rinv_e = eps0 ? 0.0f : rsqrt_fast(P.eps2);
     // the CTA's place in the grid is read again here, so that it does not hold registers through
-    // the pair loop (the all-i kernel then needs 130 registers and nothing spills)
+    // the pair loop (the all-i kernel then fits 128 registers unspilled: 4 CTAs per SM)
     unsigned bid;
     asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(bid));
     const int it2 = bid % P.n_itiles, sp2 = bid / P.n_itiles;

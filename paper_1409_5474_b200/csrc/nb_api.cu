@@ -78,7 +78,8 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.tileflag = off; off += up((size_t)(ntiles + 31) / 32 * 4);
     L.flag_list = off; off += up((size_t)NB_MAX_FLAGGED * 4);
     // partial sums: S * 7 * ni_pad doubles.  S = 1 needs 56 B per i; small i-sets want many splits.
-    L.part_bytes = (size_t)NOUT * sizeof(double) * (size_t)ni_pad * 2;
+    // 4x leaves the remainder segment of an all-active call room for ~16 j-subsets (a full last wave)
+    L.part_bytes = (size_t)NOUT * sizeof(double) * (size_t)ni_pad * 4;
     if (L.part_bytes < ((size_t)32 << 20)) L.part_bytes = (size_t)32 << 20;
     L.part = off; off += up(L.part_bytes);
     L.err = off; off += up(sizeof(int));
@@ -673,6 +674,22 @@ int nb_kernel_times(nb_ctx* c, double* out)
         out[k] = c->prof_ms[k];
         out[3 + k] = (double)c->prof_n[k];
     }
+    return NB_OK;
+}
+
+int nb_probe_fp32(nb_ctx* c, int kind, double* lane_ops_per_s)
+{
+    if (!c || !lane_ops_per_s || (kind != 0 && kind != 1)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    // scratch: the partial buffer (>= 32 MiB; the probe writes sm_count x 8 x 128 floats); the
+    // probe synchronises the stream, so no force call is in flight on it
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    if (probe_fp32(kind, c->sm_count, reinterpret_cast<float*>(c->part), c->stream, lane_ops_per_s) !=
+        cudaSuccess)
+        return NB_ERR_CUDA;
+    c->launches += 4;
     return NB_OK;
 }
 

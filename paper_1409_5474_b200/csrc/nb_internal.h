@@ -95,6 +95,7 @@ cudaError_t force_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_force(const ForceArgs& a, int jl, int atomic_mode, double* acc, double* jrk,
                          double* pot, cudaStream_t s);
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);
+cudaError_t probe_fp32(int kind, int sm_count, float* scratch, cudaStream_t s, double* lane_ops_per_s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 
 // Hermite predictor of one component (R1), shared by predict / get_predicted / the flagged-pair

@@ -194,10 +194,11 @@ def test_whole_wave_segment_plus_remainder(nbmod):
     remainder with a split j (two pair-kernel launches, one reduction).  Duplicates keep N small."""
     c = _random_case(3000, 92, eps2=2.0 ** -18)
     c.flags[[7, 2999]] = 1
-    ni = 148 * 3 * 256 + 1234                                     # > 444 full i-tiles + a ragged one
+    ni = 148 * 4 * 256 + 1234                                     # > 592 full i-tiles + a ragged one
     il = (nbgen.permutation(93, ni) % c.n).astype(np.int32)
     got, info = _gpu_force(nbmod, c, 0.1, il)
-    assert info["kernels"] >= 3 and info["ctas"] > 444
+    # whether 3 or 4 CTAs are resident per SM, a whole-wave segment and a split remainder exist
+    assert info["kernels"] >= 3 and info["ctas"] > (ni + 255) // 256
     ref_all = _oracle_force(c, 0.1, np.arange(c.n, dtype=np.int32))
     ref = [ref_all[0][:, il], ref_all[1][:, il], ref_all[2][il]]
     check_parity(got, ref)
