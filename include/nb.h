@@ -46,8 +46,8 @@ typedef enum {
 
 /* Create a context for up to n_max j-particles and up to ni_max i-particles per force call, on
  * CUDA device `device`, enqueuing on `stream` (a cudaStream_t passed as void*; NULL = legacy
- * default stream).  Internal buffers (j-store 112 B, predicted state 48 B, packed force record
- * 48 B per particle, plus the partial-force buffer) are allocated on first use with cudaMalloc,
+ * default stream).  Internal buffers (j-store 112 B + step 8 B, packed force record 44 B per
+ * particle, plus the partial-force and block buffers) are allocated on first use with cudaMalloc,
  * unless nb_set_workspace lent memory before that. */
 int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* stream);
 int nb_destroy(nb_ctx* c);
@@ -167,6 +167,53 @@ int64_t nb_launch_count(const nb_ctx* c);
  * nb_set_profiling(on) resets the totals.  NB_ERR_STATE if profiling is off. */
 int nb_set_profiling(nb_ctx* c, int on);
 int nb_kernel_times(nb_ctx* c, double* out_ms);
+
+/* ---- block-step layer: scheduler, corrector, time-step criterion on the device --------------
+ * (SURVEY.md 8(f) NEXT-1.)  The paper names the pieces -- "4th order Hermite predictor-corrector"
+ * (PAPER.md:129), "individual time stepping", "block time steps", "only
+ * the particles are updated that require a force update at a certain time" -- and
+ * calls the host link "the crucial bottleneck"; it prints no formula.  Readings
+ * (DESIGN.md): R12 corrector, R18 interpolated derivatives, R19 Aarseth criterion, R20 power-of-two
+ * block rule, R21 scheduler.  Each particle carries a step dt_j next to the 14 j-store fields.
+ * dt_min and dt_max must be powers of two, 0 < dt_min <= dt_max (NB_ERR_ARG otherwise). */
+
+/* Set the steps of particles [first, first+count) from a DEVICE fp64 array. */
+int nb_set_dt(nb_ctx* c, int64_t first, int64_t count, const double* dt);
+
+/* Copy the stored state of particles [first, first+count) to a DEVICE fp64 buffer laid out
+ * [15][count]: the 14 j-store fields in nb_set_j's order (m, x,y,z, vx,vy,vz, ax,ay,az, jx,jy,jz,
+ * t), then dt. */
+int nb_get_state(nb_ctx* c, int64_t first, int64_t count, double* out);
+
+/* Start of a run (R19, R20): for particle i_list[k] (DEVICE int32) store acc/jrk (DEVICE fp64,
+ * nb_force's layout [3][ni]) as its (a, jerk) and give it the largest power-of-two step
+ * <= eta_s |a| / |jerk|, clamped to [dt_min, dt_max]. */
+int nb_init_steps(nb_ctx* c, const int32_t* i_list, int64_t ni, const double* acc, const double* jrk,
+                  double eta_s, double dt_min, double dt_max);
+
+/* Scheduler (R21): *t_next = min_j (t_j + dt_j) over the n particles, *ni = how many are due then;
+ * their indices, ascending, are left in a context-owned DEVICE list whose address is returned in
+ * *i_list (may be NULL) and stays valid until the next nb_next_block / nb_step.  One cooperative
+ * kernel; synchronises the stream to bring the two scalars back (HOST outputs).  NB_ERR_ARG (with
+ * *t_next and *ni still set) if more than ni_max particles are due: the list is then truncated. */
+int nb_next_block(nb_ctx* c, double* t_next, int64_t* ni, const int32_t** i_list);
+
+/* Corrector + new step (R12, R18, R19, R20) for particles i_list[0..ni) (DEVICE) that were
+ * predicted to t1 and whose forces at t1 are acc/jrk (DEVICE fp64, [3][ni] in i_list order): with
+ * h = t1 - t_i, v1 = v0 + (a0+a1) h/2 + (j0-j1) h^2/12; x1 = x0 + (v0+v1) h/2 + (a0-a1) h^2/12;
+ * the step wanted is sqrt(eta (|a1||a2| + |j1|^2) / (|j1||a3| + |a2|^2)) with a2, a3 from the
+ * Hermite interpolation; the stored step is halved while above it, or doubled once when allowed.
+ * Writes x1, v1, a1, j1, t1 and the new dt into the j-store, in place.  Duplicate indices: undefined. */
+int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const double* acc,
+               const double* jrk, double eta, double dt_min, double dt_max);
+
+/* One whole block step on the device: nb_next_block -> nb_predict(t) -> nb_force(due particles,
+ * eps2) -> nb_correct.  HOST outputs *t (the block time) and *ni (particles advanced).  The forces
+ * of the block stay in a context-owned buffer (nb_block_forces). */
+int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, double* t, int64_t* ni);
+
+/* DEVICE addresses of the last nb_step's acc [3][ni], jrk [3][ni], pot [ni] (any may be NULL). */
+int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const double** pot);
 
 /* Measure what the FP32 FMA pipe of this device sustains, with the instruction kinds the pair
  * kernel is built from: kind 0 = scalar FFMA, kind 1 = packed FFMA2

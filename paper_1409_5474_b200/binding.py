@@ -18,7 +18,8 @@ EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_host", "nb_set_tuning",
-    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_probe_fp32", "nb_sync", "nb_strerror", "nb_version",
+    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_probe_fp32", "nb_sync",
+    "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_block_forces", "nb_strerror", "nb_version",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -57,6 +58,13 @@ lib.nb_sync.argtypes = [_vp]
 lib.nb_strerror.argtypes = [_i32]
 lib.nb_strerror.restype = ctypes.c_char_p
 lib.nb_probe_fp32.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(_dbl)]
+lib.nb_set_dt.argtypes = [_vp, _i64, _i64, _vp]
+lib.nb_get_state.argtypes = [_vp, _i64, _i64, _vp]
+lib.nb_init_steps.argtypes = [_vp, _vp, _i64, _vp, _vp, _dbl, _dbl, _dbl]
+lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(_dbl), ctypes.POINTER(_i64), ctypes.POINTER(_vp)]
+lib.nb_correct.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _dbl, _dbl, _dbl]
+lib.nb_step.argtypes = [_vp, _dbl, _dbl, _dbl, _dbl, ctypes.POINTER(_dbl), ctypes.POINTER(_i64)]
+lib.nb_block_forces.argtypes = [_vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp), ctypes.POINTER(_vp)]
 lib.nb_version.restype = ctypes.c_char_p
 
 
@@ -197,6 +205,45 @@ def nb_launch_count(c):
 
 def nb_set_profiling(c, on=True):
     _check(lib.nb_set_profiling(c, 1 if on else 0), "nb_set_profiling")
+
+
+def nb_set_dt(c, first, count, dt):
+    _check(lib.nb_set_dt(c, first, count, _ptr(dt)), "nb_set_dt")
+
+
+def nb_get_state(c, first, count, out):
+    """out: DEVICE fp64 (15, count)."""
+    _check(lib.nb_get_state(c, first, count, _ptr(out)), "nb_get_state")
+
+
+def nb_init_steps(c, i_list, ni, acc, jrk, eta_s, dt_min, dt_max):
+    _check(lib.nb_init_steps(c, _ptr(i_list), ni, _ptr(acc), _ptr(jrk), eta_s, dt_min, dt_max),
+           "nb_init_steps")
+
+
+def nb_next_block(c):
+    """Returns (t_next, ni, device address of the context-owned int32 list)."""
+    t, ni, lst = _dbl(0.0), _i64(0), _vp()
+    _check(lib.nb_next_block(c, ctypes.byref(t), ctypes.byref(ni), ctypes.byref(lst)), "nb_next_block")
+    return t.value, ni.value, lst.value
+
+
+def nb_correct(c, i_list, ni, t1, acc, jrk, eta, dt_min, dt_max):
+    _check(lib.nb_correct(c, _ptr(i_list), ni, t1, _ptr(acc), _ptr(jrk), eta, dt_min, dt_max), "nb_correct")
+
+
+def nb_step(c, eps2, eta, dt_min, dt_max):
+    """One block step on the device; returns (t, ni)."""
+    t, ni = _dbl(0.0), _i64(0)
+    _check(lib.nb_step(c, eps2, eta, dt_min, dt_max, ctypes.byref(t), ctypes.byref(ni)), "nb_step")
+    return t.value, ni.value
+
+
+def nb_block_forces(c):
+    """Device addresses (acc, jrk, pot) of the last nb_step's forces."""
+    a, j, p = _vp(), _vp(), _vp()
+    _check(lib.nb_block_forces(c, ctypes.byref(a), ctypes.byref(j), ctypes.byref(p)), "nb_block_forces")
+    return a.value, j.value, p.value
 
 
 def nb_probe_fp32(c, kind):

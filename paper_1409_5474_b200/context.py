@@ -4,6 +4,14 @@ import torch
 from . import binding as nb
 
 
+class _DeviceView:
+    """A context-owned device array seen through __cuda_array_interface__ (no copy)."""
+
+    def __init__(self, ptr, n, typestr):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": typestr,
+                                         "data": (int(ptr), False), "version": 2}
+
+
 class Context:
     def __init__(self, n_max, ni_max=None, device=0, stream=None):
         self.device = torch.device("cuda", device)
@@ -100,6 +108,39 @@ class Context:
         """HOST int32 i_list and HOST fp64 outputs acc, jrk (3, ni), pot (ni,); returns after
         the results are back on the host."""
         nb.nb_force_host(self.h, i_list, i_list.shape[0], eps2, acc, jrk, pot)
+
+    # -- block-step layer (marshalling only) --------------------------------------------------
+    def init_steps(self, i_list, acc, jrk, eta_s, dt_min, dt_max):
+        il = self._dev(i_list, torch.int32)
+        nb.nb_init_steps(self.h, il, il.shape[0], acc, jrk, eta_s, dt_min, dt_max)
+        self._keep = [il, acc, jrk]
+
+    def set_dt(self, dt, first=0):
+        d = self._dev(dt)
+        nb.nb_set_dt(self.h, first, d.shape[0], d)
+        self._keep = [d]
+
+    def state(self, first=0, count=None):
+        """(15, count) fp64 device tensor: the 14 stored fields, then dt."""
+        count = nb.lib.nb_count(self.h) - first if count is None else count
+        out = torch.empty((15, count), dtype=torch.float64, device=self.device)
+        nb.nb_get_state(self.h, first, count, out)
+        return out
+
+    def next_block(self):
+        """(t_next, ni, int32 device tensor viewing the context-owned list of due particles)."""
+        t, ni, addr = nb.nb_next_block(self.h)
+        if ni == 0:
+            return t, ni, torch.empty(0, dtype=torch.int32, device=self.device)
+        return t, ni, torch.as_tensor(_DeviceView(addr, ni, "<i4"), device=self.device)
+
+    def correct(self, i_list, t1, acc, jrk, eta, dt_min, dt_max):
+        il = self._dev(i_list, torch.int32)
+        nb.nb_correct(self.h, il, il.shape[0], t1, acc, jrk, eta, dt_min, dt_max)
+        self._keep = [il, acc, jrk]
+
+    def step(self, eps2, eta, dt_min, dt_max):
+        return nb.nb_step(self.h, eps2, eta, dt_min, dt_max)
 
     # -- measurement --------------------------------------------------------------------------
     def profiling(self, on=True):

@@ -30,8 +30,17 @@ struct nb_ctx {
     double* h_out = nullptr;      // [7][ni_max]
     double* h_in = nullptr;       // [14][ni_pad] staging of nb_update_j_host
     int64_t ni_pad = 0;
+    // block-step state (hermite.cu): per-particle step, the scheduler's list and meta words, and
+    // the forces of the current block
+    double* dts = nullptr;              // [n_cap]
+    int32_t* blk_list = nullptr;        // [ni_pad]
+    double* blk_out = nullptr;          // [7][ni_pad]
+    unsigned long long* sel_meta = nullptr;   // [0] key of t1, [1] count
+    int* sel_counts = nullptr;          // [SEL_MAX_BLOCKS]
+    double blk_t = 0.0;                 // what the last nb_next_block returned
+    int64_t blk_ni = -1;
 
-    int* err_pinned = nullptr;
+    int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
 
     bool predicted = false;
@@ -59,7 +68,8 @@ constexpr size_t ALIGN = 256;
 inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t store, pack, flags, tileflag, flag_list, part, err, ilist, out, in, total;
+    size_t store, pack, flags, tileflag, flag_list, part, err, ilist, out, in, dts, blk_list, blk_out,
+        sel_meta, sel_counts, total;
     int64_t ni_pad;
     size_t part_bytes;
     int64_t n_cap;
@@ -86,6 +96,11 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.ilist = off; off += up((size_t)ni_pad * 4);
     L.out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
     L.in = off; off += up((size_t)NFIELD * ni_pad * sizeof(double));
+    L.dts = off; off += up((size_t)L.n_cap * sizeof(double));
+    L.blk_list = off; off += up((size_t)ni_pad * 4);
+    L.blk_out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
+    L.sel_meta = off; off += up(16);
+    L.sel_counts = off; off += up((size_t)SEL_MAX_BLOCKS * 4);
     L.ni_pad = ni_pad;
     L.total = off;
     return L;
@@ -120,6 +135,11 @@ int ensure_alloc(nb_ctx* c)
     c->h_ilist = reinterpret_cast<int32_t*>(c->slab + L.ilist);
     c->h_out = reinterpret_cast<double*>(c->slab + L.out);
     c->h_in = reinterpret_cast<double*>(c->slab + L.in);
+    c->dts = reinterpret_cast<double*>(c->slab + L.dts);
+    c->blk_list = reinterpret_cast<int32_t*>(c->slab + L.blk_list);
+    c->blk_out = reinterpret_cast<double*>(c->slab + L.blk_out);
+    c->sel_meta = reinterpret_cast<unsigned long long*>(c->slab + L.sel_meta);
+    c->sel_counts = reinterpret_cast<int*>(c->slab + L.sel_counts);
     c->ni_pad = L.ni_pad;
     c->allocated = true;
     return NB_OK;
@@ -365,7 +385,7 @@ int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* str
         delete c;
         return NB_ERR_CUDA;
     }
-    if (cudaMallocHost(&c->err_pinned, sizeof(int)) != cudaSuccess) {
+    if (cudaMallocHost(&c->err_pinned, 32) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return NB_ERR_ALLOC;
@@ -505,7 +525,10 @@ int nb_clear(nb_ctx* c)
     if (c->allocated) {
         const Layout L = layout(c->n_max, c->ni_max);
         if (cudaMemsetAsync(c->slab, 0, L.part, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+        if (cudaMemsetAsync(c->dts, 0, (size_t)c->n_cap * sizeof(double), c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
     }
+    c->blk_ni = -1;
     c->n = 0;
     c->flagged.clear();
     c->predicted = false;
@@ -674,6 +697,127 @@ int nb_kernel_times(nb_ctx* c, double* out)
         out[k] = c->prof_ms[k];
         out[3 + k] = (double)c->prof_n[k];
     }
+    return NB_OK;
+}
+
+// ---- block-step layer (hermite.cu; R12, R18..R21) ---------------------------------
+
+static bool steps_ok(double dt_min, double dt_max)
+{
+    // both must be powers of two (block grid), 0 < dt_min <= dt_max
+    if (!(dt_min > 0.0) || !(dt_max >= dt_min) || !isfinite(dt_max)) return false;
+    int e;
+    return frexp(dt_min, &e) == 0.5 && frexp(dt_max, &e) == 0.5;
+}
+
+int nb_set_dt(nb_ctx* c, int64_t first, int64_t count, const double* dt)
+{
+    if (!c || first < 0 || count < 0 || first + count > c->n || (count > 0 && !dt)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (count > 0 && cudaMemcpyAsync(c->dts + first, dt, (size_t)count * sizeof(double),
+                                     cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    return NB_OK;
+}
+
+int nb_get_state(nb_ctx* c, int64_t first, int64_t count, double* out)
+{
+    if (!c || first < 0 || count < 0 || first + count > c->n || (count > 0 && !out)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (launch_get_state(c->store, c->dts, first, count, out, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    if (count > 0) c->launches += 1;
+    return NB_OK;
+}
+
+int nb_init_steps(nb_ctx* c, const int32_t* i_list, int64_t ni, const double* acc, const double* jrk,
+                  double eta_s, double dt_min, double dt_max)
+{
+    if (!c || ni < 0 || !(eta_s > 0.0) || !steps_ok(dt_min, dt_max)) return NB_ERR_ARG;
+    if (ni > 0 && (!i_list || !acc || !jrk)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (launch_init_steps(c->store, c->dts, i_list, ni, c->n, acc, jrk, eta_s, dt_min, dt_max, c->err,
+                          c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    if (ni > 0) c->launches += 1;
+    return NB_OK;
+}
+
+int nb_next_block(nb_ctx* c, double* t_next, int64_t* ni, const int32_t** i_list)
+{
+    if (!c || !t_next || !ni) return NB_ERR_ARG;
+    if (c->n < 1) return NB_ERR_STATE;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (launch_select(c->store.f[F_T], c->dts, c->n, c->sel_meta, c->sel_counts, c->blk_list, c->ni_pad,
+                      c->sm_count, c->stream) != cudaSuccess) {
+        cudaGetLastError();
+        return NB_ERR_CUDA;
+    }
+    c->launches += 1;
+    unsigned long long* host = reinterpret_cast<unsigned long long*>(c->err_pinned) + 1;
+    if (cudaMemcpyAsync(host, c->sel_meta, 16, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    // decode the order-preserving key (hermite.cu key_of)
+    const long long b = (long long)host[0];
+    const long long bits = b ^ ((~b >> 63) | (long long)0x8000000000000000ull);
+    double t;
+    memcpy(&t, &bits, 8);
+    c->blk_t = t;
+    c->blk_ni = (int64_t)host[1];
+    *t_next = t;
+    *ni = c->blk_ni;
+    if (i_list) *i_list = c->blk_list;
+    if (c->blk_ni > c->ni_max) return NB_ERR_ARG;     // the list was truncated to ni_max entries
+    return NB_OK;
+}
+
+int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const double* acc,
+               const double* jrk, double eta, double dt_min, double dt_max)
+{
+    if (!c || ni < 0 || !isfinite(t1) || !(eta > 0.0) || !steps_ok(dt_min, dt_max)) return NB_ERR_ARG;
+    if (ni > 0 && (!i_list || !acc || !jrk)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (launch_correct(c->store, c->dts, i_list, ni, c->n, t1, acc, jrk, eta, dt_min, dt_max, c->err,
+                       c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+    if (ni > 0) c->launches += 1;
+    return NB_OK;
+}
+
+int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, double* t, int64_t* ni)
+{
+    if (!c || !t || !ni || !isfinite(eps2) || eps2 < 0.0 || !(eta > 0.0) || !steps_ok(dt_min, dt_max))
+        return NB_ERR_ARG;
+    int rc = nb_next_block(c, t, ni, nullptr);
+    if (rc != NB_OK) return rc;
+    rc = nb_predict(c, *t);
+    if (rc != NB_OK) return rc;
+    DeviceGuard g(c->device);
+    const int64_t k = *ni;
+    double* acc = c->blk_out;
+    double* jrk = c->blk_out + 3 * k;
+    double* pot = c->blk_out + 6 * k;
+    rc = force_impl(c, c->blk_list, k, eps2, acc, jrk, pot);
+    if (rc != NB_OK) return rc;
+    return nb_correct(c, c->blk_list, k, *t, acc, jrk, eta, dt_min, dt_max);
+}
+
+int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const double** pot)
+{
+    if (!c || c->blk_ni < 0 || !c->allocated) return c ? NB_ERR_STATE : NB_ERR_ARG;
+    if (acc) *acc = c->blk_out;
+    if (jrk) *jrk = c->blk_out + 3 * c->blk_ni;
+    if (pot) *pot = c->blk_out + 6 * c->blk_ni;
     return NB_OK;
 }
 

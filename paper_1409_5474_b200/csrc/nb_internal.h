@@ -95,6 +95,17 @@ cudaError_t force_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_force(const ForceArgs& a, int jl, int atomic_mode, double* acc, double* jrk,
                          double* pot, cudaStream_t s);
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);
+constexpr int SEL_MAX_BLOCKS = 1024;          // most CTAs the cooperative scheduler kernel uses
+cudaError_t launch_select(const double* t, const double* dt, int64_t n, unsigned long long* meta,
+                          int* counts, int32_t* list, int64_t cap, int sm_count, cudaStream_t s);
+cudaError_t launch_correct(const StorePtrs& st, double* dts, const int32_t* list, int64_t ni, int64_t n,
+                           double t1, const double* acc, const double* jrk, double eta, double dt_min,
+                           double dt_max, int* err, cudaStream_t s);
+cudaError_t launch_init_steps(const StorePtrs& st, double* dts, const int32_t* list, int64_t ni, int64_t n,
+                              const double* acc, const double* jrk, double eta_s, double dt_min,
+                              double dt_max, int* err, cudaStream_t s);
+cudaError_t launch_get_state(const StorePtrs& st, const double* dts, int64_t first, int64_t count,
+                             double* out, cudaStream_t s);
 cudaError_t probe_fp32(int kind, int sm_count, float* scratch, cudaStream_t s, double* lane_ops_per_s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 
