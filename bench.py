@@ -49,6 +49,10 @@ def parse():
     ap.add_argument("--sweep", action="store_true",
                     help="also time nb_force alone on every active-subset size of the workload "
                          "(config 3: 1, 1024, 16384, 262144, 2^20) and add it as \"sweep\"")
+    ap.add_argument("--blockstep", type=int, default=0, metavar="N",
+                    help="instead of the default line: time --steps device block steps (nb_step: "
+                         "scheduler + predictor + force + corrector) of a Plummer sphere of N "
+                         "particles with individual power-of-two steps")
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target duration of the cpu_baseline sample")
     return ap.parse_args()
@@ -435,10 +439,61 @@ def run_ours(args):
     return 0
 
 
+def run_blockstep(args):
+    """Block-time-step regime: every step advances only the particles that are
+    due, so N_i << N and the O(N) pieces (scheduler, predictor) and launch latency matter."""
+    import numpy as np
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    import nbgen
+    import paper_1409_5474_b200 as nbm
+    n = args.blockstep
+    eps2, eta, lo, hi = (4.0 / n) ** 2, 0.02, 2.0 ** -24, 2.0 ** -4
+    m, x, v = nbgen.plummer(n, nbgen.SEED0 + 6)
+    il = np.arange(n, dtype=np.int32)
+    with nbm.Context(n) as ctx:
+        ctx.set_j(m, x, v)
+        ctx.predict(0.0)
+        ga, gj, gp = ctx.force(il, eps2)
+        ctx.init_steps(il, ga, gj, eta, lo, hi)
+        for _ in range(max(args.warmup, 3)):
+            ctx.step(eps2, eta, lo, hi)
+        ctx.sync()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = ctx.launch_count()
+        sizes = []
+        w0 = time.perf_counter()
+        e0.record()
+        for _ in range(args.steps):
+            t, ni = ctx.step(eps2, eta, lo, hi)
+            sizes.append(ni)
+        e1.record()
+        ctx.sync()
+        wall = time.perf_counter() - w0
+        ms = e0.elapsed_time(e1)
+        launches = ctx.launch_count() - l0
+    sizes = np.array(sizes, dtype=np.float64)
+    line = {"metric": "interactions/s", "value": float(sizes.sum() * n / (ms * 1e-3)),
+            "unit": "interactions/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / args.steps, "wall_ms_per_step": wall / args.steps * 1e3,
+            "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "blockstep_plummer_N%d" % n, "eta": eta, "eps2": eps2,
+                       "step": "nb_step = nb_next_block + nb_predict + nb_force + nb_correct"},
+            "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),
+                      "min_n_i": int(sizes.min()), "max_n_i": int(sizes.max()),
+                      "particle_steps_per_s": float(sizes.sum() / (ms * 1e-3)), "t_end": t},
+            "gpu_launches": int(launches)}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.blockstep > 0:
+        return run_blockstep(args)
     return run_ours(args)
 
 
