@@ -137,6 +137,19 @@ int nb_get_predicted(nb_ctx* c, int64_t first, int64_t count, double* out);
 int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
              double* acc, double* jrk, double* pot);
 
+/* Forces on i-particles that are NOT members of the j-set, given by value -- "the particles in
+ * subset j can either belong to the same or a completely different set as the i-particles"
+ * (PAPER.md:49); this is the kick one system receives from another in the Hamiltonian-split
+ * coupling of PAPER.md:118-123.  x, v: DEVICE fp64 [3][ni] (x-row, y-row,
+ * z-row).  Same sums as nb_force over all n j-particles at their predicted state, but no pair is
+ * skipped by index and no pair is unsoftened (flags concern j-set members only); a j-particle at
+ * exactly the position of an i-particle with eps2 == 0 contributes nothing (R6).
+ * v == NULL and jrk == NULL together select the acc + pot only variant (19 instead of 33 FP32
+ * lane-operations per interaction); one NULL without the other is NB_ERR_ARG.
+ * Outputs as nb_force.  ni in [0, ni_max]; NB_ERR_STATE before the first nb_predict. */
+int nb_force_ext(nb_ctx* c, int64_t ni, const double* x, const double* v, double eps2, double* acc,
+                 double* jrk, double* pot);
+
 /* HOST-pointer form: i_list, acc, jrk, pot are host arrays; copies in, runs, copies back and
  * synchronises the stream before returning (so it also returns latched errors). */
 int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,

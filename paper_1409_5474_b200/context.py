@@ -109,6 +109,18 @@ class Context:
         the results are back on the host."""
         nb.nb_force_host(self.h, i_list, i_list.shape[0], eps2, acc, jrk, pot)
 
+    def force_ext(self, x, v, eps2):
+        """Forces on particles given by value: x, v (3, ni) of any kind; v None -> (acc, None, pot)."""
+        dx = self._dev(x)
+        dv = self._dev(v)
+        ni = dx.shape[1]
+        acc = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        jrk = torch.empty((3, ni), dtype=torch.float64, device=self.device) if dv is not None else None
+        pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
+        nb.nb_force_ext(self.h, ni, dx, dv, eps2, acc, jrk, pot)
+        self._keep = [dx, dv]
+        return acc, jrk, pot
+
     # -- block-step layer (marshalling only) --------------------------------------------------
     def init_steps(self, i_list, acc, jrk, eta_s, dt_min, dt_max):
         il = self._dev(i_list, torch.int32)

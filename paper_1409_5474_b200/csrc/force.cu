@@ -101,6 +101,29 @@ __device__ __forceinline__ void pair2(const IPart& I, Acc32& A, float2 xh, float
     A.jz = __ffma2_rn(mr3, __ffma2_rn(al, dz, wz), A.jz);
 }
 
+// acc + pot only (the kick of a bridge between two systems):
+// 9 FADD2 + 6 FFMA2 + 3 FMUL2 + 1 FADD2 = 19 lane-ops per interaction, no velocities.
+__device__ __forceinline__ void pair2_acc(const IPart& I, Acc32& A, float2 xh, float2 yh, float2 zh,
+                                          float2 xl, float2 yl, float2 zl, float2 m, float2 eps2)
+{
+    const float2 dx = __fadd2_rn(__fadd2_rn(xh, I.nxh), __fadd2_rn(xl, I.nxl));
+    const float2 dy = __fadd2_rn(__fadd2_rn(yh, I.nyh), __fadd2_rn(yl, I.nyl));
+    const float2 dz = __fadd2_rn(__fadd2_rn(zh, I.nzh), __fadd2_rn(zl, I.nzl));
+    float2 r2 = __ffma2_rn(dx, dx, eps2);
+    r2 = __ffma2_rn(dy, dy, r2);
+    r2 = __ffma2_rn(dz, dz, r2);
+    float2 rinv;
+    rinv.x = rsqrt_fast(r2.x);
+    rinv.y = rsqrt_fast(r2.y);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 mr = __fmul2_rn(m, rinv);
+    const float2 mr3 = __fmul2_rn(mr, rinv2);
+    A.p = __fadd2_rn(A.p, mr);
+    A.ax = __ffma2_rn(mr3, dx, A.ax);
+    A.ay = __ffma2_rn(mr3, dy, A.ay);
+    A.az = __ffma2_rn(mr3, dz, A.az);
+}
+
 // Masked scalar pair for the rare tiles that hold the i-particle itself, a flagged partner of a
 // flagged i, or when eps2 == 0 (R5, R6, R7): a skipped pair gets rinv = 0, i.e. contributes nothing.
 __device__ __forceinline__ void pair1_masked(const IPart& I, Acc32& A, const float* T, int p,
@@ -132,15 +155,17 @@ __device__ __forceinline__ void pair1_masked(const IPart& I, Acc32& A, const flo
 
 // S = distance between the 7 sums of one i: 1 when they sit in registers, FORCE_THREADS when they
 // sit in shared memory (the all-i kernel keeps them there: 28 registers fewer, 4 CTAs per SM)
-template <int S>
+template <int S, bool JERK>
 __device__ __forceinline__ void flush(Acc32& A, double* d)
 {
     d[0 * S] += (double)(A.ax.x + A.ax.y);
     d[1 * S] += (double)(A.ay.x + A.ay.y);
     d[2 * S] += (double)(A.az.x + A.az.y);
-    d[3 * S] += (double)(A.jx.x + A.jx.y);
-    d[4 * S] += (double)(A.jy.x + A.jy.y);
-    d[5 * S] += (double)(A.jz.x + A.jz.y);
+    if (JERK) {
+        d[3 * S] += (double)(A.jx.x + A.jx.y);
+        d[4 * S] += (double)(A.jy.x + A.jy.y);
+        d[5 * S] += (double)(A.jz.x + A.jz.y);
+    }
     d[6 * S] -= (double)(A.p.x + A.p.y);
     A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.p = make_float2(0.f, 0.f);
 }
@@ -152,12 +177,16 @@ __device__ __forceinline__ void flush(Acc32& A, double* d)
 // ring depth: the few-i variants do little arithmetic per tile and live on bytes in flight
 __host__ __device__ constexpr int stages_for(int jl) { return jl == 1 ? STAGES : 2 * STAGES; }
 
-template <bool ATOMIC, int JL>
+// MODE 0: i-particles are members of the j-set, given by index (nb_force).  MODE 1: i-particles
+// given by value, "a completely different set", acc + jerk + pot; MODE 2: the same,
+// acc + pot only (nb_force_ext).  No self pair and no flags in modes 1 and 2.
+template <bool ATOMIC, int JL, int MODE>
 __global__ void __launch_bounds__(FORCE_THREADS, NB_MINB)
 force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
              double* __restrict__ opot)
 {
     constexpr int STG = stages_for(JL);
+    constexpr bool JERK = (MODE != 2);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG * TILE_BYTES);
@@ -195,6 +224,24 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 #pragma unroll
     for (int u = 0; u < IPT; ++u) {
         const int ku = it * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;   // position inside the segment
+        if (MODE != 0) {
+            // by value: fp64 position split in two floats here, velocity rounded
+            const bool on = P.k0 + ku < P.ni;
+            const int64_t e = on ? P.k0 + ku : 0;
+            float h[3], l[3], w[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double xc = P.ext_x[(int64_t)c * P.ni + e];
+                h[c] = __double2float_rn(xc);
+                l[c] = __double2float_rn(xc - (double)h[c]);
+                w[c] = (MODE == 1) ? __double2float_rn(P.ext_v[(int64_t)c * P.ni + e]) : 0.0f;
+            }
+            I[u].nxh = dup(-h[0]); I[u].nyh = dup(-h[1]); I[u].nzh = dup(-h[2]);
+            I[u].nxl = dup(-l[0]); I[u].nyl = dup(-l[1]); I[u].nzl = dup(-l[2]);
+            I[u].nvx = dup(-w[0]); I[u].nvy = dup(-w[1]); I[u].nvz = dup(-w[2]);
+            sidx[u * FORCE_THREADS] = on ? -2 : -1;      // -2: active, member of no tile
+            continue;
+        }
         int q = (P.k0 + ku < P.ni) ? P.i_list[P.k0 + ku] : 0;
         const bool bad = (q < 0) || (q >= P.n);
         if (bad) {
@@ -246,9 +293,21 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
             for (int p = p0; p < p0 + JPT; p += 4) {
                 float4 f[10];
 #pragma unroll
-                for (int c = 0; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+                for (int c = 0; c < 10; ++c)
+                    if (JERK || c < 6 || c == 9) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
 #pragma unroll
                 for (int u = 0; u < IPT; ++u) {
+                    if (!JERK) {
+                        pair2_acc(I[u], A[u], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
+                                  make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y),
+                                  make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                                  make_float2(f[9].x, f[9].y), eps2);
+                        pair2_acc(I[u], A[u], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w),
+                                  make_float2(f[2].z, f[2].w), make_float2(f[3].z, f[3].w),
+                                  make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                                  make_float2(f[9].z, f[9].w), eps2);
+                        continue;
+                    }
                     pair2(I[u], A[u], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
                           make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y),
                           make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
@@ -276,8 +335,8 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         if (FLUSH_EVERY == 1 || (t - t0) % FLUSH_EVERY == FLUSH_EVERY - 1 || t == t1 - 1) {
 #pragma unroll
             for (int u = 0; u < IPT; ++u) {
-                if (DSM) flush<FORCE_THREADS>(A[u], sd + u * NOUT * FORCE_THREADS);
-                else flush<1>(A[u], D[DSM ? 0 : u]);
+                if (DSM) flush<FORCE_THREADS, JERK>(A[u], sd + u * NOUT * FORCE_THREADS);
+                else flush<1, JERK>(A[u], D[DSM ? 0 : u]);
             }
         }
 
@@ -323,16 +382,16 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         for (int c = 0; c < NOUT; ++c) o[c] = DSM ? sd[(u * NOUT + c) * FORCE_THREADS] : D[DSM ? 0 : u][c];
         const int ku = it2 * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;
         const int q = sidx[u * FORCE_THREADS];
-        if (!eps0 && !((iflags >> u) & 1u) && q >= u0 && q < u1) {
+        if (MODE == 0 && !eps0 && !((iflags >> u) & 1u) && q >= u0 && q < u1) {
             const float mi = P.pack[(int64_t)(q / TJ) * TILE_FLOATS + P_M * TJ + (q % TJ)];
             o[6] += (double)(mi * rinv_e);
         }
         if (ATOMIC) {
-            if (q >= 0) {
+            if (q != -1) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     atomicAdd(oacc + (int64_t)c * P.ni + P.k0 + ku, o[c]);
-                    atomicAdd(ojrk + (int64_t)c * P.ni + P.k0 + ku, o[3 + c]);
+                    if (JERK) atomicAdd(ojrk + (int64_t)c * P.ni + P.k0 + ku, o[3 + c]);
                 }
                 atomicAdd(opot + P.k0 + ku, o[6]);
             }
@@ -382,11 +441,11 @@ __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
         }
     }
     if (WARP && lane != 0) return;
-    const int i = R.i_list[k];
+    const int i = R.i_list ? R.i_list[k] : 0;     // by-value calls (nb_force_ext) carry no index list
     if (i < 0 || i >= R.n) {
 #pragma unroll
         for (int c = 0; c < NOUT; ++c) o[c] = __longlong_as_double(0x7ff8000000000000LL);
-    } else if (R.nflag > 1 && (R.flags[i] & 1)) {
+    } else if (R.i_list && R.nflag > 1 && (R.flags[i] & 1)) {
         double xi[3], vi[3];
         const double dti = R.t_pred - R.store.f[F_T][i];
 #pragma unroll
@@ -424,7 +483,7 @@ __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         R.acc[(int64_t)c * R.ni + k] = o[c];
-        R.jrk[(int64_t)c * R.ni + k] = o[3 + c];
+        if (R.jrk) R.jrk[(int64_t)c * R.ni + k] = o[3 + c];
     }
     R.pot[k] = o[6];
 }
@@ -453,13 +512,13 @@ __host__ __device__ constexpr int force_smem(int jl)
 template <int JL>
 cudaError_t setup_one(int* blocks)
 {
-    cudaError_t e = cudaFuncSetAttribute(force_kernel<false, JL>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, force_smem(JL));
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(force_kernel<true, JL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             force_smem(JL));
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks, force_kernel<false, JL>,
+    const void* k[4] = {(const void*)force_kernel<false, JL, 0>, (const void*)force_kernel<true, JL, 0>,
+                        (const void*)force_kernel<false, JL, 1>, (const void*)force_kernel<false, JL, 2>};
+    for (int q = 0; q < 4; ++q) {
+        cudaError_t e = cudaFuncSetAttribute(k[q], cudaFuncAttributeMaxDynamicSharedMemorySize, force_smem(JL));
+        if (e != cudaSuccess) return e;
+    }
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks, force_kernel<false, JL, 0>,
                                                          FORCE_THREADS, force_smem(JL));
 }
 
@@ -473,23 +532,29 @@ cudaError_t force_kernel_setup(int* blocks_per_sm)
     return setup_one<1>(blocks_per_sm);
 }
 
+// mode: 0 = by index (nb_force), 1 = by value with jerk, 2 = by value, acc + pot only (nb_force_ext;
+// no atomics variant there)
 template <int JL>
-void launch_one(const ForceArgs& a, int atomic_mode, double* acc, double* jrk, double* pot,
+void launch_one(const ForceArgs& a, int mode, int atomic_mode, double* acc, double* jrk, double* pot,
                 cudaStream_t s)
 {
     const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
-    if (atomic_mode)
-        force_kernel<true, JL><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+    if (mode == 1)
+        force_kernel<false, JL, 1><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+    else if (mode == 2)
+        force_kernel<false, JL, 2><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+    else if (atomic_mode)
+        force_kernel<true, JL, 0><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
     else
-        force_kernel<false, JL><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+        force_kernel<false, JL, 0><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
 }
 
-cudaError_t launch_force(const ForceArgs& a, int jl, int atomic_mode, double* acc, double* jrk,
+cudaError_t launch_force(const ForceArgs& a, int jl, int mode, int atomic_mode, double* acc, double* jrk,
                          double* pot, cudaStream_t s)
 {
-    if (jl == JL_MAX) launch_one<JL_MAX>(a, atomic_mode, acc, jrk, pot, s);
-    else if (jl == JL_MID) launch_one<JL_MID>(a, atomic_mode, acc, jrk, pot, s);
-    else launch_one<1>(a, atomic_mode, acc, jrk, pot, s);
+    if (jl == JL_MAX) launch_one<JL_MAX>(a, mode, atomic_mode, acc, jrk, pot, s);
+    else if (jl == JL_MID) launch_one<JL_MID>(a, mode, atomic_mode, acc, jrk, pot, s);
+    else launch_one<1>(a, mode, atomic_mode, acc, jrk, pot, s);
     return cudaGetLastError();
 }
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s)

@@ -228,9 +228,11 @@ int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, siz
     return best;
 }
 
+// ext_x != NULL: i-particles by value (nb_force_ext); ext_v == NULL then means acc + pot only
 int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc, double* jrk,
-               double* pot)
+               double* pot, const double* ext_x = nullptr, const double* ext_v = nullptr)
 {
+    const int kmode = ext_x ? (ext_v ? 1 : 2) : 0;
     if (!c->predicted) return NB_ERR_STATE;
     c->last[0] = c->last[1] = c->last[2] = 0;
     if (ni == 0) return NB_OK;
@@ -238,6 +240,8 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     ForceArgs a{};
     a.pack = c->pack;
     a.i_list = i_list;
+    a.ext_x = ext_x;
+    a.ext_v = ext_v;
     a.flags = c->flags;
     a.tileflag = c->tileflag;
     a.err = c->err;
@@ -245,8 +249,8 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     a.n = (int)n_launch;
     a.ntiles = (int)((n_launch + TJ - 1) / TJ);
     a.eps2 = (float)eps2;
-    a.any_flagged = c->flagged.empty() ? 0 : 1;
-    const int mode = c->tune_reduce ? 1 : 0;
+    a.any_flagged = (c->flagged.empty() || kmode != 0) ? 0 : 1;
+    const int mode = (c->tune_reduce && kmode == 0) ? 1 : 0;
     // few active i: several threads share one i-particle and split the j of a tile
     const int jl = ni <= ITILE / JL_MAX ? JL_MAX : (ni <= ITILE / JL_MID ? JL_MID : 1);
     const int itile = ITILE / jl;
@@ -280,7 +284,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             a.ni_pad = (int)pad_a;
             a.splits = 1;
             a.part = c->part;
-            if (launch_force(a, jl, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            if (launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
             ++launched;
         }
         if (tiles_b > 0) {
@@ -289,7 +293,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             a.ni_pad = (int)pad_b;
             a.splits = splits_b;
             a.part = part_b;
-            if (launch_force(a, jl, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            if (launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
             ++launched;
         }
         if (rec) cudaEventRecord(rec->e[1], c->stream);
@@ -620,6 +624,16 @@ int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* 
     if (ni > 0 && (!i_list || !acc || !jrk || !pot)) return NB_ERR_ARG;
     DeviceGuard g(c->device);
     return force_impl(c, i_list, ni, eps2, acc, jrk, pot);
+}
+
+int nb_force_ext(nb_ctx* c, int64_t ni, const double* x, const double* v, double eps2, double* acc,
+                 double* jrk, double* pot)
+{
+    if (!c || ni < 0 || ni > c->ni_max || !isfinite(eps2) || eps2 < 0.0) return NB_ERR_ARG;
+    if (ni > 0 && (!x || !acc || !pot)) return NB_ERR_ARG;
+    if ((v == nullptr) != (jrk == nullptr)) return NB_ERR_ARG;     // jerk needs velocities, and only then
+    DeviceGuard g(c->device);
+    return force_impl(c, nullptr, ni, eps2, acc, jrk, pot, x, v);
 }
 
 int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc,

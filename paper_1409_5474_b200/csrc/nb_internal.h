@@ -54,7 +54,9 @@ struct SrcPtrs {
 
 struct ForceArgs {
     const float* pack;        // [ntiles][NPF][TJ]
-    const int32_t* i_list;    // [ni]
+    const int32_t* i_list;    // [ni] (by-index calls, nb_force)
+    const double* ext_x;      // [3][ni]: i-particles by value (nb_force_ext), else unused
+    const double* ext_v;      // [3][ni], or NULL for acc + pot only
     double* part;             // [S][NOUT][ni_pad] partial sums (reduce_mode 0)
     const uint8_t* flags;     // [n_cap] bit 0: unsoftened among flagged
     const uint32_t* tileflag; // bit t: tile t holds a flagged particle
@@ -92,7 +94,7 @@ cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* 
 cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
                                  double* out, cudaStream_t s);
 cudaError_t force_kernel_setup(int* blocks_per_sm);
-cudaError_t launch_force(const ForceArgs& a, int jl, int atomic_mode, double* acc, double* jrk,
+cudaError_t launch_force(const ForceArgs& a, int jl, int mode, int atomic_mode, double* acc, double* jrk,
                          double* pot, cudaStream_t s);
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);
 constexpr int SEL_MAX_BLOCKS = 1024;          // most CTAs the cooperative scheduler kernel uses

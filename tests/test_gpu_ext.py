@@ -1,0 +1,135 @@
+"""-m gpu: nb_force_ext (i-particles by value, "a completely different set"; with jerk,
+or acc + pot only) against the fp64 oracle.  The oracle needs no new code for this: the i-particles
+are appended to the j-set as MASSLESS particles and addressed by index -- massless particles exert
+nothing on each other and the self pair of an appended particle is skipped by index (R5), so
+oracle.force on the joined set is exactly the by-value sum."""
+import numpy as np
+import pytest
+
+import nbgen
+import oracle
+from util import check_parity, rel_err_scalar, rel_err_vec, TOL_ACC, TOL_POT
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def nbmod():
+    import __graft_entry__ as g
+    g.build()
+    import paper_1409_5474_b200 as nbm
+    return nbm
+
+
+def _j_set(n, seed):
+    m, x, v = nbgen.plummer(n, seed)
+    m = m * (0.5 + nbgen.Streams(seed + 1, n).uniform())
+    a, j = nbgen.mean_field(x, v)
+    t = 0.25 * nbgen.Streams(seed + 2, n).uniform()
+    return m, x, v, a, j, t
+
+
+def _i_set(ni, seed, shift):
+    """A second Plummer sphere, displaced so that the two systems overlap partly."""
+    _, x, v = nbgen.plummer(max(ni, 2), seed)
+    x, v = x[:, :ni].copy(), v[:, :ni].copy()
+    x[0] += shift
+    return x, v
+
+
+def _oracle_ext(m, xp, vp, xi, vi, eps2):
+    n, ni = m.shape[0], xi.shape[1]
+    mm = np.concatenate([m, np.zeros(ni)])
+    xx = np.concatenate([xp, xi], axis=1)
+    vv = np.concatenate([vp, vi], axis=1)
+    return oracle.force(mm, xx, vv, np.arange(n, n + ni, dtype=np.int32), eps2)
+
+
+@pytest.mark.parametrize("ni", [1, 7, 64, 300, 2049])
+@pytest.mark.parametrize("eps2", [2.0 ** -14, 0.0])
+def test_force_ext_with_jerk(nbmod, ni, eps2):
+    n, t = 6000, 0.3
+    m, x, v, a, j, tj = _j_set(n, 700)
+    xi, vi = _i_set(ni, 800 + ni, 0.7)
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    if ni >= 7:
+        # an i-particle exactly on top of a j-particle: -m/eps in pot when softened, nothing when not (R6)
+        xi[:, 3], vi[:, 3] = xp[:, 1234], vp[:, 1234]
+    ref = _oracle_ext(m, xp, vp, xi, vi, eps2)
+    with nbmod.Context(n, max(ni, 1)) as ctx:
+        ctx.set_j(m, x, v, a, j, tj)
+        ctx.predict(t)
+        for splits in (0, 1, 5):
+            ctx.tuning(splits, 0)
+            got = [q.cpu().numpy() for q in ctx.force_ext(xi, vi, eps2)]
+            check_parity(got, ref)
+        again = [q.cpu().numpy() for q in ctx.force_ext(xi, vi, eps2)]
+        assert all((p == q).all() for p, q in zip(again, got))          # deterministic (R9)
+        ctx.sync()
+
+
+@pytest.mark.parametrize("ni", [1, 9, 300, 2049])
+def test_force_ext_acc_pot_only(nbmod, ni):
+    n, t, eps2 = 6000, 0.3, 2.0 ** -14
+    m, x, v, a, j, tj = _j_set(n, 710)
+    xi, vi = _i_set(ni, 810 + ni, -0.4)
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    ra, _, rp = _oracle_ext(m, xp, vp, xi, np.zeros_like(xi), eps2)
+    with nbmod.Context(n, max(ni, 1)) as ctx:
+        ctx.set_j(m, x, v, a, j, tj)
+        ctx.predict(t)
+        acc, jrk, pot = ctx.force_ext(xi, None, eps2)
+        assert jrk is None
+        ga, gp = acc.cpu().numpy(), pot.cpu().numpy()
+        ctx.sync()
+    assert rel_err_vec(ga, ra).max() <= TOL_ACC and rel_err_scalar(gp, rp).max() <= TOL_POT
+
+
+def test_force_ext_argument_errors(nbmod):
+    nb = nbmod.binding
+    with nbmod.Context(64, 8) as ctx:
+        z = torch.zeros((3, 4), dtype=torch.float64, device=ctx.device)
+        p = torch.zeros(4, dtype=torch.float64, device=ctx.device)
+        with pytest.raises(nb.NBError) as e:                     # before any nb_predict
+            nb.nb_force_ext(ctx.h, 4, z, z, 1e-4, z, z, p)
+        assert e.value.status == nb.NB_ERR_STATE
+        m, x, v = nbgen.plummer(64, 5)
+        ctx.set_j(m, x, v)
+        ctx.predict(0.0)
+        for args in ((4, z, None, 1e-4, z, z, p),                # jerk asked for without velocities
+                     (4, z, z, 1e-4, z, None, p),                # velocities given, no jerk buffer
+                     (9, z, z, 1e-4, z, z, p),                   # ni > ni_max
+                     (4, z, z, -1.0, z, z, p)):                  # negative eps2
+            with pytest.raises(nb.NBError) as e:
+                nb.nb_force_ext(ctx.h, *args)
+            assert e.value.status == nb.NB_ERR_ARG
+        nb.nb_force_ext(ctx.h, 0, None, None, 1e-4, None, None, None)   # ni = 0: no-op
+        ctx.sync()
+
+
+def test_bridge_kick_two_galaxies(nbmod):
+    """The use NEXT-2 names: the kick galaxy B's stars receive from galaxy A (config 4's two
+    spheres at a quarter of the size), acc + pot only, checked on 1024 sampled stars of B; and the
+    momentum the two mutual kicks exchange cancels (sum m a over B = - sum m a over A)."""
+    c = nbgen.config4(n_gal=1 << 17)
+    na = (1 << 17) + 1
+    eps2 = c.eps2
+    A = (c.m[:na].copy(), np.ascontiguousarray(c.x[:, :na]), np.ascontiguousarray(c.v[:, :na]))
+    B = (c.m[na:].copy(), np.ascontiguousarray(c.x[:, na:]), np.ascontiguousarray(c.v[:, na:]))
+    with nbmod.Context(na) as ctx:
+        ctx.set_j(*A)
+        ctx.predict(0.0)
+        acc_b, _, pot_b = ctx.force_ext(B[1], None, eps2)
+        acc_b, pot_b = acc_b.cpu().numpy(), pot_b.cpu().numpy()
+        ctx.set_j(*B)
+        ctx.predict(0.0)
+        acc_a = ctx.force_ext(A[1], None, eps2)[0].cpu().numpy()
+        ctx.sync()
+    pos = nbgen.sample_positions(nbgen.SEED0 * 100 + 42, B[0].shape[0], 1024)
+    ra, _, rp = _oracle_ext(A[0], A[1], A[2], B[1][:, pos], np.zeros((3, len(pos))), eps2)
+    assert rel_err_vec(acc_b[:, pos], ra).max() <= TOL_ACC
+    assert rel_err_scalar(pot_b[pos], rp).max() <= TOL_POT
+    pa, pb = (A[0] * acc_a).sum(1), (B[0] * acc_b).sum(1)
+    assert np.abs(pa + pb).max() <= 1e-7 * np.abs(pa).max()
