@@ -53,6 +53,9 @@ def parse():
                     help="instead of the default line: time --steps device block steps (nb_step: "
                          "scheduler + predictor + force + corrector) of a Plummer sphere of N "
                          "particles with individual power-of-two steps")
+    ap.add_argument("--kick", action="store_true",
+                    help="instead of the default line: time nb_force_ext on config 4's two galaxies "
+                         "(stars of B by value against galaxy A as j-set), with jerk and acc + pot only")
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target duration of the cpu_baseline sample")
     return ap.parse_args()
@@ -488,10 +491,64 @@ def run_blockstep(args):
     return 0
 
 
+def run_kick(args):
+    """NEXT-2: the kick one system receives from another ("completely different set",
+    PAPER.md:118-123), i-particles by value."""
+    import numpy as np
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    import nbgen
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import binding as nb
+    c = nbgen.config4()
+    na = (c.n // 2)
+    dev = torch.device("cuda", 0)
+    with nbm.Context(na, c.n - na) as ctx:
+        ctx.set_j(c.m[:na].copy(), np.ascontiguousarray(c.x[:, :na]), np.ascontiguousarray(c.v[:, :na]))
+        ctx.predict(0.0)
+        xb = torch.from_numpy(np.ascontiguousarray(c.x[:, na:])).to(dev)
+        vb = torch.from_numpy(np.ascontiguousarray(c.v[:, na:])).to(dev)
+        ni = xb.shape[1]
+        acc = torch.empty((3, ni), dtype=torch.float64, device=dev)
+        jrk = torch.empty((3, ni), dtype=torch.float64, device=dev)
+        pot = torch.empty((ni,), dtype=torch.float64, device=dev)
+        props = torch.cuda.get_device_properties(dev)
+        peak = props.multi_processor_count * FP32_LANES_PER_SM * 1965e6     # lane-ops/s
+        out = {}
+        for name, v, j, lane_ops in (("acc_jerk_pot", vb, jrk, 33.0), ("acc_pot", None, None, 19.0)):
+            def call():
+                nb.nb_force_ext(ctx.h, ni, xb, v, c.eps2, acc, j, pot)
+            for _ in range(max(args.warmup, 3)):
+                call()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ctx.sync()
+            e0.record()
+            for _ in range(args.steps):
+                call()
+            e1.record()
+            ctx.sync()
+            ms = e0.elapsed_time(e1) / args.steps
+            rate = float(ni) * na / (ms * 1e-3)
+            out[name] = {"ms_per_call": ms, "interactions_per_s": rate,
+                         "fp32_lane_ops_per_interaction": lane_ops,
+                         "frac_of_fma_pipe": rate * lane_ops / peak}
+    line = {"metric": "interactions/s", "value": out["acc_pot"]["interactions_per_s"],
+            "unit": "interactions/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": out["acc_pot"]["ms_per_call"], "higher_is_better": True, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": "cfg4_kick_B_from_A", "n_j": int(na), "n_i": int(ni), "eps2": c.eps2},
+            "variants": out}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.kick:
+        return run_kick(args)
     if args.blockstep > 0:
         return run_blockstep(args)
     return run_ours(args)
