@@ -1,4 +1,6 @@
-"""Multi-GPU decomposition of one force call: i-sharding with a replicated j-set.
+"""Multi-GPU decompositions of one force call.
+
+(1) i-sharding with a replicated j-set (bench.py's N > 1 path):
 
 The i-particles of a call are independent ("embarrassingly parallel"), so rank r of P
 takes a contiguous slice of the active list and evaluates it against all N j-particles held in
@@ -47,3 +49,63 @@ def gather_forces(acc, jrk, pot, ni, group=None):
         a, b = shard_bounds(ni, r, world)
         out[:, a:b] = blocks[r][:, :b - a]
     return out[0:3], out[3:6], out[6]
+
+
+# ---- (2) j-sharding: the paper's own multi-GPU scheme ---------------------------
+#
+# "Multi-GPU parallelization is achieved by distributing the j particles over the various GPUs ...
+# This reduces the memory usage, transfer time and the time required to execute the optional
+# prediction step on the j particles.  In this scheme the first kernel computes the partial forces
+# ... and the second kernel sums these."  Rank r stores and predicts only particles
+# [lo_r, hi_r) (contiguous blocks: the sum is order-free, so this equals the paper's round-robin).
+# One force call on a global active list:
+#   1. every rank takes the predicted state and mass of the active particles it OWNS;
+#   2. one all_gather gives every rank the state of all active particles (7 fp64 each);
+#   3. every rank evaluates them BY VALUE against its own j-slice (nb_force_ext): partial forces;
+#   4. one all_reduce(sum) of [7][ni] fp64 -- the paper's "second kernel", across GPUs;
+#   5. the self pair was included by the owner's slice (by-value calls skip nothing): with
+#      eps2 > 0 it added nothing to acc and jerk and -m_i/eps to pot, which is taken back here;
+#      with eps2 = 0 a coincident pair contributes nothing (R6), so nothing is to be undone.
+# Unsoftened flagged pairs (R7) are not available on this path.
+
+
+def owned(i_list, lo, hi):
+    """Positions k (ascending) of the global active list whose particle lies in [lo, hi)."""
+    il = torch.as_tensor(i_list)
+    return torch.nonzero((il >= lo) & (il < hi)).flatten()
+
+
+def gather_active_state(state_local, pos_local, ni, group=None):
+    """state_local: (7, n_owned) fp64 = predicted x, y, z, vx, vy, vz and mass of the owned active
+    particles, pos_local: their positions in the global active list.  Returns (7, ni) on every
+    rank, in active-list order.  One all_gather of padded blocks + one of the positions."""
+    world = dist.get_world_size(group)
+    dev = state_local.device
+    counts = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(world)]
+    dist.all_gather(counts, torch.tensor([state_local.shape[1]], dtype=torch.int64, device=dev), group=group)
+    width = max(int(c.item()) for c in counts)
+    block = torch.zeros((8, max(width, 1)), dtype=torch.float64, device=dev)
+    k = state_local.shape[1]
+    block[:7, :k] = state_local
+    block[7, :k] = pos_local.to(torch.float64)           # positions < 2^53: exact in fp64
+    blocks = [torch.empty_like(block) for _ in range(world)]
+    dist.all_gather(blocks, block, group=group)
+    out = torch.empty((7, ni), dtype=torch.float64, device=dev)
+    for r in range(world):
+        kr = int(counts[r].item())
+        if kr:
+            out[:, blocks[r][7, :kr].to(torch.int64)] = blocks[r][:7, :kr]
+    return out
+
+
+def force_j_sharded(force_by_value, state_local, pos_local, ni, eps2, group=None):
+    """Steps 2-5 above.  force_by_value(x (3, ni), v (3, ni)) -> (acc (3, ni), jrk (3, ni),
+    pot (ni,)) against the CALLING rank's j-slice (Context.force_ext on a GPU).  Returns the
+    complete acc, jrk, pot of the active list on every rank."""
+    st = gather_active_state(state_local, pos_local, ni, group)
+    acc, jrk, pot = force_by_value(st[0:3].contiguous(), st[3:6].contiguous())
+    part = torch.cat([acc, jrk, pot.reshape(1, -1)], dim=0).contiguous()
+    dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
+    if eps2 > 0.0:
+        part[6] += st[6] / (eps2 ** 0.5)
+    return part[0:3], part[3:6], part[6]

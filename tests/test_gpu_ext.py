@@ -133,3 +133,34 @@ def test_bridge_kick_two_galaxies(nbmod):
     assert rel_err_scalar(pot_b[pos], rp).max() <= TOL_POT
     pa, pb = (A[0] * acc_a).sum(1), (B[0] * acc_b).sum(1)
     assert np.abs(pa + pb).max() <= 1e-7 * np.abs(pa).max()
+
+
+def test_j_sharded_path_on_one_gpu(nbmod):
+    """sharding.force_j_sharded with the real kernel behind it (world size 1 over NCCL): the
+    by-value partial forces + self-term correction reproduce the by-index force call."""
+    import socket
+    import torch.distributed as dist
+    from paper_1409_5474_b200 import sharding
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1)
+    try:
+        n, ni, t, eps2 = 5000, 700, 0.3, 2.0 ** -14
+        m, x, v, a, j, tj = _j_set(n, 720)
+        il = nbgen.permutation(721, n)[:ni].astype(np.int32)
+        xp, vp = oracle.predict(t, x, v, a, j, tj)
+        ref = oracle.force(m, xp, vp, il, eps2)
+        with nbmod.Context(n, ni) as ctx:
+            ctx.set_j(m, x, v, a, j, tj)
+            ctx.predict(t)
+            px, pv = ctx.predicted()
+            pos = sharding.owned(il, 0, n).to(ctx.device)
+            idx = torch.from_numpy(il.astype(np.int64)).to(ctx.device)
+            state = torch.cat([px[:, idx], pv[:, idx], torch.from_numpy(m).to(ctx.device)[None, idx]], 0)
+            got = sharding.force_j_sharded(lambda xi, vi: ctx.force_ext(xi, vi, eps2), state, pos, ni, eps2)
+            got = [q.cpu().numpy() for q in got]
+            ctx.sync()
+        check_parity(got, ref)
+    finally:
+        dist.destroy_process_group()

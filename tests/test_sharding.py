@@ -75,3 +75,61 @@ def test_gather_forces_world2_gloo(ni):
     assert sorted(r[0] for r in res) == [0, 1]
     assert all(r[1] for r in res)
     assert all(r[2] == (3, ni) for r in res)
+
+
+def _worker_j(rank, world, port, ni, eps2, out_q):
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch.distributed as dist
+    import nbgen
+    import oracle
+    from paper_1409_5474_b200 import sharding
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        c = nbgen.config1(777)
+        c.m = c.m * (0.5 + nbgen.Streams(9, c.n).uniform())
+        il = nbgen.permutation(6, c.n)[:ni]
+        lo, hi = sharding.shard_bounds(c.n, rank, world)             # this rank's j-slice
+        pos = sharding.owned(il, lo, hi)
+        mine = il[pos.numpy()]
+        state = torch.from_numpy(np.concatenate([c.x[:, mine], c.v[:, mine], c.m[None, mine]], 0))
+
+        def by_value(x, v):
+            # the rank's "nb_force_ext": the oracle on its j-slice, i-particles appended massless
+            xi, vi = x.numpy(), v.numpy()
+            k = xi.shape[1]
+            mm = np.concatenate([c.m[lo:hi], np.zeros(k)])
+            xx = np.concatenate([c.x[:, lo:hi], xi], 1)
+            vv = np.concatenate([c.v[:, lo:hi], vi], 1)
+            a, j, p = oracle.force(mm, xx, vv, np.arange(hi - lo, hi - lo + k, dtype=np.int32), eps2)
+            return torch.from_numpy(a), torch.from_numpy(j), torch.from_numpy(p)
+
+        acc, jrk, pot = sharding.force_j_sharded(by_value, state, pos, len(il), eps2)
+        ra, rj, rp = oracle.force(c.m, c.x, c.v, il, eps2)
+        ea = np.abs(acc.numpy() - ra).max() / np.abs(ra).max()
+        ej = np.abs(jrk.numpy() - rj).max() / np.abs(rj).max()
+        ep = np.abs(pot.numpy() - rp).max() / np.abs(rp).max()
+        out_q.put((rank, float(max(ea, ej, ep))))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("ni,eps2", [(301, 1e-4), (5, 1e-4), (64, 0.0)])
+def test_force_j_sharded_world2_gloo(ni, eps2):
+    """j distributed over the ranks, partial forces summed.  Equal to the unsharded
+    sum up to the order of the fp64 additions (and the self term taken back when eps2 > 0)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker_j, args=(r, 2, port, ni, eps2, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=120) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [0, 1]
+    assert all(r[1] < 1e-12 for r in res), res
