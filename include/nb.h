@@ -157,6 +157,19 @@ int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
 
 /* ---- control ------------------------------------------------------------------------------ */
 
+/* Arithmetic of the pair loop.  0 (default): position differences carry >= 48 bits, pair terms
+ * are fp32, sums fp64 ("emulating double precision" for the inter-particle distance).
+ * 1: IEEE double precision throughout -- differences, products, sums, and a reciprocal square
+ * root refined to fp64 rounding -- for "objects with an extreme mass ratio, like planetesimals
+ * around super-massive black holes".  Mode 1 keeps a second,
+ * fp64 copy of the predicted j-set (64 B per particle, cudaMalloc'ed by this call, not part of
+ * the lent workspace) and agrees with exact summation to ~1e-13 relative; pairs closer than
+ * ~1e-19 or farther than ~1e19 length units are treated as coincident / out of range.  Changing
+ * the mode invalidates the predicted state: call nb_predict before the next force call
+ * (NB_ERR_STATE otherwise).  The atomics reduce mode and the threads-per-i variants are mode-0
+ * only; results of mode 1 are deterministic. */
+int nb_set_precision(nb_ctx* c, int mode);
+
 /* Force-call tuning, for tests and experiments.  j_splits: 0 = let the dispatcher choose the
  * number of j-subsets, >0 = use exactly this many (clamped to what the partial
  * buffer holds).  reduce_mode: 0 = partial buffer + reduction kernel (deterministic;

@@ -17,7 +17,7 @@ NB_MAX_FLAGGED = 1024
 EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
-    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_host", "nb_set_tuning",
+    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_host", "nb_set_precision", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_probe_fp32", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_block_forces", "nb_strerror", "nb_version",
 ]
@@ -49,6 +49,7 @@ lib.nb_get_predicted.argtypes = [_vp, _i64, _i64, _vp]
 for _f in (lib.nb_force, lib.nb_force_host):
     _f.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _vp]
 lib.nb_set_tuning.argtypes = [_vp, _i32, _i32]
+lib.nb_set_precision.argtypes = [_vp, _i32]
 lib.nb_last_launch.argtypes = [_vp, ctypes.POINTER(_i64)]
 lib.nb_launch_count.argtypes = [_vp]
 lib.nb_launch_count.restype = _i64
@@ -211,6 +212,10 @@ def nb_set_profiling(c, on=True):
 def nb_force_ext(c, ni, x, v, eps2, acc, jrk, pot):
     """DEVICE x, v (3, ni) fp64 (v and jrk both None: acc + pot only)."""
     _check(lib.nb_force_ext(c, ni, _ptr(x), _ptr(v), eps2, _ptr(acc), _ptr(jrk), _ptr(pot)), "nb_force_ext")
+
+
+def nb_set_precision(c, mode):
+    _check(lib.nb_set_precision(c, int(mode)), "nb_set_precision")
 
 
 def nb_set_dt(c, first, count, dt):

@@ -86,6 +86,10 @@ class Context:
         self._keep_i = il
         return acc, jrk, pot
 
+    def precision(self, mode):
+        """0 = mixed (48-bit differences, fp32 pair terms), 1 = IEEE double throughout."""
+        nb.nb_set_precision(self.h, mode)
+
     def tuning(self, j_splits=0, reduce_mode=0):
         nb.nb_set_tuning(self.h, j_splits, reduce_mode)
 

@@ -1,0 +1,244 @@
+// force64.cu -- the pair loop in IEEE double precision throughout.
+//
+// "The integration of the orbits of objects with an extreme mass ratio, like
+// planetesimals around super-massive black holes, remains hard to achieve without IEEE-754 double
+// precision arithmetic.  The latest GPUs support double precision and therefore enable such
+// research."  nb_set_precision(ctx, 1) selects this kernel for nb_force / nb_force_ext.
+//
+// Same mapping as force.cu (CTA = 128 threads x 2 i-particles, one j-subset, j-tiles brought in by
+// 1-D bulk copies into an mbarrier ring, partial sums for reduce_kernel), but: the tile holds the
+// predicted state as doubles (8 arrays of TJ: x y z vx vy vz m flag = 8 KB), every difference,
+// product and sum is fp64, and the reciprocal square root is MUFU.RSQ on the fp32-rounded s
+// followed by two Newton steps in fp64 (error 2^-22 -> 1e-13 -> rounding).  The self pair is
+// masked by index (no epilogue correction), s = 0 pairs contribute nothing (R6), flagged-flagged
+// pairs use eps2 = 0 inside the loop (R7).  35 fp64 operations per interaction; the FP64 pipe
+// issues 64 lanes/clk/SM, so the ceiling is 1.83 interactions/clk/SM = 43 % of the 60-flop FP32
+// roofline.
+#include "nb_internal.h"
+
+namespace nb {
+
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32_(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init_(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s_(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+        "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+
+// 1/sqrt(s) to fp64 rounding: hardware approximation on the fp32-rounded argument + 2 Newton steps
+__device__ __forceinline__ double rsqrt64(double s)
+{
+    float y0;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(__double2float_rn(s)));
+    double y = (double)y0;
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const double e = fma(-(s * y), y, 1.0);      // 1 - s y^2
+        y = fma(0.5 * y, e, y);
+    }
+    return y;
+}
+
+struct Acc64 {
+    double ax, ay, az, jx, jy, jz, p;
+};
+
+template <bool JERK>
+__device__ __forceinline__ void pair64(const double* xi, Acc64& A, double xj, double yj, double zj,
+                                       double vxj, double vyj, double vzj, double mj, double e2, bool skip)
+{
+    const double dx = xj - xi[0], dy = yj - xi[1], dz = zj - xi[2];
+    const double s = fma(dz, dz, fma(dy, dy, fma(dx, dx, e2)));
+    double y = rsqrt64(s);
+    y = (skip || !(s > 0.0)) ? 0.0 : y;                // self pair (R5) or coincident with eps2 = 0 (R6)
+    const double y2 = y * y;
+    const double mr = mj * y;
+    const double mr3 = mr * y2;
+    A.p -= mr;
+    A.ax = fma(mr3, dx, A.ax);
+    A.ay = fma(mr3, dy, A.ay);
+    A.az = fma(mr3, dz, A.az);
+    if (JERK) {
+        const double wx = vxj - xi[3], wy = vyj - xi[4], wz = vzj - xi[5];
+        const double rv = fma(dz, wz, fma(dy, wy, dx * wx));
+        const double al = (y2 * -3.0) * rv;
+        A.jx = fma(mr3, fma(al, dx, wx), A.jx);
+        A.jy = fma(mr3, fma(al, dy, wy), A.jy);
+        A.jz = fma(mr3, fma(al, dz, wz), A.jz);
+    }
+}
+
+constexpr int STAGES64 = 4;
+constexpr int F64_SMEM = STAGES64 * (TILE64_BYTES + 16);
+
+// FLAGS: some particle carries the unsoftened flag (R7).  MODE as in force.cu: 0 = i by index,
+// 1 = i by value, 2 = i by value and acc + pot only.
+template <bool FLAGS, int MODE>
+__global__ void __launch_bounds__(FORCE_THREADS, 3) force64_kernel(ForceArgs P)
+{
+    constexpr bool JERK = (MODE != 2);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* tiles = reinterpret_cast<double*>(smem_raw);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STAGES64 * TILE64_BYTES);
+    int* rel = reinterpret_cast<int*>(smem_raw + STAGES64 * TILE64_BYTES + STAGES64 * 8);
+
+    const int tid = threadIdx.x;
+    const int it = blockIdx.x % P.n_itiles;
+    const int sp = blockIdx.x / P.n_itiles;
+    const int t0 = (int)(((int64_t)P.ntiles * sp) / P.splits);
+    const int t1 = (int)(((int64_t)P.ntiles * (sp + 1)) / P.splits);
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES64; ++s) {
+            mbar_init_(smem_u32_(&bars[s]), 1);
+            rel[s] = 0;
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int s = 0; s < STAGES64 && t0 + s < t1; ++s) {
+            mbar_expect_tx_(smem_u32_(&bars[s]), TILE64_BYTES);
+            bulk_g2s_(smem_u32_(tiles + s * TILE64_DOUBLES), P.pack64 + (int64_t)(t0 + s) * TILE64_DOUBLES,
+                      TILE64_BYTES, smem_u32_(&bars[s]));
+        }
+    }
+
+    // a2: i-gather, fp64
+    double xi[IPT][6];
+    int idx[IPT];
+    bool ifl[IPT];
+    Acc64 A[IPT];
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        const int ku = it * ITILE + u * FORCE_THREADS + tid;
+        const bool on = P.k0 + ku < P.ni;
+        ifl[u] = false;
+        if (MODE != 0) {
+            const int64_t e = on ? P.k0 + ku : 0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                xi[u][c] = P.ext_x[(int64_t)c * P.ni + e];
+                xi[u][3 + c] = (MODE == 1) ? P.ext_v[(int64_t)c * P.ni + e] : 0.0;
+            }
+            idx[u] = on ? -2 : -1;
+        } else {
+            int q = on ? P.i_list[P.k0 + ku] : 0;
+            const bool bad = (q < 0) || (q >= P.n);
+            if (bad) {
+                atomicOr(P.err, 1);
+                q = 0;
+            }
+            idx[u] = (on && !bad) ? q : -1;
+            const double* b = P.pack64 + (int64_t)(q / TJ) * TILE64_DOUBLES + (q % TJ);
+#pragma unroll
+            for (int c = 0; c < 6; ++c) xi[u][c] = b[c * TJ];
+            if (FLAGS) ifl[u] = (P.flags[q] & 1) != 0;
+        }
+        A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = 0.0;
+    }
+    __syncthreads();
+
+    for (int t = t0; t < t1; ++t) {
+        const int st = (t - t0) % STAGES64;
+        mbar_wait_(smem_u32_(&bars[st]), ((t - t0) / STAGES64) & 1);
+        const double* T = tiles + st * TILE64_DOUBLES;
+        const int jbase = t * TJ;
+#pragma unroll 2
+        for (int p = 0; p < TJ; p += 2) {
+            double2 g[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                if ((JERK || c < 3 || c == 6) && (FLAGS || c < 7))
+                    g[c] = *reinterpret_cast<const double2*>(T + c * TJ + p);
+#pragma unroll
+            for (int u = 0; u < IPT; ++u) {
+                double e0 = P.eps2d, e1 = P.eps2d;
+                if (FLAGS) {
+                    e0 = (ifl[u] && g[7].x != 0.0) ? 0.0 : P.eps2d;
+                    e1 = (ifl[u] && g[7].y != 0.0) ? 0.0 : P.eps2d;
+                }
+                pair64<JERK>(xi[u], A[u], g[0].x, g[1].x, g[2].x, g[3].x, g[4].x, g[5].x, g[6].x, e0,
+                             idx[u] == jbase + p);
+                pair64<JERK>(xi[u], A[u], g[0].y, g[1].y, g[2].y, g[3].y, g[4].y, g[5].y, g[6].y, e1,
+                             idx[u] == jbase + p + 1);
+            }
+        }
+        __syncwarp();
+        if ((tid & 31) == 0) {
+            const int old = atomicAdd(&rel[st], 1);
+            if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STAGES64 < t1) {
+                mbar_expect_tx_(smem_u32_(&bars[st]), TILE64_BYTES);
+                bulk_g2s_(smem_u32_(tiles + st * TILE64_DOUBLES),
+                          P.pack64 + (int64_t)(t + STAGES64) * TILE64_DOUBLES, TILE64_BYTES,
+                          smem_u32_(&bars[st]));
+            }
+        }
+    }
+
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        const int ku = it * ITILE + u * FORCE_THREADS + tid;
+        const double o[NOUT] = {A[u].ax, A[u].ay, A[u].az, A[u].jx, A[u].jy, A[u].jz, A[u].p};
+#pragma unroll
+        for (int c = 0; c < NOUT; ++c) P.part[((int64_t)sp * NOUT + c) * P.ni_pad + ku] = o[c];
+    }
+}
+
+template <bool FLAGS, int MODE>
+cudaError_t setup64(int* blocks)
+{
+    cudaError_t e = cudaFuncSetAttribute(force64_kernel<FLAGS, MODE>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM);
+    if (e != cudaSuccess) return e;
+    int b = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, force64_kernel<FLAGS, MODE>, FORCE_THREADS, F64_SMEM);
+    if (e == cudaSuccess && (*blocks == 0 || b < *blocks)) *blocks = b;
+    return e;
+}
+
+}  // namespace
+
+cudaError_t force64_kernel_setup(int* blocks_per_sm)
+{
+    *blocks_per_sm = 0;
+    cudaError_t e = setup64<false, 0>(blocks_per_sm);
+    if (e == cudaSuccess) e = setup64<true, 0>(blocks_per_sm);
+    if (e == cudaSuccess) e = setup64<false, 1>(blocks_per_sm);
+    if (e == cudaSuccess) e = setup64<false, 2>(blocks_per_sm);
+    return e;
+}
+
+cudaError_t launch_force64(const ForceArgs& a, int mode, cudaStream_t s)
+{
+    const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
+    if (mode == 1) force64_kernel<false, 1><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
+    else if (mode == 2) force64_kernel<false, 2><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
+    else if (a.any_flagged) force64_kernel<true, 0><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
+    else force64_kernel<false, 0><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace nb

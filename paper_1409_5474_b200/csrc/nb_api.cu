@@ -40,6 +40,11 @@ struct nb_ctx {
     double blk_t = 0.0;                 // what the last nb_next_block returned
     int64_t blk_ni = -1;
 
+    // full-double pair loop (force64.cu): fp64 tiles, allocated when the mode is first selected
+    int precision = 0;
+    double* pack64 = nullptr;
+    int blocks_per_sm64 = 1;
+
     int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
 
@@ -204,9 +209,9 @@ SrcPtrs make_src(const double* m, const double* x, const double* y, const double
 
 // choose the number of j-subsets S so that (i-tiles x S) fills the chip.  Efficiency
 // of a choice = useful tile-passes / (waves x resident CTAs x tiles per CTA).
-int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t part_bytes)
+int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t part_bytes,
+                  int64_t resident)
 {
-    const int64_t resident = (int64_t)c->sm_count * c->blocks_per_sm;
     int64_t smax = (int64_t)(part_bytes / (NOUT * sizeof(double) * (size_t)ni_pad));
     if (smax > ntiles) smax = ntiles;
     if (smax > 4096) smax = 4096;
@@ -233,6 +238,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
                double* pot, const double* ext_x = nullptr, const double* ext_v = nullptr)
 {
     const int kmode = ext_x ? (ext_v ? 1 : 2) : 0;
+    const bool f64 = c->precision == 1;
     if (!c->predicted) return NB_ERR_STATE;
     c->last[0] = c->last[1] = c->last[2] = 0;
     if (ni == 0) return NB_OK;
@@ -250,12 +256,14 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     a.ntiles = (int)((n_launch + TJ - 1) / TJ);
     a.eps2 = (float)eps2;
     a.any_flagged = (c->flagged.empty() || kmode != 0) ? 0 : 1;
-    const int mode = (c->tune_reduce && kmode == 0) ? 1 : 0;
+    a.pack64 = c->pack64;
+    a.eps2d = eps2;
+    const int mode = (c->tune_reduce && kmode == 0 && !f64) ? 1 : 0;
     // few active i: several threads share one i-particle and split the j of a tile
-    const int jl = ni <= ITILE / JL_MAX ? JL_MAX : (ni <= ITILE / JL_MID ? JL_MID : 1);
+    const int jl = f64 ? 1 : (ni <= ITILE / JL_MAX ? JL_MAX : (ni <= ITILE / JL_MID ? JL_MID : 1));
     const int itile = ITILE / jl;
     const int n_itiles = (int)((ni + itile - 1) / itile);
-    const int resident = c->sm_count * c->blocks_per_sm;
+    const int resident = c->sm_count * (f64 ? c->blocks_per_sm64 : c->blocks_per_sm);
 
     // the i-tiles are cut in two segments.  A = the largest multiple of the resident CTA
     // count, one j-subset each (whole waves of equal CTAs); B = the rest, whose j is split in S
@@ -270,7 +278,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     if (a.ntiles > 0) {
         if (tiles_b > 0) {
             const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a;
-            splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left);
+            splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left, resident);
         }
         if (mode) {
             if (launch_zero_out(acc, jrk, pot, ni, c->stream) != cudaSuccess) return NB_ERR_CUDA;
@@ -284,7 +292,9 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             a.ni_pad = (int)pad_a;
             a.splits = 1;
             a.part = c->part;
-            if (launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            if ((f64 ? launch_force64(a, kmode, c->stream)
+                     : launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
+                return NB_ERR_CUDA;
             ++launched;
         }
         if (tiles_b > 0) {
@@ -293,7 +303,9 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             a.ni_pad = (int)pad_b;
             a.splits = splits_b;
             a.part = part_b;
-            if (launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            if ((f64 ? launch_force64(a, kmode, c->stream)
+                     : launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
+                return NB_ERR_CUDA;
             ++launched;
         }
         if (rec) cudaEventRecord(rec->e[1], c->stream);
@@ -313,7 +325,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     r.store = c->store;
     r.flags = c->flags;
     r.flag_list = c->flag_list;
-    r.nflag = (int)c->flagged.size();
+    r.nflag = f64 ? 0 : (int)c->flagged.size();      // the fp64 kernel handles flagged pairs itself
     r.ni = (int)ni;
     r.ni_pad = (int)pad_a;
     r.splits = splits_a;
@@ -404,6 +416,7 @@ int nb_destroy(nb_ctx* c)
     DeviceGuard g(c->device);
     cudaStreamSynchronize(c->stream);
     if (c->own_slab && c->slab) cudaFree(c->slab);
+    if (c->pack64) cudaFree(c->pack64);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
     for (nb_ctx::Rec& R : c->ring)
         for (cudaEvent_t e : R.e)
@@ -593,7 +606,8 @@ int nb_predict(nb_ctx* c, double t)
     if (rc != NB_OK) return rc;
     nb_ctx::Rec* rec = c->n > 0 ? prof_next(c) : nullptr;
     if (rec) cudaEventRecord(rec->e[0], c->stream);
-    if (launch_predict(c->store, c->flags, c->pack, c->n, t, c->stream) != cudaSuccess)
+    if (launch_predict(c->store, c->flags, c->pack, c->precision == 1 ? c->pack64 : nullptr, c->n, t,
+                       c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
     if (rec) {
         cudaEventRecord(rec->e[1], c->stream);
@@ -658,6 +672,30 @@ int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, dou
         cudaMemcpyAsync(pot, d_pot, b, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
     return nb_sync(c);
+}
+
+int nb_set_precision(nb_ctx* c, int mode)
+{
+    if (!c || (mode != 0 && mode != 1)) return NB_ERR_ARG;
+    if (mode == c->precision) return NB_OK;
+    DeviceGuard g(c->device);
+    if (mode == 1 && !c->pack64) {
+        int rc = ensure_alloc(c);
+        if (rc != NB_OK) return rc;
+        if (force64_kernel_setup(&c->blocks_per_sm64) != cudaSuccess || c->blocks_per_sm64 < 1) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        const size_t bytes = (size_t)(c->n_cap / TJ) * TILE64_BYTES;
+        if (cudaMalloc(&c->pack64, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            c->pack64 = nullptr;
+            return NB_ERR_ALLOC;
+        }
+    }
+    c->precision = mode;
+    c->predicted = false;      // the tiles of the new mode are written by the next nb_predict
+    return NB_OK;
 }
 
 int nb_set_tuning(nb_ctx* c, int j_splits, int reduce_mode)

@@ -42,6 +42,11 @@ constexpr int JL_MID = 4, JL_MAX = 32;        // threads per i in the few-i vari
 constexpr int STAGES = NB_STAGES;             // j-tile ring depth
 constexpr int NOUT = 7;                       // ax ay az jx jy jz pot
 
+// pack64: the same tiles in fp64 for the full-double pair loop (force64.cu): 8 double arrays of TJ
+enum Pack64Field { Q_X = 0, Q_Y, Q_Z, Q_VX, Q_VY, Q_VZ, Q_M, Q_FLAG, NQF };
+constexpr int TILE64_DOUBLES = TJ * NQF;      // 1024
+constexpr int TILE64_BYTES = TILE64_DOUBLES * 8;   // 8192
+
 constexpr float PAD_POS = 1.0e10f;            // where the m = 0 padding records of the last tile sit
 
 struct StorePtrs {
@@ -67,6 +72,8 @@ struct ForceArgs {
     int n, ntiles, splits;
     float eps2;
     int any_flagged;
+    const double* pack64;     // fp64 tiles (precision mode 1), else unused
+    double eps2d;
 };
 
 struct ReduceArgs {
@@ -89,11 +96,13 @@ cudaError_t launch_set_j(const StorePtrs& dst, const SrcPtrs& src, int64_t first
                          cudaStream_t s);
 cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int32_t* idx,
                             int64_t count, int64_t n, int* err, cudaStream_t s);
-cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, int64_t n,
+cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64, int64_t n,
                            double t, cudaStream_t s);
 cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
                                  double* out, cudaStream_t s);
 cudaError_t force_kernel_setup(int* blocks_per_sm);
+cudaError_t force64_kernel_setup(int* blocks_per_sm);
+cudaError_t launch_force64(const ForceArgs& a, int mode, cudaStream_t s);
 cudaError_t launch_force(const ForceArgs& a, int jl, int mode, int atomic_mode, double* acc, double* jrk,
                          double* pot, cudaStream_t s);
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);

@@ -54,8 +54,11 @@ __device__ __forceinline__ void split(double x, float& hi, float& lo)
 
 // One thread = particles 2q, 2q+1.  n_pad = ntiles * TJ; particles in [n, n_pad) become m = 0
 // padding records far away.  Store arrays are n_cap >= n_pad long, so loads never leave them.
+// P64: also write the fp64 tiles of the full-double pair loop (force64.cu; 64 B more per particle).
+template <bool P64>
 __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_t* __restrict__ flags,
-                                                      float* __restrict__ pack, int64_t n,
+                                                      float* __restrict__ pack,
+                                                      double* __restrict__ pack64, int64_t n,
                                                       int64_t n_pad, double t)
 {
     const int64_t p = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
@@ -63,6 +66,7 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
     const double2 tj = ld2(st.f[F_T], p);
     const double dt0 = t - tj.x, dt1 = t - tj.y;
     float2 out[NPF];
+    double2 o64[NQF];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const double2 x = ld2(st.f[F_X + c], p), v = ld2(st.f[F_VX + c], p);
@@ -73,6 +77,10 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
         split(xp0, out[P_XH + c].x, out[P_XL + c].x);
         split(xp1, out[P_XH + c].y, out[P_XL + c].y);
         out[P_VX + c] = make_float2(__double2float_rn(vp0), __double2float_rn(vp1));
+        if (P64) {
+            o64[Q_X + c] = make_double2(xp0, xp1);
+            o64[Q_VX + c] = make_double2(vp0, vp1);
+        }
     }
     const double2 m = ld2(st.f[F_M], p);
     out[P_M] = make_float2(__double2float_rn(m.x), __double2float_rn(m.y));
@@ -85,6 +93,19 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
             if (p >= n) out[f].x = pad;
             if (p + 1 >= n) out[f].y = pad;
         }
+    }
+    if (P64) {
+        o64[Q_M] = m;
+        o64[Q_FLAG] = make_double2((double)(fl.x & 1u), (double)(fl.y & 1u));
+#pragma unroll
+        for (int f = 0; f < NQF; ++f) {
+            const double pad = (f <= Q_Z) ? (double)PAD_POS : 0.0;
+            if (p >= n) o64[f].x = pad;
+            if (p + 1 >= n) o64[f].y = pad;
+        }
+        double* b64 = pack64 + (p / TJ) * TILE64_DOUBLES + (p % TJ);
+#pragma unroll
+        for (int f = 0; f < NQF; ++f) *reinterpret_cast<double2*>(b64 + f * TJ) = o64[f];
     }
     float* base = pack + (p / TJ) * TILE_FLOATS + (p % TJ);
 #pragma unroll
@@ -133,13 +154,15 @@ cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int3
     return cudaGetLastError();
 }
 
-cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, int64_t n,
-                           double t, cudaStream_t s)
+cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64,
+                           int64_t n, double t, cudaStream_t s)
 {
     if (n == 0) return cudaSuccess;
     const int64_t n_pad = (n + TJ - 1) / TJ * TJ;
     const int64_t threads = n_pad / 2;
-    predict_kernel<<<(unsigned)((threads + 127) / 128), 128, 0, s>>>(store, flags, pack, n, n_pad, t);
+    const unsigned grid = (unsigned)((threads + 127) / 128);
+    if (pack64) predict_kernel<true><<<grid, 128, 0, s>>>(store, flags, pack, pack64, n, n_pad, t);
+    else predict_kernel<false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, n, n_pad, t);
     return cudaGetLastError();
 }
 
