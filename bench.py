@@ -53,6 +53,9 @@ def parse():
                     help="instead of the default line: time --steps device block steps (nb_step: "
                          "scheduler + predictor + force + corrector) of a Plummer sphere of N "
                          "particles with individual power-of-two steps")
+    ap.add_argument("--fp64", action="store_true",
+                    help="run the step with the full-double pair loop (nb_set_precision 1); the roofline "
+                         "is then the FP64 pipe (64 lanes per SM per clock)")
     ap.add_argument("--kick", action="store_true",
                     help="instead of the default line: time nb_force_ext on config 4's two galaxies "
                          "(stars of B by value against galaxy A as j-set), with jerk and acc + pot only")
@@ -262,6 +265,8 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     ctx = nbm.Context(n, max(ni, 1), device=local)
+    if args.fp64:
+        ctx.precision(1)
     ctx.load_case(case)
     h = ctx.h
     # device-resident step inputs: the active list and the active particles' corrected state (here:
@@ -402,9 +407,17 @@ def run_ours(args):
         "frac_of_ffma2_rate": (ach * 1e12 / FLOP_PER_INTERACTION * 33.0) / rate_ffma2,
         "note": "the pair body executes 33 FP32 lane-ops per interaction (DESIGN.md 7.2); "
                 "frac_of_ffma2_rate = executed lane-ops/s over the measured packed-FMA rate"}
+    if args.fp64:
+        # FP64 pipe: 64 lanes per SM per clock (measured DFMA/DADD rate, profiles/r1_pipe_probes.md)
+        p64 = fp32_peak_tflops / 2.0
+        roofline.update({"kernel": "force64_kernel", "peak": p64, "frac": ach / p64,
+                         "peak_source": "derived: %d SMs x 64 FP64 lanes x 2 x %.0f MHz" % (
+                             props.multi_processor_count, sm_max)})
+        roofline["fma_probe"]["note"] = "FP32 probe, not applicable to the fp64 loop (35 fp64 ops per interaction)"
+        roofline["fma_probe"]["frac_of_ffma2_rate"] = None
     if clocks:
         obs = props.multi_processor_count * FP32_LANES_PER_SM * 2 * clocks["sm_mhz"] * 1e6 / 1e12
-        roofline["frac_at_observed_clock"] = ach / obs
+        roofline["frac_at_observed_clock"] = ach / (obs / 2.0 if args.fp64 else obs)
     pred_gbs = PREDICT_BYTES_PER_PARTICLE * n / (pred_ms * 1e-3) / 1e9
     roofline_predict = {"kernel": "predict_kernel", "bound": "hbm", "achieved": pred_gbs,
                         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_gbs / peaks["hbm_gbs"],
@@ -413,15 +426,17 @@ def run_ours(args):
     line = {
         "metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
-        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f64" if args.fp64 else "f32",
         "data": "synthetic", "gflops": value * FLOP_PER_INTERACTION / 1e9,
         "config": {"workload": workload, "n_j": n, "n_i": ni, "eps2": case.eps2,
                    "step": "nb_update_j(active) + nb_predict + nb_force (gather, pairs, reduce)",
                    "parallelism": "i-sharded x%d, j replicated" % world,
                    "l2": "no flush: per-step working set (j-store %.0f MB + pack %.0f MB + outputs "
                          "%.0f MB) exceeds the L2" % (112e-6 * n, 44e-6 * n, 56e-6 * ni),
-                   "arithmetic": "two-float (48-bit) position differences, fp32 pair terms, "
-                                 "fp32 per-tile sums flushed to fp64"},
+                   "arithmetic": ("IEEE double throughout (rsqrt: MUFU + 2 Newton steps)" if args.fp64 else
+                                  "two-float (48-bit) position differences, fp32 pair terms, "
+                                  "fp32 per-tile sums flushed to fp64")},
         "clocks": ({"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"],
                     "reasons": clocks["reasons"], "power_w_max": clocks["power_w_max"],
                     "samples": clocks["samples"]} if clocks else None),
