@@ -398,7 +398,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         } else {
 #pragma unroll
             for (int c = 0; c < NOUT; ++c)
-                P.part[((int64_t)sp2 * NOUT + c) * P.ni_pad + ku] = o[c];
+                P.part[((int64_t)c * P.ni_pad + ku) * P.splits + sp2] = o[c];   // [c][i][subset]
         }
     }
 }
@@ -431,7 +431,7 @@ __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
         const int kl = in_b ? k - R.kA : k, ns = in_b ? R.splits_b : R.splits;
         for (int s = WARP ? lane : 0; s < ns; s += WARP ? 32 : 1) {
 #pragma unroll
-            for (int c = 0; c < NOUT; ++c) o[c] += part[((int64_t)s * NOUT + c) * stride + kl];
+            for (int c = 0; c < NOUT; ++c) o[c] += part[((int64_t)c * stride + kl) * ns + s];
         }
         if (WARP) {
 #pragma unroll

@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, 3) force64_kernel(ForceArgs P)
         const int ku = it * ITILE + u * FORCE_THREADS + tid;
         const double o[NOUT] = {A[u].ax, A[u].ay, A[u].az, A[u].jx, A[u].jy, A[u].jz, A[u].p};
 #pragma unroll
-        for (int c = 0; c < NOUT; ++c) P.part[((int64_t)sp * NOUT + c) * P.ni_pad + ku] = o[c];
+        for (int c = 0; c < NOUT; ++c) P.part[((int64_t)c * P.ni_pad + ku) * P.splits + sp] = o[c];
     }
 }
 

@@ -227,10 +227,8 @@ get_state_kernel(StorePtrs st, const double* __restrict__ dts, int64_t first, in
 cudaError_t launch_select(const double* t, const double* dt, int64_t n, unsigned long long* meta,
                           int* counts, int32_t* list, int64_t cap, int sm_count, cudaStream_t s)
 {
-    // meta[0] = ~0 (identity of the min), meta[1] = 0
+    // meta[0] = ~0 (identity of the min); meta[1] is plainly written by block 0
     cudaError_t e = cudaMemsetAsync(meta, 0xff, 8, s);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(meta + 1, 0, 8, s);
     if (e != cudaSuccess) return e;
     int64_t want = (n + SEL_THREADS - 1) / SEL_THREADS;
     int grid = sm_count * 4;                       // co-resident by a wide margin (256 threads, ~2 KB smem)

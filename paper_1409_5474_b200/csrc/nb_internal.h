@@ -77,8 +77,8 @@ struct ForceArgs {
 };
 
 struct ReduceArgs {
-    const double* part;       // segment A: [splits][NOUT][ni_pad], positions [0, kA)
-    const double* part_b;     // segment B: [splits_b][NOUT][ni_pad_b], positions [kA, ni)
+    const double* part;       // segment A: [NOUT][ni_pad][splits] (subset index fastest), positions [0, kA)
+    const double* part_b;     // segment B: [NOUT][ni_pad_b][splits_b], positions [kA, ni)
     int kA, ni_pad_b, splits_b;
     const int32_t* i_list;
     double *acc, *jrk, *pot;

@@ -1,0 +1,327 @@
+// pipe_probe.cu -- standalone probe of the SM pipes the pair kernels live on.
+// Not part of libnb.so and not on any product path: it exists so that the rates DESIGN.md quotes
+// (FFMA vs FFMA2, FP64 lanes per clock, MUFU, and whether fp32 and fp64 warps overlap) can be
+// re-measured:   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o pipe_probe pipe_probe.cu && ./pipe_probe
+// Part 1: raw instruction rates (8 independent register chains per thread, full chip).
+// Part 2: the fp32 two-float pair body and an fp64 pair body, alone and side by side in one CTA.
+#include <cstdio>
+#include <cstdlib>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#define CK(x) do { cudaError_t e = (x); if (e != cudaSuccess) { printf("CUDA error %s at %d\n", cudaGetErrorString(e), __LINE__); exit(1);} } while (0)
+
+__device__ __forceinline__ float rsq(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// ---------------- raw pipe rates: NCH independent chains per thread ----------------
+// kind 0 FFMA2, 1 FFMA, 2 FADD2, 3 DADD, 4 F2F.F32.F64 (+DADD feed), 5 MUFU.RSQ, 6 FMUL2, 7 DFMA
+// 8 IADD3/LOP3 mix (alu), 9: FFMA2 + alu interleaved 1:1, 10: FFMA2 + DADD 4:1, 11: FFMA2 + F2F 4:1
+// 12: FFMA2 + MUFU 8:1
+template <int KIND>
+__global__ void __launch_bounds__(128) rate_kernel(float* out, int iters, float a0, double d0)
+{
+    constexpr int NCH = 8;
+    float2 f[NCH];
+    double d[NCH];
+    unsigned u[NCH];
+    float s[NCH];
+    for (int c = 0; c < NCH; ++c) {
+        f[c] = make_float2(a0 + c + threadIdx.x, a0 - c);
+        d[c] = d0 + c + threadIdx.x;
+        u[c] = threadIdx.x * 31 + c;
+        s[c] = a0 + c * 0.5f + threadIdx.x;
+    }
+    const float2 m = make_float2(a0 * 0.999f, a0 * 1.001f);
+    const float2 b = make_float2(a0 * 1e-3f, -a0 * 1e-3f);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                if (KIND == 0) f[c] = __ffma2_rn(f[c], m, b);
+                if (KIND == 1) s[c] = fmaf(s[c], m.x, b.x);
+                if (KIND == 2) f[c] = __fadd2_rn(f[c], b);
+                if (KIND == 3) d[c] = __dadd_rn(d[c], d0);
+                if (KIND == 4) { s[c] = __double2float_rn(d[c]); d[c] = __dadd_rn(d[c], (double)s[c] * 0.0 + d0); }
+                if (KIND == 5) s[c] = rsq(s[c]);
+                if (KIND == 6) f[c] = __fmul2_rn(f[c], m);
+                if (KIND == 7) d[c] = fma(d[c], d0, d0);
+                if (KIND == 8) { u[c] = (u[c] + 0x9e3779b9u) ^ (u[c] >> 3); }
+                if (KIND == 9) { f[c] = __ffma2_rn(f[c], m, b); u[c] = (u[c] & 0x7fffffffu) + 0x38000001u; }
+                if (KIND == 10) { f[c] = __ffma2_rn(f[c], m, b); if ((c & 3) == 0) d[c] = __dadd_rn(d[c], d0); }
+                if (KIND == 13) { f[c] = __ffma2_rn(f[c], m, b); s[c] = fmaf(s[c], m.x, b.x); }
+                if (KIND == 14) { f[c] = __ffma2_rn(f[c], m, b); if (c & 1) s[c] = fmaf(s[c], m.x, b.x); }
+                if (KIND == 12) { f[c] = __ffma2_rn(f[c], m, b); if (c == 0) s[c] = rsq(s[c]); }
+            }
+        }
+    }
+    float acc = 0.f;
+    for (int c = 0; c < NCH; ++c) acc += f[c].x + f[c].y + (float)d[c] + s[c] + (float)u[c];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
+
+constexpr int TJ = 128;
+struct Acc { float2 ax, ay, az, jx, jy, jz, p; };
+
+__device__ __forceinline__ void body32(float2 dx, float2 dy, float2 dz, float2 wx, float2 wy, float2 wz,
+                                       float2 m, float2 eps2, float2 m3, Acc& A)
+{
+    float2 r2 = __ffma2_rn(dx, dx, eps2);
+    r2 = __ffma2_rn(dy, dy, r2);
+    r2 = __ffma2_rn(dz, dz, r2);
+    float2 rinv;
+    rinv.x = rsq(r2.x);
+    rinv.y = rsq(r2.y);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 mr = __fmul2_rn(m, rinv);
+    const float2 mr3 = __fmul2_rn(mr, rinv2);
+    float2 rv = __fmul2_rn(dx, wx);
+    rv = __ffma2_rn(dy, wy, rv);
+    rv = __ffma2_rn(dz, wz, rv);
+    const float2 al = __fmul2_rn(__fmul2_rn(rinv2, m3), rv);
+    A.p = __fadd2_rn(A.p, mr);
+    A.ax = __ffma2_rn(mr3, dx, A.ax);
+    A.ay = __ffma2_rn(mr3, dy, A.ay);
+    A.az = __ffma2_rn(mr3, dz, A.az);
+    A.jx = __ffma2_rn(mr3, __ffma2_rn(al, dx, wx), A.jx);
+    A.jy = __ffma2_rn(mr3, __ffma2_rn(al, dy, wy), A.jy);
+    A.jz = __ffma2_rn(mr3, __ffma2_rn(al, dz, wz), A.jz);
+}
+__device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
+
+// fp64 -> fp32 (truncating) and fp32 -> fp64 through the integer pipe (normal numbers only)
+__device__ __forceinline__ float d2f_bits(double d)
+{
+    const unsigned hi = (unsigned)__double2hiint(d), lo = (unsigned)__double2loint(d);
+    const unsigned h2 = hi - 0x38000000u;
+    return __uint_as_float(__funnelshift_l(lo, h2, 3));
+}
+__device__ __forceinline__ double f2d_bits(float f)
+{
+    const unsigned u = __float_as_uint(f);
+    return __hiloint2double((int)((u >> 3) + 0x38000000u), (int)(u << 29));
+}
+
+struct Acc64 { double ax, ay, az, jx, jy, jz, p; };
+
+// CONV: 0 = F2F conversions (XU pipe), 1 = integer-pipe bit conversions
+template <int CONV>
+__device__ __forceinline__ void body64(double xi, double yi, double zi, double vxi, double vyi, double vzi,
+                                       double xj, double yj, double zj, double vxj, double vyj, double vzj,
+                                       double m, double eps2, Acc64& A)
+{
+    const double dx = xj - xi, dy = yj - yi, dz = zj - zi;
+    const double wx = vxj - vxi, wy = vyj - vyi, wz = vzj - vzi;
+    const double r2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, eps2)));
+    const float r2f = CONV ? d2f_bits(r2) : __double2float_rn(r2);
+    const float rf = rsq(r2f);
+    const double rinv = CONV ? f2d_bits(rf) : (double)rf;
+    const double rinv2 = rinv * rinv;
+    const double mr = m * rinv;
+    const double mr3 = mr * rinv2;
+    const double rv = fma(dz, wz, fma(dy, wy, dx * wx));
+    const double al = (rinv2 * -3.0) * rv;
+    A.p += mr;
+    A.ax = fma(mr3, dx, A.ax);
+    A.ay = fma(mr3, dy, A.ay);
+    A.az = fma(mr3, dz, A.az);
+    A.jx = fma(mr3, fma(al, dx, wx), A.jx);
+    A.jy = fma(mr3, fma(al, dy, wy), A.jy);
+    A.jz = fma(mr3, fma(al, dz, wz), A.jz);
+}
+
+// NW32 warps run the fp32 two-float body (2 i per thread), NW64 warps the fp64 body (IPT64 i per
+// thread); all read the same tile in shared memory, reps times.
+template <int NW32, int NW64, int IPT64, int CONV, int MINB>
+__global__ void __launch_bounds__((NW32 + NW64) * 32, MINB)
+hetero_kernel(float* out, int reps, float eps2f, double eps2d)
+{
+    __shared__ __align__(16) float T[10 * TJ];       // xh yh zh xl yl zl vx vy vz m
+    __shared__ __align__(16) double TD[7 * TJ];      // x y z vx vy vz m
+    const int tid = threadIdx.x, nthr = (NW32 + NW64) * 32;
+    for (int q = tid; q < TJ; q += nthr) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.37 * ((q * 2654435761u + c * 40503u) % 1000) / 1000.0 - 0.18;
+            TD[c * TJ + q] = x;
+            const float h = (float)x;
+            T[c * TJ + q] = h;
+            T[(3 + c) * TJ + q] = (float)(x - (double)h);
+            T[(6 + c) * TJ + q] = 0.01f * (float)((q * 7 + c * 13) % 17 - 8);
+            TD[(3 + c) * TJ + q] = 0.01 * ((q * 7 + c * 13) % 17 - 8);
+        }
+        T[9 * TJ + q] = 1.0f / 1048576.0f;
+        TD[6 * TJ + q] = 1.0 / 1048576.0;
+    }
+    __syncthreads();
+    const int warp = tid >> 5;
+    float res = 0.f;
+    if (warp < NW32) {
+        constexpr int IPT = 2;
+        float2 nxh[IPT][3], nxl[IPT][3], nv[IPT][3];
+        Acc A[IPT];
+        for (int u = 0; u < IPT; ++u) {
+            for (int c = 0; c < 3; ++c) {
+                const double x = 0.001 * (tid + 128 * u) + 0.1 * c + 1e-9 * blockIdx.x;
+                const float h = (float)x;
+                nxh[u][c] = dup(-h);
+                nxl[u][c] = dup(-(float)(x - (double)h));
+                nv[u][c] = dup(0.003f * (tid % 7) - 0.01f * c);
+            }
+            A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
+        }
+        const float2 eps2 = dup(eps2f), m3 = dup(-3.0f);
+        for (int r = 0; r < reps; ++r) {
+#pragma unroll 2
+            for (int p = 0; p < TJ; p += 4) {
+                float4 f[10];
+#pragma unroll
+                for (int c = 0; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        float2 d[3], w[3];
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const float2 xh = h ? make_float2(f[c].z, f[c].w) : make_float2(f[c].x, f[c].y);
+                            const float2 xl = h ? make_float2(f[3 + c].z, f[3 + c].w) : make_float2(f[3 + c].x, f[3 + c].y);
+                            const float2 vv = h ? make_float2(f[6 + c].z, f[6 + c].w) : make_float2(f[6 + c].x, f[6 + c].y);
+                            d[c] = __fadd2_rn(__fadd2_rn(xh, nxh[u][c]), __fadd2_rn(xl, nxl[u][c]));
+                            w[c] = __fadd2_rn(vv, nv[u][c]);
+                        }
+                        const float2 mm = h ? make_float2(f[9].z, f[9].w) : make_float2(f[9].x, f[9].y);
+                        body32(d[0], d[1], d[2], w[0], w[1], w[2], mm, eps2, m3, A[u]);
+                    }
+                }
+            }
+        }
+        for (int u = 0; u < IPT; ++u)
+            res += A[u].ax.x + A[u].ax.y + A[u].ay.x + A[u].ay.y + A[u].az.x + A[u].az.y + A[u].jx.x + A[u].jx.y +
+                   A[u].jy.x + A[u].jy.y + A[u].jz.x + A[u].jz.y + A[u].p.x + A[u].p.y;
+    } else {
+        double xi[IPT64][6];
+        Acc64 A[IPT64];
+        for (int u = 0; u < IPT64; ++u) {
+            for (int c = 0; c < 3; ++c) {
+                xi[u][c] = 0.001 * (tid + 128 * u) + 0.1 * c + 1e-9 * blockIdx.x;
+                xi[u][3 + c] = 0.003 * (tid % 7) - 0.01 * c;
+            }
+            A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = 0.0;
+        }
+        for (int r = 0; r < reps; ++r) {
+#pragma unroll 2
+            for (int p = 0; p < TJ; p += 2) {
+                double2 g[7];
+#pragma unroll
+                for (int c = 0; c < 7; ++c) g[c] = *reinterpret_cast<const double2*>(TD + c * TJ + p);
+#pragma unroll
+                for (int u = 0; u < IPT64; ++u) {
+                    body64<CONV>(xi[u][0], xi[u][1], xi[u][2], xi[u][3], xi[u][4], xi[u][5], g[0].x, g[1].x,
+                                 g[2].x, g[3].x, g[4].x, g[5].x, g[6].x, eps2d, A[u]);
+                    body64<CONV>(xi[u][0], xi[u][1], xi[u][2], xi[u][3], xi[u][4], xi[u][5], g[0].y, g[1].y,
+                                 g[2].y, g[3].y, g[4].y, g[5].y, g[6].y, eps2d, A[u]);
+                }
+            }
+        }
+        for (int u = 0; u < IPT64; ++u)
+            res += (float)(A[u].ax + A[u].ay + A[u].az + A[u].jx + A[u].jy + A[u].jz + A[u].p);
+    }
+    out[blockIdx.x * nthr + tid] = res;
+}
+
+static float* d_out;
+static int nsm;
+
+template <typename F>
+float time_ms(F launch)
+{
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    launch(); launch();
+    CK(cudaDeviceSynchronize());
+    float best = 1e30f;
+    for (int r = 0; r < 3; ++r) {
+        CK(cudaEventRecord(e0));
+        launch();
+        CK(cudaEventRecord(e1));
+        CK(cudaEventSynchronize(e1));
+        float ms; CK(cudaEventElapsedTime(&ms, e0, e1));
+        if (ms < best) best = ms;
+    }
+    CK(cudaGetLastError());
+    return best;
+}
+
+template <int NW32, int NW64, int IPT64, int CONV, int MINB>
+void run(int reps32_only = 0)
+{
+    const int reps = 300;
+    const int grid = nsm * MINB * 5;
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hetero_kernel<NW32, NW64, IPT64, CONV, MINB>,
+                                                     (NW32 + NW64) * 32, 0));
+    cudaFuncAttributes fa;
+    CK(cudaFuncGetAttributes(&fa, hetero_kernel<NW32, NW64, IPT64, CONV, MINB>));
+    float ms = time_ms([&] { hetero_kernel<NW32, NW64, IPT64, CONV, MINB><<<grid, (NW32 + NW64) * 32>>>(d_out, reps, 1e-6f, 1e-6); });
+    const double i32 = (double)grid * NW32 * 64 * (double)TJ * reps;
+    const double i64 = (double)grid * NW64 * 32 * IPT64 * (double)TJ * reps;
+    const double r = (i32 + i64) / (ms * 1e-3);
+    printf("fp32 warps %d  fp64 warps %d (ipt %d, conv %d) minb %d regs %3d occ %d : %8.3f ms  %9.3e inter/s = %5.1f%% of 1.2408e12"
+           "   (fp32 share %.2f)\n",
+           NW32, NW64, IPT64, CONV, MINB, fa.numRegs, occ, ms, r, r / 1.2408e12 * 100, i32 / (i32 + i64));
+}
+
+template <int KIND>
+void run_rate(const char* name, double ops_per_iter_thread, int ctas_per_sm)
+{
+    const int iters = 4000;
+    const int grid = nsm * ctas_per_sm;
+    float ms = time_ms([&] { rate_kernel<KIND><<<grid, 128>>>(d_out, iters, 1.0f, 1.0); });
+    // ops per thread per iter = 64 (8 x 8) of the primary kind
+    const double ops = (double)grid * 128 * iters * ops_per_iter_thread;
+    printf("rate %-28s ctas/SM %2d : %8.3f ms  %7.2f Gop/s/SM  (thread-ops; per-clk needs the clock)\n", name,
+           ctas_per_sm, ms, ops / (ms * 1e-3) / nsm / 1e9);
+}
+
+
+int main()
+{
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, 0));
+    nsm = prop.multiProcessorCount;
+    printf("device %s, %d SMs\n", prop.name, nsm);
+    CK(cudaMalloc(&d_out, (size_t)nsm * 64 * 1024 * 4));
+    printf("-- raw rates, thread-operations per second per SM (divide by the clock for lanes per clock)\n");
+    run_rate<1>("FFMA", 64, 4);
+    run_rate<0>("FFMA2", 64, 4);
+    run_rate<2>("FADD2", 64, 4);
+    run_rate<6>("FMUL2", 64, 4);
+    run_rate<3>("DADD", 64, 4);
+    run_rate<7>("DFMA", 64, 4);
+    run_rate<5>("MUFU.RSQ", 64, 4);
+    run_rate<8>("alu IADD+LOP/SHF", 64, 4);
+    run_rate<10>("FFMA2 + DADD 4:1 (count FFMA2)", 64, 4);
+    run_rate<13>("FFMA2 + FFMA 1:1 (count FFMA2)", 64, 4);
+    printf("-- pair bodies: fp32 two-float (2 i per thread) and fp64 (ipt i per thread) warps in one CTA\n");
+    run<4, 0, 1, 0, 3>();
+    run<0, 4, 1, 0, 3>();
+    run<0, 4, 1, 1, 3>();
+    run<0, 4, 2, 1, 3>();
+    run<0, 4, 2, 0, 3>();
+    run<0, 4, 2, 1, 4>();
+    run<0, 8, 2, 1, 2>();
+    run<4, 4, 1, 1, 1>();
+    run<4, 4, 2, 1, 1>();
+    run<4, 4, 2, 0, 1>();
+    run<8, 4, 1, 1, 1>();
+    run<8, 4, 2, 1, 1>();
+    run<8, 8, 1, 1, 1>();
+    run<8, 8, 2, 1, 1>();
+    run<4, 4, 1, 1, 2>();
+    run<4, 4, 2, 1, 2>();
+    run<4, 2, 2, 1, 2>();
+    run<8, 4, 2, 0, 1>();
+    run<12, 4, 2, 1, 1>();
+    return 0;
+}
