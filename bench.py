@@ -228,9 +228,12 @@ def measured_peaks():
         return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE force_kernel launch of the default workload,
-# from the committed `ncu --set full` capture (profiles/r1_force_full.md); None until captured.
-FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": None}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant force_kernel launch of the default
+# workload (the whole-wave segment, 3552 of the call's CTAs and 86 % of its time), from the committed
+# `ncu --set full` capture profiles/r1_cfg3_full.md: 56.97 MB read + 37.72 MB written.  (ncu returned
+# no DRAM counters for the call's second, shorter launch.)  Algorithmic bytes of that launch: the
+# 46 MB pack once + 51 MB of partial sums.
+FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": 94.69e6}
 
 
 def run_ours(args):
