@@ -225,7 +225,7 @@ int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, siz
         const int64_t per = (ntiles + s - 1) / s;
         // each CTA also pays a fixed cost of about two tiles (gather, pipeline fill, partial store)
         const double eff = (double)n_itiles * ntiles / ((double)waves * resident * (per + 2));
-        if (eff > best_eff * 1.02) {   // prefer fewer splits unless clearly better
+        if (eff > best_eff * 1.004) {   // prefer fewer splits unless better by more than noise
             best_eff = eff;
             best = (int)s;
         }

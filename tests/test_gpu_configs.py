@@ -128,3 +128,36 @@ def test_config5_group(nbmod):
         ctx.predict(0.0)
         errs, info, nchk = sampled_parity(ctx, c, il, 0.0, 4096, nbgen.SEED0 * 100 + 5)
         print("cfg5 checked=%d" % nchk, errs, info)
+
+
+def test_p10_smooth_field_of_the_big_plummer_sphere(nbmod):
+    """P10: where the oracle is only sampled, a gross error anywhere would still show
+    in the mean field.  Radially binned mean of a.r_hat and of pot against the analytic Plummer
+    sphere (a = 3 pi / 16, M = 1): -r / (r^2 + a^2)^(3/2) and -1 / sqrt(r^2 + a^2), within 3 % in
+    every bin that holds >= 1e4 particles.  Statistical, not a parity test."""
+    c = nbgen.config3()
+    il = c.i_lists[-1]
+    with nbmod.Context(c.n) as ctx:
+        ctx.set_j(c.m, c.x, c.v)                       # t = 0: positions as sampled
+        ctx.predict(0.0)
+        acc, jrk, pot = _np(ctx.force(il, c.eps2))
+        ctx.sync()
+    x = c.x[:, il]
+    r = np.sqrt((x * x).sum(0))
+    ar = (acc * x).sum(0) / r
+    a = nbgen.HENON_A
+    # (the sampler's 0.999 mass-fraction cut shifts both means by ~0.1-0.2 %, far inside the 3 %)
+    edges = np.quantile(r, np.linspace(0.0, 1.0, 41))
+    which = np.clip(np.searchsorted(edges, r, side="right") - 1, 0, 39)
+    checked = 0
+    for b in range(40):
+        sel = which == b
+        if sel.sum() < 10000:
+            continue
+        rb = r[sel]
+        want_a = (-rb / (rb * rb + a * a) ** 1.5).mean()
+        want_p = (-1.0 / np.sqrt(rb * rb + a * a)).mean()
+        assert abs(ar[sel].mean() / want_a - 1.0) < 0.03, (b, ar[sel].mean(), want_a)
+        assert abs(pot[sel].mean() / want_p - 1.0) < 0.03, (b, pot[sel].mean(), want_p)
+        checked += 1
+    assert checked >= 30
