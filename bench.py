@@ -473,27 +473,34 @@ def run_blockstep(args):
     eps2, eta, lo, hi = (4.0 / n) ** 2, 0.02, 2.0 ** -24, 2.0 ** -4
     m, x, v = nbgen.plummer(n, nbgen.SEED0 + 6)
     il = np.arange(n, dtype=np.int32)
-    with nbm.Context(n) as ctx:
-        ctx.set_j(m, x, v)
-        ctx.predict(0.0)
-        ga, gj, gp = ctx.force(il, eps2)
-        ctx.init_steps(il, ga, gj, eta, lo, hi)
-        for _ in range(max(args.warmup, 3)):
-            ctx.step(eps2, eta, lo, hi)
-        ctx.sync()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        l0 = ctx.launch_count()
-        sizes = []
-        w0 = time.perf_counter()
-        e0.record()
-        for _ in range(args.steps):
-            t, ni = ctx.step(eps2, eta, lo, hi)
-            sizes.append(ni)
-        e1.record()
-        ctx.sync()
-        wall = time.perf_counter() - w0
-        ms = e0.elapsed_time(e1)
-        launches = ctx.launch_count() - l0
+    def run(fused):
+        """The same `--steps` block steps from the same start, with or without the fused path."""
+        with nbm.Context(n) as ctx:
+            ctx.fused(fused)
+            ctx.set_j(m, x, v)
+            ctx.predict(0.0)
+            ga, gj, gp = ctx.force(il, eps2)
+            ctx.init_steps(il, ga, gj, eta, lo, hi)
+            for _ in range(max(args.warmup, 3)):
+                ctx.step(eps2, eta, lo, hi)
+            ctx.sync()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = ctx.launch_count()
+            sz = []
+            w0 = time.perf_counter()
+            e0.record()
+            for _ in range(args.steps):
+                t, ni = ctx.step(eps2, eta, lo, hi)
+                sz.append(ni)
+            e1.record()
+            ctx.sync()
+            return e0.elapsed_time(e1), time.perf_counter() - w0, ctx.launch_count() - l0, sz, t
+
+    # A/B inside one process, interleaved (off, on, off, on): numbers from different gpurun calls
+    # differ by +-20 % for a latency-bound loop and must not be compared with each other
+    runs = [(f, run(f)) for f in (False, True, False, True)]
+    ms_off = min(r[0] for f, r in runs if not f)
+    ms, wall, launches, sizes, t = min((r for f, r in runs if f), key=lambda r: r[0])
     sizes = np.array(sizes, dtype=np.float64)
     line = {"metric": "interactions/s", "value": float(sizes.sum() * n / (ms * 1e-3)),
             "unit": "interactions/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -504,6 +511,8 @@ def run_blockstep(args):
             "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),
                       "min_n_i": int(sizes.min()), "max_n_i": int(sizes.max()),
                       "particle_steps_per_s": float(sizes.sum() / (ms * 1e-3)), "t_end": t},
+            "fused_ab": {"ms_per_step_fused_off": ms_off / args.steps, "ms_per_step_fused_on": ms / args.steps,
+                         "note": "same process, same schedule, best of 2 each, interleaved"},
             "gpu_launches": int(launches)}
     print(json.dumps(line))
     return 0

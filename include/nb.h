@@ -150,6 +150,17 @@ int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
 int nb_force_ext(nb_ctx* c, int64_t ni, const double* x, const double* v, double eps2, double* acc,
                  double* jrk, double* pot);
 
+/* Forces at time t on a HANDFUL of members of the j-set (ni <= NB_FUSED_MAX), in one pass over the
+ * j-store: the Hermite predictor (R1) runs inside the pair loop, for i and j alike, instead of as a
+ * separate nb_predict pass (PAPER.md:55 counts the prediction step among the costs of a step;
+ * PAPER.md:51 is about few active particles).  IEEE double throughout (the
+ * call is HBM-bound: 112 B read per j-particle), self pair masked by index, flagged pairs
+ * unsoftened (R5-R7).  Same outputs and layout as nb_force; needs no prior nb_predict and neither
+ * reads nor refreshes the packed predicted state.  ni > NB_FUSED_MAX is NB_ERR_ARG. */
+#define NB_FUSED_MAX 8
+int nb_force_fused(nb_ctx* c, double t, const int32_t* i_list, int64_t ni, double eps2, double* acc,
+                   double* jrk, double* pot);
+
 /* HOST-pointer form: i_list, acc, jrk, pot are host arrays; copies in, runs, copies back and
  * synchronises the stream before returning (so it also returns latched errors). */
 int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
@@ -237,6 +248,11 @@ int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const do
  * eps2) -> nb_correct.  HOST outputs *t (the block time) and *ni (particles advanced).  The forces
  * of the block stay in a context-owned buffer (nb_block_forces). */
 int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, double* t, int64_t* ni);
+
+/* nb_step takes blocks of <= NB_FUSED_MAX particles through nb_force_fused (default on); after
+ * such a step the packed predicted state is stale: call nb_predict before nb_force /
+ * nb_get_predicted (they return NB_ERR_STATE until then).  on = 0 switches this off. */
+int nb_set_fused(nb_ctx* c, int on);
 
 /* DEVICE addresses of the last nb_step's acc [3][ni], jrk [3][ni], pot [ni] (any may be NULL). */
 int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const double** pot);

@@ -17,7 +17,7 @@ NB_MAX_FLAGGED = 1024
 EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
-    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_host", "nb_set_precision", "nb_set_tuning",
+    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_precision", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_probe_fp32", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_block_forces", "nb_strerror", "nb_version",
 ]
@@ -59,6 +59,8 @@ lib.nb_sync.argtypes = [_vp]
 lib.nb_strerror.argtypes = [_i32]
 lib.nb_strerror.restype = ctypes.c_char_p
 lib.nb_probe_fp32.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(_dbl)]
+lib.nb_force_fused.argtypes = [_vp, _dbl, _vp, _i64, _dbl, _vp, _vp, _vp]
+lib.nb_set_fused.argtypes = [_vp, _i32]
 lib.nb_force_ext.argtypes = [_vp, _i64, _vp, _vp, _dbl, _vp, _vp, _vp]
 lib.nb_set_dt.argtypes = [_vp, _i64, _i64, _vp]
 lib.nb_get_state.argtypes = [_vp, _i64, _i64, _vp]
@@ -207,6 +209,18 @@ def nb_launch_count(c):
 
 def nb_set_profiling(c, on=True):
     _check(lib.nb_set_profiling(c, 1 if on else 0), "nb_set_profiling")
+
+
+NB_FUSED_MAX = 8
+
+
+def nb_force_fused(c, t, i_list, ni, eps2, acc, jrk, pot):
+    _check(lib.nb_force_fused(c, float(t), _ptr(i_list), ni, float(eps2), _ptr(acc), _ptr(jrk), _ptr(pot)),
+           "nb_force_fused")
+
+
+def nb_set_fused(c, on):
+    _check(lib.nb_set_fused(c, int(bool(on))), "nb_set_fused")
 
 
 def nb_force_ext(c, ni, x, v, eps2, acc, jrk, pot):

@@ -113,6 +113,20 @@ class Context:
         the results are back on the host."""
         nb.nb_force_host(self.h, i_list, i_list.shape[0], eps2, acc, jrk, pot)
 
+    def force_fused(self, t, i_list, eps2):
+        """Forces at time t on <= NB_FUSED_MAX members of the j-set, predictor fused in (one pass)."""
+        il = self._dev(i_list, torch.int32)
+        ni = il.shape[0]
+        acc = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        jrk = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
+        nb.nb_force_fused(self.h, t, il, ni, eps2, acc, jrk, pot)
+        self._keep = [il]
+        return acc, jrk, pot
+
+    def fused(self, on=True):
+        nb.nb_set_fused(self.h, on)
+
     def force_ext(self, x, v, eps2):
         """Forces on particles given by value: x, v (3, ni) of any kind; v None -> (acc, None, pot)."""
         dx = self._dev(x)

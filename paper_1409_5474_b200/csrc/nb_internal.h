@@ -117,6 +117,9 @@ cudaError_t launch_init_steps(const StorePtrs& st, double* dts, const int32_t* l
                               double dt_max, int* err, cudaStream_t s);
 cudaError_t launch_get_state(const StorePtrs& st, const double* dts, int64_t first, int64_t count,
                              double* out, cudaStream_t s);
+cudaError_t launch_fused(const StorePtrs& st, const uint8_t* flags, const int32_t* i_list, int ni, int64_t n,
+                         double t, double eps2, int any_flagged, double* part, int* err, int sm_count,
+                         int* grid_out, int* ni_pad_out, cudaStream_t s);
 cudaError_t probe_fp32(int kind, int sm_count, float* scratch, cudaStream_t s, double* lane_ops_per_s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 
