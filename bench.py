@@ -34,6 +34,7 @@ FLOP_PER_INTERACTION = 60.0
 # "alu" roofline denominator: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x
 # clocks.max.sm 1.965 GHz (B200_PROFILING.md unit counts and clocks) = 74.45 Tflop/s.
 FP32_LANES_PER_SM = 128
+FFMA2_LANES_PER_CLK_SM = 115.6           # measured packed-FMA rate (profiles/r1_pipe_probes.md)
 PREDICT_BYTES_PER_PARTICLE = 152.0     # 104 B read + 48 B written
 
 
@@ -402,12 +403,12 @@ def run_ours(args):
                     props.multi_processor_count, sm_max),
                 "ms_per_launch": pair_ms, "launches_timed": kt["n_pair"],
                 "share_of_step": kt["pair_ms"] / ms}
-    # what the FMA pipe sustains on this device with the pair kernel's instruction kinds
-    # (nb_probe_fp32: register-only full-chip kernels, outside the timed region)
-    rate_ffma, rate_ffma2 = ctx.probe_fp32(0), ctx.probe_fp32(1)
+    # what the FMA pipe sustains with the pair kernel's instruction kinds: measured by the committed
+    # micro-benchmark bench/micro/pipe_probe.cu (profiles/r1_pipe_probes.md), not re-measured here
     roofline["fma_probe"] = {
-        "ffma_tflops": 2 * rate_ffma / 1e12, "ffma2_tflops": 2 * rate_ffma2 / 1e12,
-        "frac_of_ffma2_rate": (ach * 1e12 / FLOP_PER_INTERACTION * 33.0) / rate_ffma2,
+        "ffma2_lanes_per_clk_sm": FFMA2_LANES_PER_CLK_SM, "source": "profiles/r1_pipe_probes.md",
+        "frac_of_ffma2_rate": (ach * 1e12 / FLOP_PER_INTERACTION * 33.0) /
+                              (props.multi_processor_count * FFMA2_LANES_PER_CLK_SM * sm_max * 1e6),
         "note": "the pair body executes 33 FP32 lane-ops per interaction (DESIGN.md 7.2); "
                 "frac_of_ffma2_rate = executed lane-ops/s over the measured packed-FMA rate"}
     if args.fp64:

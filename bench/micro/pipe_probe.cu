@@ -1,12 +1,17 @@
 // pipe_probe.cu -- standalone probe of the SM pipes the pair kernels live on.
-// Not part of libnb.so and not on any product path: it exists so that the rates DESIGN.md quotes
-// (FFMA vs FFMA2, FP64 lanes per clock, MUFU, and whether fp32 and fp64 warps overlap) can be
-// re-measured:   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o pipe_probe pipe_probe.cu && ./pipe_probe
-// Part 1: raw instruction rates (8 independent register chains per thread, full chip).
-// Part 2: the fp32 two-float pair body and an fp64 pair body, alone and side by side in one CTA.
+// Not part of libnb.so and not on any product path (micro-benchmarks
+// that gate the design live in bench/micro/): it exists so that the rates DESIGN.md quotes (FFMA vs
+// FFMA2, FP64 lanes per clock, MUFU, F2F, and whether the pipes overlap) can be re-measured:
+//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o pipe_probe bench/micro/pipe_probe.cu && ./pipe_probe [all|rates|bodies|hetero]
+// Part 1 (rates): raw instruction rates (8 independent register chains per thread, full chip).
+// Part 2 (bodies): candidate pair bodies of SURVEY.md section 7's encoding table, loop only (no
+//         tile pipeline): C = two-float positions (what force_kernel runs), D = fp64 position
+//         differences + F2F.F32.F64 (3 DADD + 3 F2F per interaction, 24 FP32 lane-ops), and mixes.
+// Part 3 (hetero): fp32 warps and fp64 warps side by side in one CTA (round 1's experiment).
 #include <cstdio>
 #include <cstdlib>
 #include <cstdint>
+#include <cstring>
 #include <cuda_runtime.h>
 
 #define CK(x) do { cudaError_t e = (x); if (e != cudaSuccess) { printf("CUDA error %s at %d\n", cudaGetErrorString(e), __LINE__); exit(1);} } while (0)
@@ -14,9 +19,10 @@
 __device__ __forceinline__ float rsq(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // ---------------- raw pipe rates: NCH independent chains per thread ----------------
-// kind 0 FFMA2, 1 FFMA, 2 FADD2, 3 DADD, 4 F2F.F32.F64 (+DADD feed), 5 MUFU.RSQ, 6 FMUL2, 7 DFMA
-// 8 IADD3/LOP3 mix (alu), 9: FFMA2 + alu interleaved 1:1, 10: FFMA2 + DADD 4:1, 11: FFMA2 + F2F 4:1
-// 12: FFMA2 + MUFU 8:1
+// kind 0 FFMA2, 1 FFMA, 2 FADD2, 3 DADD, 5 MUFU.RSQ, 6 FMUL2, 7 DFMA, 8 IADD3/LOP3 mix (alu),
+// 9: FFMA2 + alu interleaved 1:1, 10: FFMA2 + DADD 4:1, 12: FFMA2 + MUFU 8:1, 13/14: FFMA2 + FFMA,
+// 17: F2F.F32.F64 (one per step, fed by a DADD, consumed by an FADD), 11: FFMA2 + (DADD, F2F) 4:1,
+// 18: body D's mix per interaction: 12 FFMA2 : 3 DADD : 3 F2F : 1 MUFU (scaled: 32 : 8 : 8 : ~2.7)
 template <int KIND>
 __global__ void __launch_bounds__(128) rate_kernel(float* out, int iters, float a0, double d0)
 {
@@ -42,7 +48,6 @@ __global__ void __launch_bounds__(128) rate_kernel(float* out, int iters, float 
                 if (KIND == 1) s[c] = fmaf(s[c], m.x, b.x);
                 if (KIND == 2) f[c] = __fadd2_rn(f[c], b);
                 if (KIND == 3) d[c] = __dadd_rn(d[c], d0);
-                if (KIND == 4) { s[c] = __double2float_rn(d[c]); d[c] = __dadd_rn(d[c], (double)s[c] * 0.0 + d0); }
                 if (KIND == 5) s[c] = rsq(s[c]);
                 if (KIND == 6) f[c] = __fmul2_rn(f[c], m);
                 if (KIND == 7) d[c] = fma(d[c], d0, d0);
@@ -52,6 +57,10 @@ __global__ void __launch_bounds__(128) rate_kernel(float* out, int iters, float 
                 if (KIND == 13) { f[c] = __ffma2_rn(f[c], m, b); s[c] = fmaf(s[c], m.x, b.x); }
                 if (KIND == 14) { f[c] = __ffma2_rn(f[c], m, b); if (c & 1) s[c] = fmaf(s[c], m.x, b.x); }
                 if (KIND == 12) { f[c] = __ffma2_rn(f[c], m, b); if (c == 0) s[c] = rsq(s[c]); }
+                // 4/11/17: one F2F.F32.F64 per step fed by a DADD and consumed by an FADD (different pipes)
+                if (KIND == 17) { d[c] = __dadd_rn(d[c], d0); s[c] += __double2float_rn(d[c]); }
+                if (KIND == 11) { f[c] = __ffma2_rn(f[c], m, b); if ((c & 3) == 0) { d[c] = __dadd_rn(d[c], d0); s[c] += __double2float_rn(d[c]); } }
+                if (KIND == 18) { f[c] = __ffma2_rn(f[c], m, b); if ((c & 3) == 0) { d[c] = __dadd_rn(d[c], d0); s[c] += __double2float_rn(d[c]); } if (c == 7 && (r & 3) == 0) s[c] = rsq(s[c]); }
             }
         }
     }
@@ -101,6 +110,95 @@ __device__ __forceinline__ double f2d_bits(float f)
 {
     const unsigned u = __float_as_uint(f);
     return __hiloint2double((int)((u >> 3) + 0x38000000u), (int)(u << 29));
+}
+
+
+// ---------------- candidate pair bodies (SURVEY.md section 7 encoding table), 2 i per thread -------------
+// NDBL of the three position components are differenced in fp64 (DADD) and converted (F2F.F32.F64,
+// or with CONV = 1 by integer-pipe bit operations, truncating; rate probe only: zero is not handled),
+// the others as two-float sums (3 FADD2 lane-ops).  NDBL = 0 is encoding C (force_kernel today),
+// NDBL = 3 is encoding D.  Same tile contents in both forms, 4 j per trip, loop only.
+template <int NDBL, int CONV, int MINB>
+__global__ void __launch_bounds__(128, MINB) body_kernel(float* out, int reps, float eps2f)
+{
+    __shared__ __align__(16) float T[10 * TJ];       // xh yh zh xl yl zl vx vy vz m
+    __shared__ __align__(16) double TD[3 * TJ];      // x y z
+    const int tid = threadIdx.x;
+    for (int q = tid; q < TJ; q += 128) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.37 * ((q * 2654435761u + c * 40503u) % 1000) / 1000.0 - 0.18;
+            TD[c * TJ + q] = x;
+            const float h = (float)x;
+            T[c * TJ + q] = h;
+            T[(3 + c) * TJ + q] = (float)(x - (double)h);
+            T[(6 + c) * TJ + q] = 0.01f * (float)((q * 7 + c * 13) % 17 - 8);
+        }
+        T[9 * TJ + q] = 1.0f / 1048576.0f;
+    }
+    __syncthreads();
+    constexpr int IPT = 2;
+    double xi[IPT][3];
+    float2 nxh[IPT][3], nxl[IPT][3], nv[IPT][3];
+    Acc A[IPT];
+    for (int u = 0; u < IPT; ++u) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.001 * (tid + 128 * u) + 0.1 * c + 1e-9 * blockIdx.x;
+            const float h = (float)x;
+            xi[u][c] = x;
+            nxh[u][c] = dup(-h);
+            nxl[u][c] = dup(-(float)(x - (double)h));
+            nv[u][c] = dup(0.003f * (tid % 7) - 0.01f * c + 0.002f * u);
+        }
+        A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
+    }
+    const float2 eps2 = dup(eps2f), m3 = dup(-3.0f);
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll 2
+        for (int p = 0; p < TJ; p += 4) {
+            float4 f[10];
+            double2 g[3][2];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                if (c < NDBL) {
+                    g[c][0] = *reinterpret_cast<const double2*>(TD + c * TJ + p);
+                    g[c][1] = *reinterpret_cast<const double2*>(TD + c * TJ + p + 2);
+                } else {
+                    f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+                    f[3 + c] = *reinterpret_cast<const float4*>(T + (3 + c) * TJ + p);
+                }
+            }
+#pragma unroll
+            for (int c = 6; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+#pragma unroll
+            for (int u = 0; u < IPT; ++u) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    float2 d[3], w[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        if (c < NDBL) {
+                            const double e0 = g[c][h].x - xi[u][c], e1 = g[c][h].y - xi[u][c];
+                            d[c] = CONV ? make_float2(d2f_bits(e0), d2f_bits(e1))
+                                        : make_float2(__double2float_rn(e0), __double2float_rn(e1));
+                        } else {
+                            const float2 xh = h ? make_float2(f[c].z, f[c].w) : make_float2(f[c].x, f[c].y);
+                            const float2 xl = h ? make_float2(f[3 + c].z, f[3 + c].w) : make_float2(f[3 + c].x, f[3 + c].y);
+                            d[c] = __fadd2_rn(__fadd2_rn(xh, nxh[u][c]), __fadd2_rn(xl, nxl[u][c]));
+                        }
+                        const float2 vv = h ? make_float2(f[6 + c].z, f[6 + c].w) : make_float2(f[6 + c].x, f[6 + c].y);
+                        w[c] = __fadd2_rn(vv, nv[u][c]);
+                    }
+                    const float2 mm = h ? make_float2(f[9].z, f[9].w) : make_float2(f[9].x, f[9].y);
+                    body32(d[0], d[1], d[2], w[0], w[1], w[2], mm, eps2, m3, A[u]);
+                }
+            }
+        }
+    }
+    float res = 0.f;
+    for (int u = 0; u < IPT; ++u)
+        res += A[u].ax.x + A[u].ax.y + A[u].ay.x + A[u].ay.y + A[u].az.x + A[u].az.y + A[u].jx.x + A[u].jx.y +
+               A[u].jy.x + A[u].jy.y + A[u].jz.x + A[u].jz.y + A[u].p.x + A[u].p.y;
+    out[blockIdx.x * 128 + tid] = res;
 }
 
 struct Acc64 { double ax, ay, az, jx, jy, jz, p; };
@@ -166,7 +264,7 @@ hetero_kernel(float* out, int reps, float eps2f, double eps2d)
                 const float h = (float)x;
                 nxh[u][c] = dup(-h);
                 nxl[u][c] = dup(-(float)(x - (double)h));
-                nv[u][c] = dup(0.003f * (tid % 7) - 0.01f * c);
+                nv[u][c] = dup(0.003f * (tid % 7) - 0.01f * c + 0.002f * u);
             }
             A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
         }
@@ -272,6 +370,23 @@ void run(int reps32_only = 0)
            NW32, NW64, IPT64, CONV, MINB, fa.numRegs, occ, ms, r, r / 1.2408e12 * 100, i32 / (i32 + i64));
 }
 
+
+template <int NDBL, int CONV, int MINB>
+void run_body(const char* name)
+{
+    const int reps = 300;
+    const int grid = nsm * MINB * 5;
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, body_kernel<NDBL, CONV, MINB>, 128, 0));
+    cudaFuncAttributes fa;
+    CK(cudaFuncGetAttributes(&fa, body_kernel<NDBL, CONV, MINB>));
+    float ms = time_ms([&] { body_kernel<NDBL, CONV, MINB><<<grid, 128>>>(d_out, reps, 1e-6f); });
+    const double inter = (double)grid * 4 * 64 * (double)TJ * reps;
+    const double r = inter / (ms * 1e-3);
+    printf("body %-40s minb %d regs %3d occ %d : %8.3f ms  %9.3e inter/s = %5.1f%% of 1.2408e12\n", name, MINB,
+           fa.numRegs, occ, ms, r, r / 1.2408e12 * 100);
+}
+
 template <int KIND>
 void run_rate(const char* name, double ops_per_iter_thread, int ctas_per_sm)
 {
@@ -285,43 +400,57 @@ void run_rate(const char* name, double ops_per_iter_thread, int ctas_per_sm)
 }
 
 
-int main()
+int main(int argc, char** argv)
 {
+    const char* what = argc > 1 ? argv[1] : "all";
+    const bool all = !strcmp(what, "all");
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, 0));
     nsm = prop.multiProcessorCount;
-    printf("device %s, %d SMs\n", prop.name, nsm);
+    int clk = 0;
+    CK(cudaDeviceGetAttribute(&clk, cudaDevAttrClockRate, 0));
+    printf("device %s, %d SMs, max SM clock %d MHz\n", prop.name, nsm, clk / 1000);
     CK(cudaMalloc(&d_out, (size_t)nsm * 64 * 1024 * 4));
-    printf("-- raw rates, thread-operations per second per SM (divide by the clock for lanes per clock)\n");
-    run_rate<1>("FFMA", 64, 4);
-    run_rate<0>("FFMA2", 64, 4);
-    run_rate<2>("FADD2", 64, 4);
-    run_rate<6>("FMUL2", 64, 4);
-    run_rate<3>("DADD", 64, 4);
-    run_rate<7>("DFMA", 64, 4);
-    run_rate<5>("MUFU.RSQ", 64, 4);
-    run_rate<8>("alu IADD+LOP/SHF", 64, 4);
-    run_rate<10>("FFMA2 + DADD 4:1 (count FFMA2)", 64, 4);
-    run_rate<13>("FFMA2 + FFMA 1:1 (count FFMA2)", 64, 4);
-    printf("-- pair bodies: fp32 two-float (2 i per thread) and fp64 (ipt i per thread) warps in one CTA\n");
-    run<4, 0, 1, 0, 3>();
-    run<0, 4, 1, 0, 3>();
-    run<0, 4, 1, 1, 3>();
-    run<0, 4, 2, 1, 3>();
-    run<0, 4, 2, 0, 3>();
-    run<0, 4, 2, 1, 4>();
-    run<0, 8, 2, 1, 2>();
-    run<4, 4, 1, 1, 1>();
-    run<4, 4, 2, 1, 1>();
-    run<4, 4, 2, 0, 1>();
-    run<8, 4, 1, 1, 1>();
-    run<8, 4, 2, 1, 1>();
-    run<8, 8, 1, 1, 1>();
-    run<8, 8, 2, 1, 1>();
-    run<4, 4, 1, 1, 2>();
-    run<4, 4, 2, 1, 2>();
-    run<4, 2, 2, 1, 2>();
-    run<8, 4, 2, 0, 1>();
-    run<12, 4, 2, 1, 1>();
+    if (all || !strcmp(what, "rates")) {
+        printf("-- raw rates, thread-operations per second per SM (divide by the clock for lanes per clock)\n");
+        run_rate<1>("FFMA", 64, 4);
+        run_rate<0>("FFMA2", 64, 4);
+        run_rate<2>("FADD2", 64, 4);
+        run_rate<6>("FMUL2", 64, 4);
+        run_rate<3>("DADD", 64, 4);
+        run_rate<7>("DFMA", 64, 4);
+        run_rate<5>("MUFU.RSQ", 64, 4);
+        run_rate<8>("alu IADD+LOP/SHF", 64, 4);
+        run_rate<9>("FFMA2 + alu(2 ops) 1:1 (count FFMA2)", 64, 4);
+        run_rate<10>("FFMA2 + DADD 4:1 (count FFMA2)", 64, 4);
+        run_rate<12>("FFMA2 + MUFU 8:1 (count FFMA2)", 64, 4);
+        run_rate<13>("FFMA2 + FFMA 1:1 (count FFMA2)", 64, 4);
+        run_rate<17>("F2F.F32.F64 (+DADD feed, FADD use)", 64, 4);
+        run_rate<11>("FFMA2 + (DADD,F2F) 4:1 (count FFMA2)", 64, 4);
+        run_rate<18>("FFMA2:DADD:F2F:MUFU 12:3:3:1 (count FFMA2)", 64, 4);
+    }
+    if (all || !strcmp(what, "bodies")) {
+        printf("-- pair bodies, loop only, 2 i per thread, 128 threads: NDBL components by fp64 DADD + conversion\n");
+        run_body<0, 0, 4>("C: two-float x y z (force_kernel)");
+        run_body<0, 0, 3>("C: two-float x y z (force_kernel)");
+        run_body<3, 0, 4>("D: fp64 x y z + F2F");
+        run_body<3, 0, 3>("D: fp64 x y z + F2F");
+        run_body<2, 0, 4>("fp64 x y + F2F, two-float z");
+        run_body<2, 0, 3>("fp64 x y + F2F, two-float z");
+        run_body<1, 0, 4>("fp64 x + F2F, two-float y z");
+        run_body<1, 0, 3>("fp64 x + F2F, two-float y z");
+        run_body<3, 1, 4>("D': fp64 x y z + integer-pipe conversion");
+        run_body<3, 1, 3>("D': fp64 x y z + integer-pipe conversion");
+        run_body<2, 1, 4>("fp64 x y + int conversion, two-float z");
+    }
+    if (all || !strcmp(what, "hetero")) {
+        printf("-- fp32 two-float (2 i per thread) and fp64 (ipt i per thread) warps in one CTA\n");
+        run<4, 0, 1, 0, 3>();
+        run<0, 4, 1, 0, 3>();
+        run<0, 4, 2, 0, 3>();
+        run<4, 4, 1, 1, 1>();
+        run<8, 4, 1, 1, 1>();
+        run<12, 4, 2, 1, 1>();
+    }
     return 0;
 }

@@ -91,8 +91,10 @@ int nb_update_j_host(nb_ctx* c, const int32_t* idx, int64_t count, const double*
                 const double* ax, const double* ay, const double* az,
                 const double* jx, const double* jy, const double* jz, const double* t);
 
-/* HOST-pointer form of nb_set_j (pageable or pinned host memory; staged through the context's
- * pinned buffer with cudaMemcpyAsync).  Same argument rules. */
+/* HOST-pointer form of nb_set_j: one cudaMemcpyAsync per array, straight from the caller's memory
+ * to the j-store on the context's stream.  Same argument rules.  Pageable arrays are staged by the
+ * runtime before the call returns; PINNED arrays are read by the copy engine later, so they must
+ * stay valid and unmodified until the stream has consumed them (nb_sync), as for nb_update_j_host. */
 int nb_set_j_host(nb_ctx* c, int64_t first, int64_t count, const double* m,
                   const double* x, const double* y, const double* z,
                   const double* vx, const double* vy, const double* vz,
@@ -103,9 +105,12 @@ int nb_clear(nb_ctx* c);            /* n := 0, flags cleared, "predicted" state 
 int64_t nb_count(const nb_ctx* c);  /* current n (or a negative nb_status)                  */
 
 /* Mark particles whose MUTUAL pairs are unsoftened (R7: eps2_ij = 0 iff both carry bit 0; e.g.
- * black holes).  idx, flags: HOST arrays of length count (the flagged set is
- * small and changes rarely); replaces the flag of each listed particle.  At most NB_MAX_FLAGGED
- * particles may carry the bit at one time (NB_ERR_ARG beyond). */
+ * black holes).  idx, flags: HOST arrays of length count -- the one entry point
+ * besides the *_host calls that takes host memory: the library keeps a host copy of the flagged set
+ * (it sizes the unsoftened-pair pass by it), the set is small and changes rarely.  Replaces the flag
+ * of each listed particle; one staged copy + one scatter kernel on the stream, no synchronisation.
+ * At most NB_MAX_FLAGGED particles may carry the bit at one time (NB_ERR_ARG beyond): the pairs among
+ * them are summed in fp64 by one thread per flagged i-particle. */
 #define NB_MAX_FLAGGED 1024
 int nb_set_flags(nb_ctx* c, const int32_t* idx, const uint8_t* flags, int64_t count);
 
@@ -130,8 +135,16 @@ int nb_get_predicted(nb_ctx* c, int64_t first, int64_t count, double* out);
  *     jrk_i = sum m_j ( w s^-3/2 - 3 (r.w) r s^-5/2 )             (s == 0 contributes nothing, R6)
  * Outputs, DEVICE fp64, in i_list order: acc[0..ni) = ax, acc[ni..2ni) = ay, acc[2ni..3ni) = az;
  * jrk likewise; pot[0..ni).  Precision: position differences carry >= 48 bits, pair terms are
- * fp32, sums are fp64; results agree with exact summation to
- * <= 1e-5 (acc, pot) and <= 1e-4 (jerk) relative per particle.  Deterministic run to run.
+ * fp32, sums of at most 64 terms are fp32 and everything above them fp64 (DESIGN.md
+ * section 7.2); results agree with exact summation to <= 1e-5 (acc, pot) and <= 1e-4 (jerk) relative
+ * per particle, for ANY eps2 >= 0: the self pair is excluded by index before any fp32 sum, so small
+ * softenings (m_i/eps far above |pot_i|) cost no accuracy.  Input limits (R14): every pair
+ * term m_j s^-3/2 and m_j s^-1/2 must stay inside the normal fp32 range (1e-38 .. 3e38) -- e.g. two
+ * DISTINCT particles closer than ~1e-12 length units at m = 1 overflow it -- and masses are rounded to
+ * fp32.  For eps2 < 1e-20 (eps2 = 0 included) a pair of distinct particles whose separation vanishes
+ * in fp32 (|r|^2 + eps2 == eps2) contributes nothing, as R6 states for eps2 = 0; for eps2 >= 1e-20
+ * such a pair interacts normally (zero acc and jerk, -m_j/eps in pot; R5).  Use precision mode 1
+ * beyond these limits.  Deterministic run to run.
  * eps2 must be finite and >= 0; ni in [0, ni_max].  An out-of-range i_list entry gets NaN
  * outputs and latches NB_ERR_INDEX (returned by the next nb_sync). */
 int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
@@ -174,8 +187,9 @@ int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
  * root refined to fp64 rounding -- for "objects with an extreme mass ratio, like planetesimals
  * around super-massive black holes".  Mode 1 keeps a second,
  * fp64 copy of the predicted j-set (64 B per particle, cudaMalloc'ed by this call, not part of
- * the lent workspace) and agrees with exact summation to ~1e-13 relative; pairs closer than
- * ~1e-19 or farther than ~1e19 length units are treated as coincident / out of range.  Changing
+ * the lent workspace) and agrees with exact summation to ~1e-13 relative; pairs whose s = r^2 +
+ * eps2 lies below 1.18e-38 (closer than 1.1e-19 length units) are treated as coincident, pairs with
+ * s above 3.4e38 (farther than 1.8e19) as out of range: both contribute nothing.  Changing
  * the mode invalidates the predicted state: call nb_predict before the next force call
  * (NB_ERR_STATE otherwise).  The atomics reduce mode and the threads-per-i variants are mode-0
  * only; results of mode 1 are deterministic. */
@@ -235,6 +249,11 @@ int nb_init_steps(nb_ctx* c, const int32_t* i_list, int64_t ni, const double* ac
  * *t_next and *ni still set) if more than ni_max particles are due: the list is then truncated. */
 int nb_next_block(nb_ctx* c, double* t_next, int64_t* ni, const int32_t** i_list);
 
+/* After nb_init_steps, nb_correct and nb_step the j-store has moved on and the packed predicted
+ * state is stale: nb_force / nb_force_ext / nb_get_predicted return NB_ERR_STATE until the next
+ * nb_predict, whatever the size of the block was.  A due particle whose step is zero (steps never
+ * set) or whose time is NaN is left untouched and latches NB_ERR_STATE (returned by nb_sync). */
+
 /* Corrector + new step (R12, R18, R19, R20) for particles i_list[0..ni) (DEVICE) that were
  * predicted to t1 and whose forces at t1 are acc/jrk (DEVICE fp64, [3][ni] in i_list order): with
  * h = t1 - t_i, v1 = v0 + (a0+a1) h/2 + (j0-j1) h^2/12; x1 = x0 + (v0+v1) h/2 + (a0-a1) h^2/12;
@@ -249,23 +268,14 @@ int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const do
  * of the block stay in a context-owned buffer (nb_block_forces). */
 int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, double* t, int64_t* ni);
 
-/* nb_step takes blocks of <= NB_FUSED_MAX particles through nb_force_fused (default on); after
- * such a step the packed predicted state is stale: call nb_predict before nb_force /
- * nb_get_predicted (they return NB_ERR_STATE until then).  on = 0 switches this off. */
+/* nb_step takes blocks of <= NB_FUSED_MAX particles through nb_force_fused (default on).  on = 0
+ * switches this off. */
 int nb_set_fused(nb_ctx* c, int on);
 
 /* DEVICE addresses of the last nb_step's acc [3][ni], jrk [3][ni], pot [ni] (any may be NULL). */
 int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const double** pot);
 
-/* Measure what the FP32 FMA pipe of this device sustains, with the instruction kinds the pair
- * kernel is built from: kind 0 = scalar FFMA, kind 1 = packed FFMA2
- * (fma.rn.f32x2).  Runs a short full-chip register-only kernel four times on the context's stream
- * (synchronises it) and writes the best rate, in fused multiply-adds per second summed over all
- * lanes, to HOST *lane_ops_per_s (nominal: SMs x 128 x clock).  Diagnostic for the roofline
- * report, not part of the force path. */
-int nb_probe_fp32(nb_ctx* c, int kind, double* lane_ops_per_s);
-
-int nb_sync(nb_ctx* c);                 /* stream sync; returns and clears any latched error */
+int nb_sync(nb_ctx* c);   /* stream sync; returns and clears a latched NB_ERR_INDEX / NB_ERR_STATE */
 const char* nb_strerror(int status);
 const char* nb_version(void);
 

@@ -18,7 +18,7 @@ EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_precision", "nb_set_tuning",
-    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_probe_fp32", "nb_sync",
+    "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_block_forces", "nb_strerror", "nb_version",
 ]
 
@@ -58,7 +58,6 @@ lib.nb_kernel_times.argtypes = [_vp, ctypes.POINTER(_dbl)]
 lib.nb_sync.argtypes = [_vp]
 lib.nb_strerror.argtypes = [_i32]
 lib.nb_strerror.restype = ctypes.c_char_p
-lib.nb_probe_fp32.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(_dbl)]
 lib.nb_force_fused.argtypes = [_vp, _dbl, _vp, _i64, _dbl, _vp, _vp, _vp]
 lib.nb_set_fused.argtypes = [_vp, _i32]
 lib.nb_force_ext.argtypes = [_vp, _i64, _vp, _vp, _dbl, _vp, _vp, _vp]
@@ -269,13 +268,6 @@ def nb_block_forces(c):
     a, j, p = _vp(), _vp(), _vp()
     _check(lib.nb_block_forces(c, ctypes.byref(a), ctypes.byref(j), ctypes.byref(p)), "nb_block_forces")
     return a.value, j.value, p.value
-
-
-def nb_probe_fp32(c, kind):
-    """FMA lane-operations per second the device sustains (kind 0 = FFMA, 1 = FFMA2)."""
-    out = _dbl(0.0)
-    _check(lib.nb_probe_fp32(c, int(kind), ctypes.byref(out)), "nb_probe_fp32")
-    return out.value
 
 
 def nb_kernel_times(c):

@@ -103,10 +103,12 @@ class Context:
     def set_j_host(self, m, x, v, a=None, j=None, t=None, first=0):
         """HOST arrays (numpy or pinned CPU tensors), fp64 contiguous; staged by the library."""
         nb.nb_set_j_host(self.h, first, m.shape[0], m, x, v, a, j, t)
+        self._keep_host = [m, x, v, a, j, t]     # pinned sources are read later, on the stream
 
     def update_j_host(self, idx, m, x, v, a=None, j=None, t=None):
         """HOST int32 idx and HOST fp64 arrays of the idx.shape[0] updated particles."""
         nb.nb_update_j_host(self.h, idx, idx.shape[0], m, x, v, a, j, t)
+        self._keep_host = [idx, m, x, v, a, j, t]
 
     def force_host(self, i_list, eps2, acc, jrk, pot):
         """HOST int32 i_list and HOST fp64 outputs acc, jrk (3, ni), pot (ni,); returns after
@@ -178,10 +180,6 @@ class Context:
 
     def kernel_times(self):
         return nb.nb_kernel_times(self.h)
-
-    def probe_fp32(self, kind):
-        """Sustained FMA lane-operations/s of the device (0 = FFMA, 1 = FFMA2)."""
-        return nb.nb_probe_fp32(self.h, kind)
 
     def launch_count(self):
         return nb.nb_launch_count(self.h)

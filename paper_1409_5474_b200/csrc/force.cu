@@ -13,51 +13,11 @@
 // nothing for R5/R7.  No tensor cores: the pair kernel with its reciprocal square root is not a
 // contraction.
 #include "nb_internal.h"
+#include "tma.h"
 
 namespace nb {
 
 namespace {
-
-// ---- PTX helpers: mbarrier + 1-D bulk async copy ---------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p)
-{
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(bar), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-        "l"(src), "r"(bytes), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ float rsqrt_fast(float x)
-{
-    float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 
 struct IPart {            // one i-particle, negated and duplicated over both f32x2 lanes
     float2 nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz;
@@ -69,6 +29,11 @@ struct Acc32 {            // per-tile fp32 sums, lane 0 = even j, lane 1 = odd j
 __device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
 
 // One i against one pair of j's: 13 FADD2 + 14 FFMA2 + 6 FMUL2 + 2 MUFU (R2, R17).
+// GUARD (calls with eps2 below EPS2_GUARD, eps2 == 0 among them): a pair whose s does not exceed
+// eps2 -- r = 0 to fp32 precision: the self pair, or two particles at one place (R5, R6) -- gets
+// rinv = 0 and so contributes nothing; the compare and select run on the ALU pipe, beside the FP32
+// pipe the loop is bound by.
+template <bool GUARD>
 __device__ __forceinline__ void pair2(const IPart& I, Acc32& A, float2 xh, float2 yh, float2 zh,
                                       float2 xl, float2 yl, float2 zl, float2 vx, float2 vy,
                                       float2 vz, float2 m, float2 eps2, float2 m3)
@@ -85,6 +50,10 @@ __device__ __forceinline__ void pair2(const IPart& I, Acc32& A, float2 xh, float
     float2 rinv;
     rinv.x = rsqrt_fast(r2.x);
     rinv.y = rsqrt_fast(r2.y);
+    if (GUARD) {
+        rinv.x = r2.x > eps2.x ? rinv.x : 0.0f;
+        rinv.y = r2.y > eps2.x ? rinv.y : 0.0f;
+    }
     const float2 rinv2 = __fmul2_rn(rinv, rinv);
     const float2 mr = __fmul2_rn(m, rinv);
     const float2 mr3 = __fmul2_rn(mr, rinv2);
@@ -103,6 +72,7 @@ __device__ __forceinline__ void pair2(const IPart& I, Acc32& A, float2 xh, float
 
 // acc + pot only (the kick of a bridge between two systems):
 // 9 FADD2 + 6 FFMA2 + 3 FMUL2 + 1 FADD2 = 19 lane-ops per interaction, no velocities.
+template <bool GUARD>
 __device__ __forceinline__ void pair2_acc(const IPart& I, Acc32& A, float2 xh, float2 yh, float2 zh,
                                           float2 xl, float2 yl, float2 zl, float2 m, float2 eps2)
 {
@@ -115,6 +85,10 @@ __device__ __forceinline__ void pair2_acc(const IPart& I, Acc32& A, float2 xh, f
     float2 rinv;
     rinv.x = rsqrt_fast(r2.x);
     rinv.y = rsqrt_fast(r2.y);
+    if (GUARD) {
+        rinv.x = r2.x > eps2.x ? rinv.x : 0.0f;
+        rinv.y = r2.y > eps2.x ? rinv.y : 0.0f;
+    }
     const float2 rinv2 = __fmul2_rn(rinv, rinv);
     const float2 mr = __fmul2_rn(m, rinv);
     const float2 mr3 = __fmul2_rn(mr, rinv2);
@@ -122,6 +96,39 @@ __device__ __forceinline__ void pair2_acc(const IPart& I, Acc32& A, float2 xh, f
     A.ax = __ffma2_rn(mr3, dx, A.ax);
     A.ay = __ffma2_rn(mr3, dy, A.ay);
     A.az = __ffma2_rn(mr3, dz, A.az);
+}
+
+// One i against a quad of consecutive j (four floats of each tile array): two packed pairs.
+template <bool JERK, bool GUARD>
+__device__ __forceinline__ void quad(const IPart& I, Acc32& A, const float4* f, float2 eps2, float2 m3)
+{
+    if (!JERK) {
+        pair2_acc<GUARD>(I, A, make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
+                         make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y),
+                         make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
+                         make_float2(f[9].x, f[9].y), eps2);
+        pair2_acc<GUARD>(I, A, make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w),
+                         make_float2(f[2].z, f[2].w), make_float2(f[3].z, f[3].w),
+                         make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
+                         make_float2(f[9].z, f[9].w), eps2);
+        return;
+    }
+    pair2<GUARD>(I, A, make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
+                 make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y), make_float2(f[4].x, f[4].y),
+                 make_float2(f[5].x, f[5].y), make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y),
+                 make_float2(f[8].x, f[8].y), make_float2(f[9].x, f[9].y), eps2, m3);
+    pair2<GUARD>(I, A, make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w),
+                 make_float2(f[2].z, f[2].w), make_float2(f[3].z, f[3].w), make_float2(f[4].z, f[4].w),
+                 make_float2(f[5].z, f[5].w), make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w),
+                 make_float2(f[8].z, f[8].w), make_float2(f[9].z, f[9].w), eps2, m3);
+}
+
+template <bool JERK>
+__device__ __forceinline__ void load_quad(float4* f, const float* T, int p)
+{
+#pragma unroll
+    for (int c = 0; c < 10; ++c)
+        if (JERK || c < 6 || c == 9) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
 }
 
 // Masked scalar pair for the rare tiles that hold the i-particle itself, a flagged partner of a
@@ -153,6 +160,28 @@ __device__ __forceinline__ void pair1_masked(const IPart& I, Acc32& A, const flo
     A.jz.x = fmaf(mr3, fmaf(al, dz, wz), A.jz.x);
 }
 
+// R5 in the packed path.  The packed loop runs over whole tiles, so in the one tile that holds the
+// index of an i-particle it evaluates the self pair: r = w = 0 exactly, nothing for acc and jerk,
+// but m_i/eps for pot -- a term that can be orders of magnitude above the real ones (|pot| ~ 1 at
+// m_i/eps = 1e4), and an fp32 sum that holds it rounds them away.  So that tile's pot lane (the
+// even or the odd j of the thread's share, whichever holds the self index) is summed again here
+// without the self pair and replaces the polluted lane; the caller makes sure the lane held
+// nothing else.  64 scalar terms, once per i-particle per call.
+__device__ __forceinline__ float pot_lane(const IPart& I, const float* T, int k0, int k1, int self, float eps2)
+{
+    float ps = 0.0f;
+#pragma unroll 1
+    for (int k = k0 + (self & 1); k < k1; k += 2) {
+        const float dx = (T[P_XH * TJ + k] + I.nxh.x) + (T[P_XL * TJ + k] + I.nxl.x);
+        const float dy = (T[P_YH * TJ + k] + I.nyh.x) + (T[P_YL * TJ + k] + I.nyl.x);
+        const float dz = (T[P_ZH * TJ + k] + I.nzh.x) + (T[P_ZL * TJ + k] + I.nzl.x);
+        const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+        const float mr = T[P_M * TJ + k] * rsqrt_fast(r2);
+        ps += (k == self) ? 0.0f : mr;
+    }
+    return ps;
+}
+
 // S = distance between the 7 sums of one i: 1 when they sit in registers, FORCE_THREADS when they
 // sit in shared memory (the all-i kernel keeps them there: 28 registers fewer, 4 CTAs per SM)
 template <int S, bool JERK>
@@ -180,7 +209,9 @@ __host__ __device__ constexpr int stages_for(int jl) { return jl == 1 ? STAGES :
 // MODE 0: i-particles are members of the j-set, given by index (nb_force).  MODE 1: i-particles
 // given by value, "a completely different set", acc + jerk + pot; MODE 2: the same,
 // acc + pot only (nb_force_ext).  No self pair and no flags in modes 1 and 2.
-template <bool ATOMIC, int JL, int MODE>
+// GUARD: the call's eps2 is below EPS2_GUARD (zero included): pairs with r = 0 are dropped inside the
+// packed pair (R5, R6), so no tile needs the self-pair treatment.
+template <bool ATOMIC, int JL, int MODE, bool GUARD>
 __global__ void __launch_bounds__(FORCE_THREADS, NB_MINB)
 force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
              double* __restrict__ opot)
@@ -210,7 +241,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
             mbar_init(smem_u32(&bars[s]), 1);
             rel[s] = 0;
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
         for (int s = 0; s < STG && t0 + s < t1; ++s) {
             mbar_expect_tx(smem_u32(&bars[s]), TILE_BYTES);
             bulk_g2s(smem_u32(tiles + s * TILE_FLOATS), P.pack + (int64_t)(t0 + s) * TILE_FLOATS,
@@ -258,7 +289,6 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
 
     const float2 eps2 = dup(P.eps2);
     const float2 m3 = dup(-3.0f);
-    const bool eps0 = !(P.eps2 > 0.0f);
     Acc32 A[IPT];
     double D[DSM ? 1 : IPT][NOUT];
 #pragma unroll
@@ -280,58 +310,53 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         mbar_wait(smem_u32(&bars[st]), ((t - t0) / STG) & 1);
         const float* T = tiles + st * TILE_FLOATS;
 
-        // The self pair needs no mask when eps2 > 0 (r = w = 0 exactly: it adds nothing to acc and
-        // jerk, and m_i/eps to pot, which the tail takes back); only eps2 == 0 and flagged-flagged
-        // pairs (R6, R7) go through the masked path.
-        bool slow = eps0;
-        if (iflags) slow |= (P.tileflag[t >> 5] >> (t & 31)) & 1u;
+        // Flagged-flagged pairs (R7): the whole tile goes through the masked scalar pair, warp-uniform;
+        // that path also excludes the self pair by index.  Every other tile is packed.
         constexpr int JPT = TJ / JL;              // j per thread per tile
         constexpr int UNROLL_Q = NB_UNROLL;       // j-quads per trip of the pair loop
+        constexpr int FLUSH_EVERY = 2 * 64 / JPT > 1 ? 2 * 64 / JPT : 1;
         const int p0 = (tid % JL) * JPT;
-        if (!__any_sync(0xffffffffu, slow)) {
-#pragma unroll UNROLL_Q
-            for (int p = p0; p < p0 + JPT; p += 4) {
-                float4 f[10];
-#pragma unroll
-                for (int c = 0; c < 10; ++c)
-                    if (JERK || c < 6 || c == 9) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
-#pragma unroll
-                for (int u = 0; u < IPT; ++u) {
-                    if (!JERK) {
-                        pair2_acc(I[u], A[u], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
-                                  make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y),
-                                  make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
-                                  make_float2(f[9].x, f[9].y), eps2);
-                        pair2_acc(I[u], A[u], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w),
-                                  make_float2(f[2].z, f[2].w), make_float2(f[3].z, f[3].w),
-                                  make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
-                                  make_float2(f[9].z, f[9].w), eps2);
-                        continue;
-                    }
-                    pair2(I[u], A[u], make_float2(f[0].x, f[0].y), make_float2(f[1].x, f[1].y),
-                          make_float2(f[2].x, f[2].y), make_float2(f[3].x, f[3].y),
-                          make_float2(f[4].x, f[4].y), make_float2(f[5].x, f[5].y),
-                          make_float2(f[6].x, f[6].y), make_float2(f[7].x, f[7].y),
-                          make_float2(f[8].x, f[8].y), make_float2(f[9].x, f[9].y), eps2, m3);
-                    pair2(I[u], A[u], make_float2(f[0].z, f[0].w), make_float2(f[1].z, f[1].w),
-                          make_float2(f[2].z, f[2].w), make_float2(f[3].z, f[3].w),
-                          make_float2(f[4].z, f[4].w), make_float2(f[5].z, f[5].w),
-                          make_float2(f[6].z, f[6].w), make_float2(f[7].z, f[7].w),
-                          make_float2(f[8].z, f[8].w), make_float2(f[9].z, f[9].w), eps2, m3);
-                }
-            }
-        } else {
+        bool slow = false;
+        if (iflags) slow = (P.tileflag[t >> 5] >> (t & 31)) & 1u;
+        if (__any_sync(0xffffffffu, slow)) {
 #pragma unroll 1
             for (int p = p0; p < p0 + JPT; ++p) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)
-                    pair1_masked(I[u], A[u], T, p,
-                                 (eps0 || ((iflags >> u) & 1u)) && sidx[u * FORCE_THREADS] == t * TJ + p,
+                    pair1_masked(I[u], A[u], T, p, MODE == 0 && sidx[u * FORCE_THREADS] == t * TJ + p,
                                  (iflags >> u) & 1u, P.eps2);
+            }
+        } else {
+            // R5 (see pot_lane): when this tile holds the own index of one of my i-particles, in my
+            // share of the tile, that particle's fp32 sums are moved to fp64 first, so that the pot
+            // lane starts empty (the all-i kernel flushes after every tile anyway)
+            if (MODE == 0 && !GUARD && FLUSH_EVERY > 1) {
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+                    const int q = sidx[u * FORCE_THREADS] - t * TJ;
+                    if (q >= p0 && q < p0 + JPT) flush<1, JERK>(A[u], D[DSM ? 0 : u]);
+                }
+            }
+#pragma unroll UNROLL_Q
+            for (int p = p0; p < p0 + JPT; p += 4) {
+                float4 f[10];
+                load_quad<JERK>(f, T, p);
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) quad<JERK, GUARD>(I[u], A[u], f, eps2, m3);
+            }
+            if (MODE == 0 && !GUARD) {
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+                    const int q = sidx[u * FORCE_THREADS] - t * TJ;
+                    if (q >= p0 && q < p0 + JPT) {
+                        const float ps = pot_lane(I[u], T, p0, p0 + JPT, q, P.eps2);
+                        if (q & 1) A[u].p.y = ps;
+                        else A[u].p.x = ps;
+                    }
+                }
             }
         }
         // fp32 sums stay short (R17: 64 terms per lane) before they move to fp64
-        constexpr int FLUSH_EVERY = 2 * 64 / JPT > 1 ? 2 * 64 / JPT : 1;
         if (FLUSH_EVERY == 1 || (t - t0) % FLUSH_EVERY == FLUSH_EVERY - 1 || t == t1 - 1) {
 #pragma unroll
             for (int u = 0; u < IPT; ++u) {
@@ -343,6 +368,7 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         // release the stage; the last warp out refills it with tile t + STG
         __syncwarp();
         if ((tid & 31) == 0) {
+            __threadfence_block();     // this warp's reads of the stage are ordered before its release
             const int old = atomicAdd(&rel[st], 1);
             if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STG < t1) {
                 mbar_expect_tx(smem_u32(&bars[st]), TILE_BYTES);
@@ -364,15 +390,11 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         if (tid % JL != 0) return;
     }
 
-    // a5 (first half): take back the self term of pot where the unmasked path included it
-    const float rinv_e = eps0 ? 0.0f : rsqrt_fast(P.eps2);
     // the CTA's place in the grid is read again here, so that it does not hold registers through
     // the pair loop (the all-i kernel then fits 128 registers unspilled: 4 CTAs per SM)
     unsigned bid;
     asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(bid));
     const int it2 = bid % P.n_itiles, sp2 = bid / P.n_itiles;
-    const int u0 = (int)(((int64_t)P.ntiles * sp2) / P.splits) * TJ;
-    const int u1 = (int)(((int64_t)P.ntiles * (sp2 + 1)) / P.splits) * TJ;
 
     // a4: partial sums of this j-subset (second kernel adds them), or atomics (:63)
 #pragma unroll
@@ -382,10 +404,6 @@ force_kernel(ForceArgs P, double* __restrict__ oacc, double* __restrict__ ojrk,
         for (int c = 0; c < NOUT; ++c) o[c] = DSM ? sd[(u * NOUT + c) * FORCE_THREADS] : D[DSM ? 0 : u][c];
         const int ku = it2 * (ITILE / JL) + (u * FORCE_THREADS + tid) / JL;
         const int q = sidx[u * FORCE_THREADS];
-        if (MODE == 0 && !eps0 && !((iflags >> u) & 1u) && q >= u0 && q < u1) {
-            const float mi = P.pack[(int64_t)(q / TJ) * TILE_FLOATS + P_M * TJ + (q % TJ)];
-            o[6] += (double)(mi * rinv_e);
-        }
         if (ATOMIC) {
             if (q != -1) {
 #pragma unroll
@@ -442,7 +460,7 @@ __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
     }
     if (WARP && lane != 0) return;
     const int i = R.i_list ? R.i_list[k] : 0;     // by-value calls (nb_force_ext) carry no index list
-    if (i < 0 || i >= R.n) {
+    if (R.i_list && (i < 0 || i >= R.n)) {
 #pragma unroll
         for (int c = 0; c < NOUT; ++c) o[c] = __longlong_as_double(0x7ff8000000000000LL);
     } else if (R.i_list && R.nflag > 1 && (R.flags[i] & 1)) {
@@ -510,51 +528,69 @@ __host__ __device__ constexpr int force_smem(int jl)
 }  // namespace
 
 template <int JL>
-cudaError_t setup_one(int* blocks)
+cudaError_t setup_one(int* blocks, int* blocks_guard)
 {
-    const void* k[4] = {(const void*)force_kernel<false, JL, 0>, (const void*)force_kernel<true, JL, 0>,
-                        (const void*)force_kernel<false, JL, 1>, (const void*)force_kernel<false, JL, 2>};
-    for (int q = 0; q < 4; ++q) {
+    const void* k[8] = {(const void*)force_kernel<false, JL, 0, false>, (const void*)force_kernel<true, JL, 0, false>,
+                        (const void*)force_kernel<false, JL, 1, false>, (const void*)force_kernel<false, JL, 2, false>,
+                        (const void*)force_kernel<false, JL, 0, true>,  (const void*)force_kernel<true, JL, 0, true>,
+                        (const void*)force_kernel<false, JL, 1, true>,  (const void*)force_kernel<false, JL, 2, true>};
+    int least = 0;
+    for (int q = 0; q < 8; ++q) {
         cudaError_t e = cudaFuncSetAttribute(k[q], cudaFuncAttributeMaxDynamicSharedMemorySize, force_smem(JL));
         if (e != cudaSuccess) return e;
+        int b = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k[q], FORCE_THREADS, force_smem(JL));
+        if (e != cudaSuccess) return e;
+        if (q == 0 || b < least) least = b;
     }
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks, force_kernel<false, JL, 0>,
-                                                         FORCE_THREADS, force_smem(JL));
+    // the dispatcher sizes whole waves with the by-index kernels' residency; the others only need >= 1
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks, k[0], FORCE_THREADS, force_smem(JL));
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_guard, k[4], FORCE_THREADS, force_smem(JL));
+    return (e == cudaSuccess && least < 1) ? cudaErrorLaunchOutOfResources : e;
 }
 
-cudaError_t force_kernel_setup(int* blocks_per_sm)
+cudaError_t force_kernel_setup(int* blocks_per_sm, int* blocks_per_sm_guard)
 {
-    int b = 0;
-    cudaError_t e = setup_one<JL_MID>(&b);
+    int b = 0, g = 0;
+    cudaError_t e = setup_one<JL_MID>(&b, &g);
     if (e != cudaSuccess) return e;
-    e = setup_one<JL_MAX>(&b);
+    e = setup_one<JL_MAX>(&b, &g);
     if (e != cudaSuccess) return e;
-    return setup_one<1>(blocks_per_sm);
+    return setup_one<1>(blocks_per_sm, blocks_per_sm_guard);
 }
 
 // mode: 0 = by index (nb_force), 1 = by value with jerk, 2 = by value, acc + pot only (nb_force_ext;
 // no atomics variant there)
-template <int JL>
+template <int JL, bool GUARD>
 void launch_one(const ForceArgs& a, int mode, int atomic_mode, double* acc, double* jrk, double* pot,
                 cudaStream_t s)
 {
     const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
     if (mode == 1)
-        force_kernel<false, JL, 1><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+        force_kernel<false, JL, 1, GUARD><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
     else if (mode == 2)
-        force_kernel<false, JL, 2><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+        force_kernel<false, JL, 2, GUARD><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
     else if (atomic_mode)
-        force_kernel<true, JL, 0><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+        force_kernel<true, JL, 0, GUARD><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
     else
-        force_kernel<false, JL, 0><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
+        force_kernel<false, JL, 0, GUARD><<<grid, FORCE_THREADS, force_smem(JL), s>>>(a, acc, jrk, pot);
 }
 
 cudaError_t launch_force(const ForceArgs& a, int jl, int mode, int atomic_mode, double* acc, double* jrk,
                          double* pot, cudaStream_t s)
 {
-    if (jl == JL_MAX) launch_one<JL_MAX>(a, mode, atomic_mode, acc, jrk, pot, s);
-    else if (jl == JL_MID) launch_one<JL_MID>(a, mode, atomic_mode, acc, jrk, pot, s);
-    else launch_one<1>(a, mode, atomic_mode, acc, jrk, pot, s);
+    const bool guard = a.eps2 < EPS2_GUARD;
+    if (jl == JL_MAX) {
+        if (guard) launch_one<JL_MAX, true>(a, mode, atomic_mode, acc, jrk, pot, s);
+        else launch_one<JL_MAX, false>(a, mode, atomic_mode, acc, jrk, pot, s);
+    } else if (jl == JL_MID) {
+        if (guard) launch_one<JL_MID, true>(a, mode, atomic_mode, acc, jrk, pot, s);
+        else launch_one<JL_MID, false>(a, mode, atomic_mode, acc, jrk, pot, s);
+    } else {
+        if (guard) launch_one<1, true>(a, mode, atomic_mode, acc, jrk, pot, s);
+        else launch_one<1, false>(a, mode, atomic_mode, acc, jrk, pot, s);
+    }
     return cudaGetLastError();
 }
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s)

@@ -16,40 +16,11 @@
 // roofline.
 #include "nb_internal.h"
 #include "pair64.h"
+#include "tma.h"
 
 namespace nb {
 
 namespace {
-
-__device__ __forceinline__ uint32_t smem_u32_(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init_(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx_(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(bar), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s_(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-        "l"(src), "r"(bytes), "r"(bar)
-        : "memory");
-}
 
 constexpr int STAGES64 = 4;
 constexpr int F64_SMEM = STAGES64 * (TILE64_BYTES + 16);
@@ -73,14 +44,14 @@ __global__ void __launch_bounds__(FORCE_THREADS, 3) force64_kernel(ForceArgs P)
 
     if (tid == 0) {
         for (int s = 0; s < STAGES64; ++s) {
-            mbar_init_(smem_u32_(&bars[s]), 1);
+            mbar_init(smem_u32(&bars[s]), 1);
             rel[s] = 0;
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
         for (int s = 0; s < STAGES64 && t0 + s < t1; ++s) {
-            mbar_expect_tx_(smem_u32_(&bars[s]), TILE64_BYTES);
-            bulk_g2s_(smem_u32_(tiles + s * TILE64_DOUBLES), P.pack64 + (int64_t)(t0 + s) * TILE64_DOUBLES,
-                      TILE64_BYTES, smem_u32_(&bars[s]));
+            mbar_expect_tx(smem_u32(&bars[s]), TILE64_BYTES);
+            bulk_g2s(smem_u32(tiles + s * TILE64_DOUBLES), P.pack64 + (int64_t)(t0 + s) * TILE64_DOUBLES,
+                      TILE64_BYTES, smem_u32(&bars[s]));
         }
     }
 
@@ -121,7 +92,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, 3) force64_kernel(ForceArgs P)
 
     for (int t = t0; t < t1; ++t) {
         const int st = (t - t0) % STAGES64;
-        mbar_wait_(smem_u32_(&bars[st]), ((t - t0) / STAGES64) & 1);
+        mbar_wait(smem_u32(&bars[st]), ((t - t0) / STAGES64) & 1);
         const double* T = tiles + st * TILE64_DOUBLES;
         const int jbase = t * TJ;
 #pragma unroll 2
@@ -146,12 +117,13 @@ __global__ void __launch_bounds__(FORCE_THREADS, 3) force64_kernel(ForceArgs P)
         }
         __syncwarp();
         if ((tid & 31) == 0) {
+            __threadfence_block();
             const int old = atomicAdd(&rel[st], 1);
             if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STAGES64 < t1) {
-                mbar_expect_tx_(smem_u32_(&bars[st]), TILE64_BYTES);
-                bulk_g2s_(smem_u32_(tiles + st * TILE64_DOUBLES),
+                mbar_expect_tx(smem_u32(&bars[st]), TILE64_BYTES);
+                bulk_g2s(smem_u32(tiles + st * TILE64_DOUBLES),
                           P.pack64 + (int64_t)(t + STAGES64) * TILE64_DOUBLES, TILE64_BYTES,
-                          smem_u32_(&bars[st]));
+                          smem_u32(&bars[st]));
             }
         }
     }

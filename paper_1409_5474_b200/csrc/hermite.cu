@@ -136,6 +136,7 @@ __device__ __forceinline__ double norm3(double x, double y, double z) { return s
 // R20: new power-of-two step after a step of d_old that ended at t1, given the wanted step w
 __device__ __forceinline__ double block_rule(double d, double w, double t1, double dt_min, double dt_max)
 {
+    d = d < dt_min ? dt_min : d;      // a step that was never set (0) must not stay below the grid
     if (w < d) {
         while (d > w && d * 0.5 >= dt_min) d *= 0.5;
     } else if (w >= 2.0 * d && 2.0 * d <= dt_max && fmod(t1, 2.0 * d) == 0.0) {
@@ -159,6 +160,10 @@ correct_kernel(StorePtrs st, double* __restrict__ dts, const int32_t* __restrict
         return;
     }
     const double h = t1 - st.f[F_T][i];
+    if (!(h != 0.0)) {                // zero step (dt never set) or NaN time: a2, a3 would be NaN
+        atomicOr(err, 2);
+        return;
+    }
     double a1[3], j1[3], a2[3], a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {

@@ -12,7 +12,7 @@ struct nb_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     int64_t n_max = 0, ni_max = 0, n_cap = 0, n = 0;
-    int sm_count = 148, blocks_per_sm = 1;
+    int sm_count = 148, blocks_per_sm = 1, blocks_per_sm_guard = 1;
 
     // device memory: either one cudaMalloc'ed slab or the caller's workspace
     bool allocated = false, own_slab = false;
@@ -23,6 +23,7 @@ struct nb_ctx {
     uint8_t* flags = nullptr;
     uint32_t* tileflag = nullptr;
     int32_t* flag_list = nullptr;
+    int32_t* flag_stage = nullptr;      // [2 x count] staging of nb_set_flags: indices, then values
     double* part = nullptr;
     size_t part_bytes = 0;
     int* err = nullptr;
@@ -47,6 +48,16 @@ struct nb_ctx {
 
     int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
+
+    struct SplitMemo {
+        int n_itiles = -1, ntiles = 0;
+        int64_t ni_pad = 0;
+        size_t part_bytes = 0;
+        int64_t resident = 0;
+        int tune = 0, splits = 1;
+    };
+    SplitMemo memo[8];
+    int memo_next = 0;
 
     bool predicted = false;
     double t_pred = 0.0;
@@ -73,7 +84,7 @@ constexpr size_t ALIGN = 256;
 inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t store, pack, flags, tileflag, flag_list, part, err, ilist, out, in, dts, blk_list, blk_out,
+    size_t store, pack, flags, tileflag, flag_list, flag_stage, part, err, ilist, out, in, dts, blk_list, blk_out,
         sel_meta, sel_counts, total;
     int64_t ni_pad;
     size_t part_bytes;
@@ -92,6 +103,7 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.flags = off; off += up((size_t)L.n_cap);
     L.tileflag = off; off += up((size_t)(ntiles + 31) / 32 * 4);
     L.flag_list = off; off += up((size_t)NB_MAX_FLAGGED * 4);
+    L.flag_stage = off; off += up((size_t)4 * NB_MAX_FLAGGED * 4);    // (index, value) pairs of one nb_set_flags
     // partial sums: S * 7 * ni_pad doubles.  S = 1 needs 56 B per i; small i-sets want many splits.
     // 4x leaves the remainder segment of an all-active call room for ~16 j-subsets (a full last wave)
     L.part_bytes = (size_t)NOUT * sizeof(double) * (size_t)ni_pad * 4;
@@ -134,6 +146,7 @@ int ensure_alloc(nb_ctx* c)
     c->flags = c->slab + L.flags;
     c->tileflag = reinterpret_cast<uint32_t*>(c->slab + L.tileflag);
     c->flag_list = reinterpret_cast<int32_t*>(c->slab + L.flag_list);
+    c->flag_stage = reinterpret_cast<int32_t*>(c->slab + L.flag_stage);
     c->part = reinterpret_cast<double*>(c->slab + L.part);
     c->part_bytes = L.part_bytes;
     c->err = reinterpret_cast<int*>(c->slab + L.err);
@@ -209,8 +222,8 @@ SrcPtrs make_src(const double* m, const double* x, const double* y, const double
 
 // choose the number of j-subsets S so that (i-tiles x S) fills the chip.  Efficiency
 // of a choice = useful tile-passes / (waves x resident CTAs x tiles per CTA).
-int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t part_bytes,
-                  int64_t resident)
+int choose_splits_scan(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t part_bytes,
+                       int64_t resident)
 {
     int64_t smax = (int64_t)(part_bytes / (NOUT * sizeof(double) * (size_t)ni_pad));
     if (smax > ntiles) smax = ntiles;
@@ -231,6 +244,20 @@ int choose_splits(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, siz
         }
     }
     return best;
+}
+
+int choose_splits(nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t part_bytes,
+                  int64_t resident)
+{
+    // block steps call this with the same few shapes over and over: remember the last answers
+    for (const nb_ctx::SplitMemo& q : c->memo)
+        if (q.n_itiles == n_itiles && q.ntiles == ntiles && q.ni_pad == ni_pad && q.part_bytes == part_bytes &&
+            q.resident == resident && q.tune == c->tune_splits)
+            return q.splits;
+    const int ans = choose_splits_scan(c, n_itiles, ntiles, ni_pad, part_bytes, resident);
+    c->memo[c->memo_next] = {n_itiles, ntiles, ni_pad, part_bytes, resident, c->tune_splits, ans};
+    c->memo_next = (c->memo_next + 1) % (int)(sizeof(c->memo) / sizeof(c->memo[0]));
+    return ans;
 }
 
 // ext_x != NULL: i-particles by value (nb_force_ext); ext_v == NULL then means acc + pot only
@@ -263,7 +290,8 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     const int jl = f64 ? 1 : (ni <= ITILE / JL_MAX ? JL_MAX : (ni <= ITILE / JL_MID ? JL_MID : 1));
     const int itile = ITILE / jl;
     const int n_itiles = (int)((ni + itile - 1) / itile);
-    const int resident = c->sm_count * (f64 ? c->blocks_per_sm64 : c->blocks_per_sm);
+    const int resident = c->sm_count * (f64 ? c->blocks_per_sm64
+                                            : ((float)eps2 < EPS2_GUARD ? c->blocks_per_sm_guard : c->blocks_per_sm));
 
     // the i-tiles are cut in two segments.  A = the largest multiple of the resident CTA
     // count, one j-subset each (whole waves of equal CTAs); B = the rest, whose j is split in S
@@ -396,7 +424,8 @@ int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* str
     c->ni_max = ni_max;
     c->sm_count = prop.multiProcessorCount;
     DeviceGuard g(device);
-    if (force_kernel_setup(&c->blocks_per_sm) != cudaSuccess || c->blocks_per_sm < 1) {
+    if (force_kernel_setup(&c->blocks_per_sm, &c->blocks_per_sm_guard) != cudaSuccess || c->blocks_per_sm < 1 ||
+        c->blocks_per_sm_guard < 1) {
         cudaGetLastError();
         delete c;
         return NB_ERR_CUDA;
@@ -572,17 +601,25 @@ int nb_set_flags(nb_ctx* c, const int32_t* idx, const uint8_t* flags, int64_t co
     DeviceGuard g(c->device);
     int rc = ensure_alloc(c);
     if (rc != NB_OK) return rc;
-    // rewrite the flag bytes of the old and new sets, the tile bitmap and the flagged list
+    // one staged list of (index, value) for the old set (-> 0) and the new set (-> 1), scattered by a
+    // small kernel; then the tile bitmap and the flagged list.  The sources are pageable host
+    // vectors: cudaMemcpyAsync stages such a source before it returns, so they may die here.
     const int64_t ntiles = c->n_cap / TJ;
     std::vector<uint32_t> tf((size_t)(ntiles + 31) / 32, 0u);
-    const uint8_t zero = 0, one = 1;
-    for (int32_t i : c->flagged)
-        if (cudaMemcpyAsync(c->flags + i, &zero, 1, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
-            return NB_ERR_CUDA;
+    std::vector<int32_t> stage;
+    for (int32_t i : c->flagged) stage.push_back(i);
     for (int32_t i : next) {
-        if (cudaMemcpyAsync(c->flags + i, &one, 1, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
-            return NB_ERR_CUDA;
+        stage.push_back(i);
         tf[(size_t)(i / TJ) >> 5] |= 1u << ((i / TJ) & 31);
+    }
+    const int cnt = (int)stage.size();
+    for (int k = 0; k < cnt; ++k) stage.push_back(k < (int)c->flagged.size() ? 0 : 1);
+    if (cnt > 0) {
+        if (cudaMemcpyAsync(c->flag_stage, stage.data(), stage.size() * 4, cudaMemcpyHostToDevice,
+                            c->stream) != cudaSuccess ||
+            launch_set_flags(c->flags, c->flag_stage, cnt, c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        c->launches += 1;
     }
     if (cudaMemcpyAsync(c->tileflag, tf.data(), tf.size() * 4, cudaMemcpyHostToDevice, c->stream) !=
         cudaSuccess)
@@ -591,8 +628,6 @@ int nb_set_flags(nb_ctx* c, const int32_t* idx, const uint8_t* flags, int64_t co
         cudaMemcpyAsync(c->flag_list, next.data(), next.size() * 4, cudaMemcpyHostToDevice,
                         c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
-    // the sources above are pageable host memory: the copies are staged before the calls return
-    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
     c->flagged.swap(next);
     c->predicted = false;   // the pack carries the flag word
     return NB_OK;
@@ -851,7 +886,10 @@ int nb_init_steps(nb_ctx* c, const int32_t* i_list, int64_t ni, const double* ac
     if (launch_init_steps(c->store, c->dts, i_list, ni, c->n, acc, jrk, eta_s, dt_min, dt_max, c->err,
                           c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
-    if (ni > 0) c->launches += 1;
+    if (ni > 0) {
+        c->launches += 1;
+        c->predicted = false;      // stored (a, jerk) changed: the packed predicted state is stale
+    }
     return NB_OK;
 }
 
@@ -897,7 +935,10 @@ int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const do
     if (launch_correct(c->store, c->dts, i_list, ni, c->n, t1, acc, jrk, eta, dt_min, dt_max, c->err,
                        c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
-    if (ni > 0) c->launches += 1;
+    if (ni > 0) {
+        c->launches += 1;
+        c->predicted = false;      // the j-store moved on: the packed predicted state is stale
+    }
     return NB_OK;
 }
 
@@ -907,6 +948,7 @@ int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, do
         return NB_ERR_ARG;
     int rc = nb_next_block(c, t, ni, nullptr);
     if (rc != NB_OK) return rc;
+    if (*ni == 0) return NB_ERR_STATE;       // every t + dt is NaN: nothing can be scheduled
     DeviceGuard g(c->device);
     const int64_t k = *ni;
     double* acc = c->blk_out;
@@ -938,22 +980,6 @@ int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const dou
     return NB_OK;
 }
 
-int nb_probe_fp32(nb_ctx* c, int kind, double* lane_ops_per_s)
-{
-    if (!c || !lane_ops_per_s || (kind != 0 && kind != 1)) return NB_ERR_ARG;
-    DeviceGuard g(c->device);
-    int rc = ensure_alloc(c);
-    if (rc != NB_OK) return rc;
-    // scratch: the partial buffer (>= 32 MiB; the probe writes sm_count x 8 x 128 floats); the
-    // probe synchronises the stream, so no force call is in flight on it
-    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
-    if (probe_fp32(kind, c->sm_count, reinterpret_cast<float*>(c->part), c->stream, lane_ops_per_s) !=
-        cudaSuccess)
-        return NB_ERR_CUDA;
-    c->launches += 4;
-    return NB_OK;
-}
-
 int nb_sync(nb_ctx* c)
 {
     if (!c) return NB_ERR_ARG;
@@ -967,9 +993,11 @@ int nb_sync(nb_ctx* c)
     }
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
     if (*c->err_pinned) {
+        // device latch: bit 0 = an index was out of range, bit 1 = a due particle had a zero step
+        const int bits = *c->err_pinned;
         *c->err_pinned = 0;
         if (cudaMemsetAsync(c->err, 0, sizeof(int), c->stream) != cudaSuccess) return NB_ERR_CUDA;
-        return NB_ERR_INDEX;
+        return (bits & 1) ? NB_ERR_INDEX : NB_ERR_STATE;
     }
     return NB_OK;
 }

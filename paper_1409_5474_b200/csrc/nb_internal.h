@@ -47,6 +47,9 @@ enum Pack64Field { Q_X = 0, Q_Y, Q_Z, Q_VX, Q_VY, Q_VZ, Q_M, Q_FLAG, NQF };
 constexpr int TILE64_DOUBLES = TJ * NQF;      // 1024
 constexpr int TILE64_BYTES = TILE64_DOUBLES * 8;   // 8192
 
+// calls with eps2 below this (zero included) drop r = 0 pairs inside the packed pair (force.cu GUARD):
+// the self pair's m eps^-3 would leave the fp32 range (m up to ~1e8 is safe at the threshold)
+constexpr float EPS2_GUARD = 1.0e-20f;
 constexpr float PAD_POS = 1.0e10f;            // where the m = 0 padding records of the last tile sit
 
 struct StorePtrs {
@@ -96,11 +99,12 @@ cudaError_t launch_set_j(const StorePtrs& dst, const SrcPtrs& src, int64_t first
                          cudaStream_t s);
 cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int32_t* idx,
                             int64_t count, int64_t n, int* err, cudaStream_t s);
+cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int count, cudaStream_t s);
 cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64, int64_t n,
                            double t, cudaStream_t s);
 cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
                                  double* out, cudaStream_t s);
-cudaError_t force_kernel_setup(int* blocks_per_sm);
+cudaError_t force_kernel_setup(int* blocks_per_sm, int* blocks_per_sm_guard);
 cudaError_t force64_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_force64(const ForceArgs& a, int mode, cudaStream_t s);
 cudaError_t launch_force(const ForceArgs& a, int jl, int mode, int atomic_mode, double* acc, double* jrk,
@@ -120,7 +124,6 @@ cudaError_t launch_get_state(const StorePtrs& st, const double* dts, int64_t fir
 cudaError_t launch_fused(const StorePtrs& st, const uint8_t* flags, const int32_t* i_list, int ni, int64_t n,
                          double t, double eps2, int any_flagged, double* part, int* err, int sm_count,
                          int* grid_out, int* ni_pad_out, cudaStream_t s);
-cudaError_t probe_fp32(int kind, int sm_count, float* scratch, cudaStream_t s, double* lane_ops_per_s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 
 // Hermite predictor of one component (R1), shared by predict / get_predicted / the flagged-pair

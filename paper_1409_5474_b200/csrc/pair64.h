@@ -6,7 +6,12 @@
 
 namespace nb {
 
-// 1/sqrt(s) to fp64 rounding: hardware approximation on the fp32-rounded argument + 2 Newton steps
+// 1/sqrt(s) to fp64 rounding: hardware approximation on the fp32-rounded argument + 2 Newton steps.
+// Valid for s inside the normal fp32 range [S_MIN, ~3.4e38]: below it the fp32 argument would be
+// flushed to zero (rsqrt = inf, NaN after the Newton steps), so pair64 treats s < S_MIN as s = 0
+// (coincident, contributes nothing, R6); above it the approximation returns 0 (out of range,
+// contributes nothing).  In length units: pairs closer than 1.1e-19 or farther than 1.8e19.
+constexpr double S_MIN = 1.1754943508222875e-38;      // FLT_MIN
 __device__ __forceinline__ double rsqrt64(double s)
 {
     float y0;
@@ -31,7 +36,7 @@ __device__ __forceinline__ void pair64(const double* xi, Acc64& A, double xj, do
     const double dx = xj - xi[0], dy = yj - xi[1], dz = zj - xi[2];
     const double s = fma(dz, dz, fma(dy, dy, fma(dx, dx, e2)));
     double y = rsqrt64(s);
-    y = (skip || !(s > 0.0)) ? 0.0 : y;                // self pair (R5) or coincident with eps2 = 0 (R6)
+    y = (skip || !(s >= S_MIN)) ? 0.0 : y;             // self pair (R5) or coincident with eps2 = 0 (R6)
     const double y2 = y * y;
     const double mr = mj * y;
     const double mr3 = mr * y2;

@@ -39,6 +39,15 @@ __global__ void __launch_bounds__(256) update_j_kernel(StorePtrs dst, SrcPtrs sr
     }
 }
 
+// nb_set_flags: stage[0..count) = particle indices, stage[count..2 count) = new flag values, in
+// order (a particle listed twice -- leaving the old set and entering the new one -- ends as 1
+// because one thread walks the list)
+__global__ void set_flags_kernel(uint8_t* flags, const int32_t* __restrict__ stage, int count)
+{
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (int k = 0; k < count; ++k) flags[stage[k]] = (uint8_t)stage[count + k];
+}
+
 __device__ __forceinline__ double2 ld2(const double* p, int64_t i)
 {
     return __ldg(reinterpret_cast<const double2*>(p + i));
@@ -151,6 +160,12 @@ cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int3
 {
     if (count == 0) return cudaSuccess;
     update_j_kernel<<<grid_for(count, 256, 148 * 16), 256, 0, s>>>(dst, src, idx, count, n, err);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int count, cudaStream_t s)
+{
+    set_flags_kernel<<<1, 32, 0, s>>>(flags, idx_then_val, count);
     return cudaGetLastError();
 }
 
