@@ -474,46 +474,60 @@ def run_blockstep(args):
     eps2, eta, lo, hi = (4.0 / n) ** 2, 0.02, 2.0 ** -24, 2.0 ** -4
     m, x, v = nbgen.plummer(n, nbgen.SEED0 + 6)
     il = np.arange(n, dtype=np.int32)
-    def run(fused):
-        """The same `--steps` block steps from the same start, with or without the fused path."""
+    def run(mode):
+        """The same `--steps` block steps from the same start: mode "step" = one nb_step call per
+        block (five launches + a synchronisation each), "steps" = one nb_steps call (persistent
+        kernel; the host sees only the blocks above the bound)."""
         with nbm.Context(n) as ctx:
-            ctx.fused(fused)
             ctx.set_j(m, x, v)
             ctx.predict(0.0)
             ga, gj, gp = ctx.force(il, eps2)
             ctx.init_steps(il, ga, gj, eta, lo, hi)
             for _ in range(max(args.warmup, 3)):
                 ctx.step(eps2, eta, lo, hi)
+            ctx.steps(3, eps2, eta, lo, hi)
             ctx.sync()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             l0 = ctx.launch_count()
-            sz = []
             w0 = time.perf_counter()
             e0.record()
-            for _ in range(args.steps):
-                t, ni = ctx.step(eps2, eta, lo, hi)
-                sz.append(ni)
+            if mode == "step":
+                sz = []
+                for _ in range(args.steps):
+                    t, ni = ctx.step(eps2, eta, lo, hi)
+                    sz.append(ni)
+            else:
+                done, tl, sz = ctx.steps(args.steps, eps2, eta, lo, hi)
+                assert done == args.steps
+                t = float(tl[-1])
             e1.record()
             ctx.sync()
-            return e0.elapsed_time(e1), time.perf_counter() - w0, ctx.launch_count() - l0, sz, t
+            return e0.elapsed_time(e1), time.perf_counter() - w0, ctx.launch_count() - l0, list(sz), t
 
-    # A/B inside one process, interleaved (off, on, off, on): numbers from different gpurun calls
-    # differ by +-20 % for a latency-bound loop and must not be compared with each other
-    runs = [(f, run(f)) for f in (False, True, False, True)]
-    ms_off = min(r[0] for f, r in runs if not f)
-    ms, wall, launches, sizes, t = min((r for f, r in runs if f), key=lambda r: r[0])
+    # A/B inside one process, interleaved: numbers from different gpurun calls differ by +-20 % for a
+    # latency-bound loop and must not be compared with each other
+    runs = [(md, run(md)) for md in ("step", "steps", "step", "steps")]
+    ms_step, _, launches_step, _, _ = min((r for md, r in runs if md == "step"), key=lambda r: r[0])
+    ms, wall, launches, sizes, t = min((r for md, r in runs if md == "steps"), key=lambda r: r[0])
     sizes = np.array(sizes, dtype=np.float64)
+    in_kernel = int(((sizes <= 256) & (sizes * n <= 3.0e7)).sum())
     line = {"metric": "interactions/s", "value": float(sizes.sum() * n / (ms * 1e-3)),
             "unit": "interactions/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "wall_ms_per_step": wall / args.steps * 1e3,
-            "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "higher_is_better": True, "dtype": "f64 in the persistent kernel, f32 pair terms in large blocks",
+            "data": "synthetic",
             "config": {"workload": "blockstep_plummer_N%d" % n, "eta": eta, "eps2": eps2,
-                       "step": "nb_step = nb_next_block + nb_predict + nb_force + nb_correct"},
+                       "step": "nb_steps: scheduler + predictor-in-pair-loop + reduce + corrector per block in "
+                               "one persistent kernel; blocks above 256 particles or 3e7 pairs via nb_step"},
             "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),
                       "min_n_i": int(sizes.min()), "max_n_i": int(sizes.max()),
+                      "in_persistent_kernel": in_kernel,
                       "particle_steps_per_s": float(sizes.sum() / (ms * 1e-3)), "t_end": t},
-            "fused_ab": {"ms_per_step_fused_off": ms_off / args.steps, "ms_per_step_fused_on": ms / args.steps,
-                         "note": "same process, same schedule, best of 2 each, interleaved"},
+            "ab": {"us_per_block_step_nb_step": ms_step / args.steps * 1e3,
+                   "us_per_block_step_nb_steps": ms / args.steps * 1e3,
+                   "launches_per_block_nb_step": launches_step / args.steps,
+                   "launches_per_block_nb_steps": launches / args.steps,
+                   "note": "same process, same start and schedule, best of 2 each, interleaved"},
             "gpu_launches": int(launches)}
     print(json.dumps(line))
     return 0

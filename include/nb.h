@@ -268,6 +268,28 @@ int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const do
  * of the block stay in a context-owned buffer (nb_block_forces). */
 int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, double* t, int64_t* ni);
 
+/* Up to k block steps without a host round trip per step (the host link is "the
+ * crucial bottleneck"; with individual steps most blocks hold a handful of
+ * particles).  One persistent cooperative kernel runs scheduler -> predictor inside an IEEE-double
+ * pair loop over the j-store -> reduction -> corrector -> step criterion for step after step
+ * (three grid-wide barriers per step, no launch, no synchronisation; same readings R1..R9, R12,
+ * R18..R21 and the same decisions as nb_step).  It hands a block back to the host only when the block
+ * is large -- more than 256 particles, or N_i x n above the bound of nb_set_steps_bound (default
+ * 3e7 pairs) -- because nb_step's packed fp32 pair kernel is then the faster way; after that one
+ * nb_step the kernel is started again.  So the host synchronises once per LARGE block and once at the
+ * end, never per small block.
+ * Stops after k steps, or before the first block whose time exceeds t_end (+inf: no limit; NaN is
+ * NB_ERR_ARG).  HOST outputs: *done = steps taken; t_log[0..done) and ni_log[0..done) = block time and
+ * size of every step (either may be NULL; the log is kept on the device and copied once, at the end).
+ * Errors as nb_step; NB_ERR_STATE if no particle can be scheduled (every t + dt is NaN).  The forces
+ * of the last block are available through nb_block_forces. */
+int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, double dt_max, double t_end,
+             double* t_log, int64_t* ni_log, int64_t* done);
+
+/* Largest N_i x n the persistent kernel of nb_steps takes itself (0: every block goes through
+ * nb_step's launches; for tests and experiments). */
+int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs);
+
 /* nb_step takes blocks of <= NB_FUSED_MAX particles through nb_force_fused (default on).  on = 0
  * switches this off. */
 int nb_set_fused(nb_ctx* c, int on);

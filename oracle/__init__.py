@@ -54,6 +54,12 @@ def _lib():
                                    ctypes.c_int64, ctypes.POINTER(ctypes.c_int32), ctypes.c_double,
                                    dp, dp, dp]
         L.oracle_force.restype = None
+        L.oracle_force6.argtypes = [ctypes.c_int64, dp, dp, dp, dp, ctypes.POINTER(ctypes.c_uint8),
+                                    ctypes.c_int64, ctypes.POINTER(ctypes.c_int32), ctypes.c_double,
+                                    dp, dp, dp, dp]
+        L.oracle_force6.restype = None
+        L.oracle_predict_acc.argtypes = [ctypes.c_int64, ctypes.c_double, dp, dp, dp, dp]
+        L.oracle_predict_acc.restype = None
         L.oracle_threads.restype = ctypes.c_int
         _LIB = L
     return _LIB
@@ -99,3 +105,34 @@ def force(m, xp, vp, i_list, eps2, flags=None):
                         il.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), float(eps2),
                         _d(acc), _d(jrk), _d(pot))
     return acc, jrk, pot
+
+
+def predict_acc(t, a, j, tj):
+    """Predicted acceleration ap = a + jerk (t - tj), (3, n) (reading R22)."""
+    a, j, tj = _c(a), _c(j), _c(tj)
+    n = tj.shape[0]
+    assert a.shape == j.shape == (3, n)
+    ap = np.empty((3, n))
+    _lib().oracle_predict_acc(n, float(t), _d(a), _d(j), _d(tj), _d(ap))
+    return ap
+
+
+def force6(m, xp, vp, ap, i_list, eps2, flags=None):
+    """6th-order variant: acc, jrk, snp (3, ni) and pot (ni,) on particles i_list, given positions,
+    velocities and accelerations (3, n) of all particles at one instant."""
+    m, xp, vp, ap = _c(m), _c(xp), _c(vp), _c(ap)
+    n = m.shape[0]
+    assert xp.shape == vp.shape == ap.shape == (3, n)
+    il = _c(i_list, np.int32)
+    ni = il.shape[0]
+    assert ni == 0 or (il.min() >= 0 and il.max() < n)
+    fl = None
+    if flags is not None:
+        flags = _c(flags, np.uint8)
+        assert flags.shape == (n,)
+        fl = flags.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8))
+    acc, jrk, snp, pot = np.empty((3, ni)), np.empty((3, ni)), np.empty((3, ni)), np.empty(ni)
+    _lib().oracle_force6(n, _d(m), _d(xp), _d(vp), _d(ap), fl, ni,
+                         il.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), float(eps2),
+                         _d(acc), _d(jrk), _d(snp), _d(pot))
+    return acc, jrk, snp, pot

@@ -174,6 +174,13 @@ class Context:
     def step(self, eps2, eta, dt_min, dt_max):
         return nb.nb_step(self.h, eps2, eta, dt_min, dt_max)
 
+    def steps(self, k, eps2, eta, dt_min, dt_max, t_end=float("inf"), log=True):
+        """Up to k block steps without a host round trip per step: (done, t_log, ni_log)."""
+        return nb.nb_steps(self.h, k, eps2, eta, dt_min, dt_max, t_end, log)
+
+    def steps_bound(self, max_pairs):
+        nb.nb_set_steps_bound(self.h, max_pairs)
+
     # -- measurement --------------------------------------------------------------------------
     def profiling(self, on=True):
         nb.nb_set_profiling(self.h, on)

@@ -8,24 +8,13 @@
 #include <cooperative_groups.h>
 
 #include "nb_internal.h"
+#include "hermite_dev.h"
 
 namespace cg = cooperative_groups;
 
 namespace nb {
 
 namespace {
-
-// order-preserving map double -> uint64 (so that atomicMin on integers is a min on doubles)
-__device__ __forceinline__ unsigned long long key_of(double x)
-{
-    const long long b = __double_as_longlong(x);
-    return (unsigned long long)(b ^ ((b >> 63) | (long long)0x8000000000000000ull));
-}
-__device__ __forceinline__ double of_key(unsigned long long k)
-{
-    const long long b = (long long)k;
-    return __longlong_as_double(b ^ ((~b >> 63) | (long long)0x8000000000000000ull));
-}
 
 constexpr int SEL_THREADS = 256;
 
@@ -131,20 +120,6 @@ select_kernel(const double* __restrict__ t, const double* __restrict__ dt, int64
     }
 }
 
-__device__ __forceinline__ double norm3(double x, double y, double z) { return sqrt(x * x + y * y + z * z); }
-
-// R20: new power-of-two step after a step of d_old that ended at t1, given the wanted step w
-__device__ __forceinline__ double block_rule(double d, double w, double t1, double dt_min, double dt_max)
-{
-    d = d < dt_min ? dt_min : d;      // a step that was never set (0) must not stay below the grid
-    if (w < d) {
-        while (d > w && d * 0.5 >= dt_min) d *= 0.5;
-    } else if (w >= 2.0 * d && 2.0 * d <= dt_max && fmod(t1, 2.0 * d) == 0.0) {
-        d *= 2.0;
-    }
-    return d;
-}
-
 // R12 + R18 + R19 + R20 for the particles list[0..ni): forces (a1, j1) at t1 are acc/jrk[c*ni + k].
 // In place on the j-store; writes t = t1 and the new step.
 __global__ void __launch_bounds__(128)
@@ -159,34 +134,13 @@ correct_kernel(StorePtrs st, double* __restrict__ dts, const int32_t* __restrict
         atomicOr(err, 1);
         return;
     }
-    const double h = t1 - st.f[F_T][i];
-    if (!(h != 0.0)) {                // zero step (dt never set) or NaN time: a2, a3 would be NaN
-        atomicOr(err, 2);
-        return;
-    }
-    double a1[3], j1[3], a2[3], a3[3];
+    double a1[3], j1[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double x0 = st.f[F_X + c][i], v0 = st.f[F_VX + c][i];
-        const double a0 = st.f[F_AX + c][i], j0 = st.f[F_JX + c][i];
         a1[c] = acc[(int64_t)c * ni + k];
         j1[c] = jrk[(int64_t)c * ni + k];
-        const double v1 = v0 + (a0 + a1[c]) * (h / 2.0) + (j0 - j1[c]) * (h * h / 12.0);
-        const double x1 = x0 + (v0 + v1) * (h / 2.0) + (a0 - a1[c]) * (h * h / 12.0);
-        const double a2_0 = (-6.0 * (a0 - a1[c]) - h * (4.0 * j0 + 2.0 * j1[c])) / (h * h);
-        a3[c] = (12.0 * (a0 - a1[c]) + 6.0 * h * (j0 + j1[c])) / (h * h * h);
-        a2[c] = a2_0 + h * a3[c];
-        st.f[F_X + c][i] = x1;
-        st.f[F_VX + c][i] = v1;
-        st.f[F_AX + c][i] = a1[c];
-        st.f[F_JX + c][i] = j1[c];
     }
-    const double na = norm3(a1[0], a1[1], a1[2]), nj = norm3(j1[0], j1[1], j1[2]);
-    const double n2 = norm3(a2[0], a2[1], a2[2]), n3 = norm3(a3[0], a3[1], a3[2]);
-    const double num = eta * (na * n2 + nj * nj), den = nj * n3 + n2 * n2;
-    const double want = den > 0.0 ? sqrt(num / den) : __longlong_as_double(0x7ff0000000000000ll);
-    st.f[F_T][i] = t1;
-    dts[i] = block_rule(dts[i], want, t1, dt_min, dt_max);
+    correct_one(st, dts, i, t1, a1, j1, eta, dt_min, dt_max, err);
 }
 
 // Start (R19, R20): store (a, j) of the listed particles and give each its first step.

@@ -38,6 +38,13 @@ struct nb_ctx {
     double* blk_out = nullptr;          // [7][ni_pad]
     unsigned long long* sel_meta = nullptr;   // [0] key of t1, [1] count
     int* sel_counts = nullptr;          // [SEL_MAX_BLOCKS]
+    int32_t* steps_scratch = nullptr;   // [STEPS_NI_MAX] (steps.cu)
+    unsigned long long* steps_meta = nullptr;   // [8]
+    double* steps_log_t = nullptr;      // device log of nb_steps, cudaMalloc'ed and grown on demand
+    long long* steps_log_ni = nullptr;
+    int64_t steps_log_cap = 0;
+    int64_t steps_max_pairs = 30000000; // blocks with ni x n above this go through nb_step's launches
+    int steps_ok = -1;                  // -1 unknown, 0 the cooperative kernel cannot be resident, 1 fine
     double blk_t = 0.0;                 // what the last nb_next_block returned
     int64_t blk_ni = -1;
 
@@ -46,7 +53,7 @@ struct nb_ctx {
     double* pack64 = nullptr;
     int blocks_per_sm64 = 1;
 
-    int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy
+    int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy; 32..63: nb_steps status
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
 
     struct SplitMemo {
@@ -85,7 +92,7 @@ inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 
 struct Layout {
     size_t store, pack, flags, tileflag, flag_list, flag_stage, part, err, ilist, out, in, dts, blk_list, blk_out,
-        sel_meta, sel_counts, total;
+        sel_meta, sel_counts, steps_scratch, steps_meta, total;
     int64_t ni_pad;
     size_t part_bytes;
     int64_t n_cap;
@@ -118,6 +125,8 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.blk_out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
     L.sel_meta = off; off += up(16);
     L.sel_counts = off; off += up((size_t)SEL_MAX_BLOCKS * 4);
+    L.steps_scratch = off; off += up((size_t)STEPS_NI_MAX * 4);
+    L.steps_meta = off; off += up(8 * 8);
     L.ni_pad = ni_pad;
     L.total = off;
     return L;
@@ -158,6 +167,8 @@ int ensure_alloc(nb_ctx* c)
     c->blk_out = reinterpret_cast<double*>(c->slab + L.blk_out);
     c->sel_meta = reinterpret_cast<unsigned long long*>(c->slab + L.sel_meta);
     c->sel_counts = reinterpret_cast<int*>(c->slab + L.sel_counts);
+    c->steps_scratch = reinterpret_cast<int32_t*>(c->slab + L.steps_scratch);
+    c->steps_meta = reinterpret_cast<unsigned long long*>(c->slab + L.steps_meta);
     c->ni_pad = L.ni_pad;
     c->allocated = true;
     return NB_OK;
@@ -430,7 +441,7 @@ int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* str
         delete c;
         return NB_ERR_CUDA;
     }
-    if (cudaMallocHost(&c->err_pinned, 32) != cudaSuccess) {
+    if (cudaMallocHost(&c->err_pinned, 64) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return NB_ERR_ALLOC;
@@ -446,6 +457,8 @@ int nb_destroy(nb_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->own_slab && c->slab) cudaFree(c->slab);
     if (c->pack64) cudaFree(c->pack64);
+    if (c->steps_log_t) cudaFree(c->steps_log_t);
+    if (c->steps_log_ni) cudaFree(c->steps_log_ni);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
     for (nb_ctx::Rec& R : c->ring)
         for (cudaEvent_t e : R.e)
@@ -969,6 +982,126 @@ int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, do
     }
     if (rc != NB_OK) return rc;
     return nb_correct(c, c->blk_list, k, *t, acc, jrk, eta, dt_min, dt_max);
+}
+
+int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs)
+{
+    if (!c || max_pairs < 0) return NB_ERR_ARG;
+    c->steps_max_pairs = max_pairs;
+    return NB_OK;
+}
+
+int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, double dt_max, double t_end,
+             double* t_log, int64_t* ni_log, int64_t* done)
+{
+    if (!c || k < 0 || !done || !isfinite(eps2) || eps2 < 0.0 || !(eta > 0.0) || !steps_ok(dt_min, dt_max) ||
+        t_end != t_end)
+        return NB_ERR_ARG;
+    *done = 0;
+    if (k == 0) return NB_OK;
+    if (c->n < 1) return NB_ERR_STATE;
+    DeviceGuard g(c->device);
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (c->steps_ok < 0) {
+        int b = 0;
+        c->steps_ok = (steps_kernel_setup(&b) == cudaSuccess && b >= 1) ? 1 : 0;
+        cudaGetLastError();
+    }
+    if (k > c->steps_log_cap) {               // the device log grows to the largest k asked for
+        if (c->steps_log_t) cudaFree(c->steps_log_t);
+        if (c->steps_log_ni) cudaFree(c->steps_log_ni);
+        c->steps_log_t = nullptr;
+        c->steps_log_ni = nullptr;
+        c->steps_log_cap = 0;
+        if (cudaMalloc(&c->steps_log_t, (size_t)k * 8) != cudaSuccess ||
+            cudaMalloc(&c->steps_log_ni, (size_t)k * 8) != cudaSuccess) {
+            cudaGetLastError();
+            return NB_ERR_ALLOC;
+        }
+        c->steps_log_cap = k;
+    }
+    unsigned long long* status = reinterpret_cast<unsigned long long*>(c->err_pinned) + 4;
+    std::vector<int64_t> host_idx;            // steps that went through nb_step: (index, t, ni)
+    std::vector<double> host_t;
+    std::vector<int64_t> host_ni;
+    int64_t s = 0;
+    int result = NB_OK;
+    while (s < k) {
+        int reason = STEPS_BIG;
+        if (c->steps_ok == 1) {
+            StepsArgs a{};
+            a.st = c->store;
+            a.dts = c->dts;
+            a.flags = c->flags;
+            a.any_flagged = c->flagged.empty() ? 0 : 1;
+            a.n = c->n;
+            a.scratch = c->steps_scratch;
+            a.list = c->blk_list;
+            a.cap = c->ni_max;
+            a.part = c->part;
+            a.out = c->blk_out;
+            a.meta = c->steps_meta;
+            a.log_t = c->steps_log_t + s;
+            a.log_ni = c->steps_log_ni + s;
+            a.budget = k - s;
+            a.eps2 = eps2;
+            a.eta = eta;
+            a.dt_min = dt_min;
+            a.dt_max = dt_max;
+            a.t_end = t_end;
+            a.max_pairs = c->steps_max_pairs;
+            a.err = c->err;
+            if (launch_steps(a, c->sm_count, c->stream) != cudaSuccess) {
+                cudaGetLastError();
+                return NB_ERR_CUDA;
+            }
+            c->launches += 1;
+            c->predicted = false;
+            if (cudaMemcpyAsync(status, c->steps_meta + 4, 32, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+                cudaStreamSynchronize(c->stream) != cudaSuccess)
+                return NB_ERR_CUDA;
+            const int64_t did = (int64_t)status[0];
+            reason = (int)status[1];
+            if (did > 0 && reason != STEPS_BIG) c->blk_ni = (int64_t)status[3];   // for nb_block_forces
+            s += did;
+            if (reason == STEPS_DONE || reason == STEPS_T_END) break;
+            if (reason == STEPS_STUCK) {
+                result = NB_ERR_STATE;
+                break;
+            }
+        }
+        // one block the persistent kernel does not take: nb_step's launches (packed fp32 pair kernel)
+        double t = 0.0;
+        int64_t ni = 0;
+        if (c->steps_ok != 1) {               // no persistent kernel: nb_step decides everything
+            rc = nb_next_block(c, &t, &ni, nullptr);
+            if (rc != NB_OK) { result = rc; break; }
+            if (ni == 0) { result = NB_ERR_STATE; break; }
+            if (!(t <= t_end)) break;
+        }
+        rc = nb_step(c, eps2, eta, dt_min, dt_max, &t, &ni);
+        if (rc != NB_OK) { result = rc; break; }
+        host_idx.push_back(s);
+        host_t.push_back(t);
+        host_ni.push_back(ni);
+        s += 1;
+    }
+    *done = s;
+    if (s > 0 && (t_log || ni_log)) {
+        if (t_log && cudaMemcpyAsync(t_log, c->steps_log_t, (size_t)s * 8, cudaMemcpyDeviceToHost, c->stream) !=
+                         cudaSuccess)
+            return NB_ERR_CUDA;
+        if (ni_log && cudaMemcpyAsync(ni_log, c->steps_log_ni, (size_t)s * 8, cudaMemcpyDeviceToHost,
+                                      c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+        for (size_t q = 0; q < host_idx.size(); ++q) {
+            if (t_log) t_log[host_idx[q]] = host_t[q];
+            if (ni_log) ni_log[host_idx[q]] = host_ni[q];
+        }
+    }
+    return result;
 }
 
 int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const double** pot)

@@ -126,6 +126,33 @@ cudaError_t launch_fused(const StorePtrs& st, const uint8_t* flags, const int32_
                          int* grid_out, int* ni_pad_out, cudaStream_t s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 
+// ---- nb_steps (steps.cu): block steps in one persistent cooperative kernel ---------------------
+constexpr int STEPS_NI_MAX = 256;             // largest block the persistent kernel takes itself
+enum StepsReason { STEPS_RUNNING = 0, STEPS_DONE, STEPS_BIG, STEPS_T_END, STEPS_STUCK };
+struct StepsArgs {
+    StorePtrs st;
+    double* dts;
+    const uint8_t* flags;
+    int any_flagged;
+    int64_t n;
+    int32_t* scratch;             // [STEPS_NI_MAX] due particles in the order of the atomics
+    int32_t* list;                // the context's block list (ascending), as nb_next_block leaves it
+    int64_t cap;                  // ni_max
+    double* part;                 // [NOUT][ni][CTAs]
+    double* out;                  // the context's block forces [NOUT][ni]
+    unsigned long long* meta;     // [0,1] min keys, [2,3] counters (by step parity); [4..7] exit status:
+                                  // steps done, StepsReason, key of the pending block time, N_i of the
+                                  // pending block (STEPS_BIG) or of the last block completed
+    double* log_t;                // [budget] block times, from this launch's first step
+    long long* log_ni;            // [budget] block sizes
+    int64_t budget;
+    double eps2, eta, dt_min, dt_max, t_end;
+    int64_t max_pairs;            // a block with ni x n above this is left to the host path
+    int* err;
+};
+cudaError_t steps_kernel_setup(int* blocks_per_sm);
+cudaError_t launch_steps(const StepsArgs& a, int sm_count, cudaStream_t s);
+
 // Hermite predictor of one component (R1), shared by predict / get_predicted / the flagged-pair
 // fix-up so that all three see the same fp64 state.
 __device__ __forceinline__ void predict1(double x, double v, double a, double j, double dt,
