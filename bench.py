@@ -497,20 +497,25 @@ def run_blockstep(args):
                     t, ni = ctx.step(eps2, eta, lo, hi)
                     sz.append(ni)
             else:
-                done, tl, sz = ctx.steps(args.steps, eps2, eta, lo, hi)
+                done, tl, sz, us = ctx.steps(args.steps, eps2, eta, lo, hi, times=True)
                 assert done == args.steps
                 t = float(tl[-1])
+                times.append(np.array(us))
             e1.record()
             ctx.sync()
             return e0.elapsed_time(e1), time.perf_counter() - w0, ctx.launch_count() - l0, list(sz), t
 
     # A/B inside one process, interleaved: numbers from different gpurun calls differ by +-20 % for a
     # latency-bound loop and must not be compared with each other
+    times = []
     runs = [(md, run(md)) for md in ("step", "steps", "step", "steps")]
     ms_step, _, launches_step, _, _ = min((r for md, r in runs if md == "step"), key=lambda r: r[0])
     ms, wall, launches, sizes, t = min((r for md, r in runs if md == "steps"), key=lambda r: r[0])
     sizes = np.array(sizes, dtype=np.float64)
-    in_kernel = int(((sizes <= 256) & (sizes * n <= 3.0e7)).sum())
+    small = (sizes <= 512) & (sizes * n <= 3.0e7)
+    in_kernel = int(small.sum())
+    us = np.minimum(times[0], times[1])                    # per-step device time (%globaltimer), best of 2
+    floor_us = sizes * n / 1.2408e12 * 1e6                  # pair work at 100 % of the FP32 peak
     line = {"metric": "interactions/s", "value": float(sizes.sum() * n / (ms * 1e-3)),
             "unit": "interactions/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "wall_ms_per_step": wall / args.steps * 1e3,
@@ -522,6 +527,12 @@ def run_blockstep(args):
             "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),
                       "min_n_i": int(sizes.min()), "max_n_i": int(sizes.max()),
                       "in_persistent_kernel": in_kernel,
+                      "us_per_step_in_kernel_mean": float(us[small].mean()) if in_kernel else None,
+                      "us_per_step_in_kernel_median": float(np.median(us[small])) if in_kernel else None,
+                      "us_per_step_host_path_mean": float(us[~small].mean()) if in_kernel < len(sizes) else None,
+                      "us_total_in_kernel": float(us[small].sum()), "us_total_host_path": float(us[~small].sum()),
+                      "us_pair_work_at_fp32_peak_total": float(floor_us.sum()),
+                      "us_pair_work_at_fp32_peak_host_path": float(floor_us[~small].sum()),
                       "particle_steps_per_s": float(sizes.sum() / (ms * 1e-3)), "t_end": t},
             "ab": {"us_per_block_step_nb_step": ms_step / args.steps * 1e3,
                    "us_per_block_step_nb_steps": ms / args.steps * 1e3,

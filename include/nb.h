@@ -274,17 +274,19 @@ int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, do
  * pair loop over the j-store -> reduction -> corrector -> step criterion for step after step
  * (three grid-wide barriers per step, no launch, no synchronisation; same readings R1..R9, R12,
  * R18..R21 and the same decisions as nb_step).  It hands a block back to the host only when the block
- * is large -- more than 256 particles, or N_i x n above the bound of nb_set_steps_bound (default
+ * is large -- more than 512 particles, or N_i x n above the bound of nb_set_steps_bound (default
  * 3e7 pairs) -- because nb_step's packed fp32 pair kernel is then the faster way; after that one
- * nb_step the kernel is started again.  So the host synchronises once per LARGE block and once at the
- * end, never per small block.
+ * nb_step (queued without a second synchronisation: time and size of the block are known) the kernel
+ * is started again.  So the host synchronises once per LARGE block and once at the end, never per
+ * small block.
  * Stops after k steps, or before the first block whose time exceeds t_end (+inf: no limit; NaN is
- * NB_ERR_ARG).  HOST outputs: *done = steps taken; t_log[0..done) and ni_log[0..done) = block time and
- * size of every step (either may be NULL; the log is kept on the device and copied once, at the end).
+ * NB_ERR_ARG).  HOST outputs: *done = steps taken; t_log[0..done), ni_log[0..done) and us_log[0..done)
+ * = block time, block size and device time in microseconds (%globaltimer) of every step (each may be
+ * NULL; the log is kept on the device and copied once, at the end).
  * Errors as nb_step; NB_ERR_STATE if no particle can be scheduled (every t + dt is NaN).  The forces
  * of the last block are available through nb_block_forces. */
 int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, double dt_max, double t_end,
-             double* t_log, int64_t* ni_log, int64_t* done);
+             double* t_log, int64_t* ni_log, double* us_log, int64_t* done);
 
 /* Largest N_i x n the persistent kernel of nb_steps takes itself (0: every block goes through
  * nb_step's launches; for tests and experiments). */

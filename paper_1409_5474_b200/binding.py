@@ -67,7 +67,7 @@ lib.nb_init_steps.argtypes = [_vp, _vp, _i64, _vp, _vp, _dbl, _dbl, _dbl]
 lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(_dbl), ctypes.POINTER(_i64), ctypes.POINTER(_vp)]
 lib.nb_correct.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _dbl, _dbl, _dbl]
 lib.nb_step.argtypes = [_vp, _dbl, _dbl, _dbl, _dbl, ctypes.POINTER(_dbl), ctypes.POINTER(_i64)]
-lib.nb_steps.argtypes = [_vp, _i64, _dbl, _dbl, _dbl, _dbl, _dbl, _vp, _vp, ctypes.POINTER(_i64)]
+lib.nb_steps.argtypes = [_vp, _i64, _dbl, _dbl, _dbl, _dbl, _dbl, _vp, _vp, _vp, ctypes.POINTER(_i64)]
 lib.nb_set_steps_bound.argtypes = [_vp, _i64]
 lib.nb_block_forces.argtypes = [_vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp), ctypes.POINTER(_vp)]
 lib.nb_version.restype = ctypes.c_char_p
@@ -265,18 +265,20 @@ def nb_step(c, eps2, eta, dt_min, dt_max):
     return t.value, ni.value
 
 
-def nb_steps(c, k, eps2, eta, dt_min, dt_max, t_end=float("inf"), log=True):
+def nb_steps(c, k, eps2, eta, dt_min, dt_max, t_end=float("inf"), log=True, times=False):
     """Up to k block steps on the device; returns (done, t_log, ni_log) -- numpy arrays of length
-    done (None, None with log=False)."""
+    done (None, None with log=False) -- and with times=True also the device time of every step in
+    microseconds."""
     import numpy as np
     done = _i64(0)
     t_log = np.empty(max(k, 1), np.float64) if log else None
     ni_log = np.empty(max(k, 1), np.int64) if log else None
-    _check(lib.nb_steps(c, k, eps2, eta, dt_min, dt_max, t_end, _ptr(t_log), _ptr(ni_log), ctypes.byref(done)),
-           "nb_steps")
-    if not log:
-        return done.value, None, None
-    return done.value, t_log[:done.value], ni_log[:done.value]
+    us_log = np.empty(max(k, 1), np.float64) if times else None
+    _check(lib.nb_steps(c, k, eps2, eta, dt_min, dt_max, t_end, _ptr(t_log), _ptr(ni_log), _ptr(us_log),
+                        ctypes.byref(done)), "nb_steps")
+    d = done.value
+    out = (d, t_log[:d] if log else None, ni_log[:d] if log else None)
+    return out + (us_log[:d],) if times else out
 
 
 def nb_set_steps_bound(c, max_pairs):

@@ -174,9 +174,9 @@ class Context:
     def step(self, eps2, eta, dt_min, dt_max):
         return nb.nb_step(self.h, eps2, eta, dt_min, dt_max)
 
-    def steps(self, k, eps2, eta, dt_min, dt_max, t_end=float("inf"), log=True):
-        """Up to k block steps without a host round trip per step: (done, t_log, ni_log)."""
-        return nb.nb_steps(self.h, k, eps2, eta, dt_min, dt_max, t_end, log)
+    def steps(self, k, eps2, eta, dt_min, dt_max, t_end=float("inf"), log=True, times=False):
+        """Up to k block steps without a host round trip per step: (done, t_log, ni_log[, us_log])."""
+        return nb.nb_steps(self.h, k, eps2, eta, dt_min, dt_max, t_end, log, times)
 
     def steps_bound(self, max_pairs):
         nb.nb_set_steps_bound(self.h, max_pairs)

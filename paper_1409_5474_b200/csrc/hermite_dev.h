@@ -32,24 +32,43 @@ __device__ __forceinline__ double block_rule(double d, double w, double t1, doub
     return d;
 }
 
-// R12 + R18 + R19 + R20 for particle i, whose forces at t1 are (a1, j1): corrector, interpolated
-// derivatives, Aarseth step, block rule; in place on the j-store, writes t = t1 and the new step.
-// A zero step (h = 0: steps never set) or a NaN time would make a2, a3 NaN: the particle is left
-// alone and bit 1 of the error latch is set (nb_sync -> NB_ERR_STATE).
-__device__ __forceinline__ void correct_one(const StorePtrs& st, double* __restrict__ dts, int64_t i, double t1,
-                                            const double* a1, const double* j1, double eta, double dt_min,
-                                            double dt_max, int* err)
+// The stored state of one particle that the corrector reads.
+struct Stored {
+    double x[3], v[3], a[3], j[3], t, dt;
+};
+__device__ __forceinline__ Stored load_stored(const StorePtrs& st, const double* __restrict__ dts, int64_t i)
 {
-    const double h = t1 - st.f[F_T][i];
+    Stored s;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        s.x[c] = st.f[F_X + c][i];
+        s.v[c] = st.f[F_VX + c][i];
+        s.a[c] = st.f[F_AX + c][i];
+        s.j[c] = st.f[F_JX + c][i];
+    }
+    s.t = st.f[F_T][i];
+    s.dt = dts[i];
+    return s;
+}
+
+// R12 + R18 + R19 + R20 for particle i, whose stored state is s0 and whose forces at t1 are (a1, j1):
+// corrector, interpolated derivatives, Aarseth step, block rule; writes x1, v1, a1, j1, t = t1 and the
+// new step into the j-store and returns the new step.  A zero step (h = 0: steps never set) or a NaN
+// time would make a2, a3 NaN: the particle is left alone, bit 1 of the error latch is set (nb_sync ->
+// NB_ERR_STATE) and the old step is returned.
+__device__ __forceinline__ double correct_stored(const StorePtrs& st, double* __restrict__ dts, int64_t i,
+                                                 const Stored& s0, double t1, const double* a1, const double* j1,
+                                                 double eta, double dt_min, double dt_max, int* err)
+{
+    const double h = t1 - s0.t;
     if (!(h != 0.0)) {
         atomicOr(err, 2);
-        return;
+        return s0.dt;
     }
     double a2[3], a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double x0 = st.f[F_X + c][i], v0 = st.f[F_VX + c][i];
-        const double a0 = st.f[F_AX + c][i], j0 = st.f[F_JX + c][i];
+        const double x0 = s0.x[c], v0 = s0.v[c], a0 = s0.a[c], j0 = s0.j[c];
         const double v1 = v0 + (a0 + a1[c]) * (h / 2.0) + (j0 - j1[c]) * (h * h / 12.0);
         const double x1 = x0 + (v0 + v1) * (h / 2.0) + (a0 - a1[c]) * (h * h / 12.0);
         const double a2_0 = (-6.0 * (a0 - a1[c]) - h * (4.0 * j0 + 2.0 * j1[c])) / (h * h);
@@ -64,8 +83,18 @@ __device__ __forceinline__ void correct_one(const StorePtrs& st, double* __restr
     const double n2 = norm3(a2[0], a2[1], a2[2]), n3 = norm3(a3[0], a3[1], a3[2]);
     const double num = eta * (na * n2 + nj * nj), den = nj * n3 + n2 * n2;
     const double want = den > 0.0 ? sqrt(num / den) : __longlong_as_double(0x7ff0000000000000ll);
+    const double d = block_rule(s0.dt, want, t1, dt_min, dt_max);
     st.f[F_T][i] = t1;
-    dts[i] = block_rule(dts[i], want, t1, dt_min, dt_max);
+    dts[i] = d;
+    return d;
+}
+
+__device__ __forceinline__ void correct_one(const StorePtrs& st, double* __restrict__ dts, int64_t i, double t1,
+                                            const double* a1, const double* j1, double eta, double dt_min,
+                                            double dt_max, int* err)
+{
+    const Stored s0 = load_stored(st, dts, i);
+    correct_stored(st, dts, i, s0, t1, a1, j1, eta, dt_min, dt_max, err);
 }
 
 }  // namespace nb

@@ -38,10 +38,11 @@ struct nb_ctx {
     double* blk_out = nullptr;          // [7][ni_pad]
     unsigned long long* sel_meta = nullptr;   // [0] key of t1, [1] count
     int* sel_counts = nullptr;          // [SEL_MAX_BLOCKS]
-    int32_t* steps_scratch = nullptr;   // [STEPS_NI_MAX] (steps.cu)
+    StepsSlot* steps_slots = nullptr;   // [256] (steps.cu)
     unsigned long long* steps_meta = nullptr;   // [8]
     double* steps_log_t = nullptr;      // device log of nb_steps, cudaMalloc'ed and grown on demand
     long long* steps_log_ni = nullptr;
+    unsigned long long* steps_log_ns = nullptr;
     int64_t steps_log_cap = 0;
     int64_t steps_max_pairs = 30000000; // blocks with ni x n above this go through nb_step's launches
     int steps_ok = -1;                  // -1 unknown, 0 the cooperative kernel cannot be resident, 1 fine
@@ -92,7 +93,7 @@ inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 
 struct Layout {
     size_t store, pack, flags, tileflag, flag_list, flag_stage, part, err, ilist, out, in, dts, blk_list, blk_out,
-        sel_meta, sel_counts, steps_scratch, steps_meta, total;
+        sel_meta, sel_counts, steps_slots, steps_meta, total;
     int64_t ni_pad;
     size_t part_bytes;
     int64_t n_cap;
@@ -125,7 +126,7 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.blk_out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
     L.sel_meta = off; off += up(16);
     L.sel_counts = off; off += up((size_t)SEL_MAX_BLOCKS * 4);
-    L.steps_scratch = off; off += up((size_t)STEPS_NI_MAX * 4);
+    L.steps_slots = off; off += up((size_t)256 * sizeof(StepsSlot));
     L.steps_meta = off; off += up(8 * 8);
     L.ni_pad = ni_pad;
     L.total = off;
@@ -167,7 +168,7 @@ int ensure_alloc(nb_ctx* c)
     c->blk_out = reinterpret_cast<double*>(c->slab + L.blk_out);
     c->sel_meta = reinterpret_cast<unsigned long long*>(c->slab + L.sel_meta);
     c->sel_counts = reinterpret_cast<int*>(c->slab + L.sel_counts);
-    c->steps_scratch = reinterpret_cast<int32_t*>(c->slab + L.steps_scratch);
+    c->steps_slots = reinterpret_cast<StepsSlot*>(c->slab + L.steps_slots);
     c->steps_meta = reinterpret_cast<unsigned long long*>(c->slab + L.steps_meta);
     c->ni_pad = L.ni_pad;
     c->allocated = true;
@@ -459,6 +460,7 @@ int nb_destroy(nb_ctx* c)
     if (c->pack64) cudaFree(c->pack64);
     if (c->steps_log_t) cudaFree(c->steps_log_t);
     if (c->steps_log_ni) cudaFree(c->steps_log_ni);
+    if (c->steps_log_ns) cudaFree(c->steps_log_ns);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
     for (nb_ctx::Rec& R : c->ring)
         for (cudaEvent_t e : R.e)
@@ -955,6 +957,30 @@ int nb_correct(nb_ctx* c, const int32_t* i_list, int64_t ni, double t1, const do
     return NB_OK;
 }
 
+// the part of a block step after the scheduler: forces on the k particles of the context's block list
+// at time t, then corrector and new steps
+static int step_body(nb_ctx* c, double t, int64_t k, double eps2, double eta, double dt_min, double dt_max)
+{
+    double* acc = c->blk_out;
+    double* jrk = c->blk_out + 3 * k;
+    double* pot = c->blk_out + 6 * k;
+    // where the fused pass wins (DESIGN.md 12.3, one timing table): up to 4 particles at any N; 5..8
+    // only while its fp64 arithmetic (35 ops x ni per j) stays below the cost of the saved pass
+    const bool small = k <= 4 || (k <= NB_FUSED_MAX && c->n <= ((int64_t)1 << 18));
+    int rc;
+    if (small && c->tune_fused) {
+        // a handful of particles: one fused pass over the j-store instead of predict + force
+        rc = fused_impl(c, t, c->blk_list, k, eps2, acc, jrk, pot);
+        c->predicted = false;
+    } else {
+        rc = nb_predict(c, t);
+        if (rc != NB_OK) return rc;
+        rc = force_impl(c, c->blk_list, k, eps2, acc, jrk, pot);
+    }
+    if (rc != NB_OK) return rc;
+    return nb_correct(c, c->blk_list, k, t, acc, jrk, eta, dt_min, dt_max);
+}
+
 int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, double* t, int64_t* ni)
 {
     if (!c || !t || !ni || !isfinite(eps2) || eps2 < 0.0 || !(eta > 0.0) || !steps_ok(dt_min, dt_max))
@@ -963,25 +989,7 @@ int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, do
     if (rc != NB_OK) return rc;
     if (*ni == 0) return NB_ERR_STATE;       // every t + dt is NaN: nothing can be scheduled
     DeviceGuard g(c->device);
-    const int64_t k = *ni;
-    double* acc = c->blk_out;
-    double* jrk = c->blk_out + 3 * k;
-    double* pot = c->blk_out + 6 * k;
-    // where the fused pass wins (DESIGN.md 12.3, one timing table): up to 4 particles at any N; 5..8
-    // only while its fp64 arithmetic (35 ops x ni per j) stays below the cost of the saved pass
-    const bool small = k <= 4 || (k <= NB_FUSED_MAX && c->n <= ((int64_t)1 << 18));
-    if (small && c->tune_fused) {
-        // a handful of particles: one fused pass over the j-store instead of predict + force; the
-        // packed predicted state is NOT refreshed by such a step
-        rc = fused_impl(c, *t, c->blk_list, k, eps2, acc, jrk, pot);
-        c->predicted = false;
-    } else {
-        rc = nb_predict(c, *t);
-        if (rc != NB_OK) return rc;
-        rc = force_impl(c, c->blk_list, k, eps2, acc, jrk, pot);
-    }
-    if (rc != NB_OK) return rc;
-    return nb_correct(c, c->blk_list, k, *t, acc, jrk, eta, dt_min, dt_max);
+    return step_body(c, *t, *ni, eps2, eta, dt_min, dt_max);
 }
 
 int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs)
@@ -992,7 +1000,7 @@ int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs)
 }
 
 int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, double dt_max, double t_end,
-             double* t_log, int64_t* ni_log, int64_t* done)
+             double* t_log, int64_t* ni_log, double* us_log, int64_t* done)
 {
     if (!c || k < 0 || !done || !isfinite(eps2) || eps2 < 0.0 || !(eta > 0.0) || !steps_ok(dt_min, dt_max) ||
         t_end != t_end)
@@ -1011,84 +1019,123 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
     if (k > c->steps_log_cap) {               // the device log grows to the largest k asked for
         if (c->steps_log_t) cudaFree(c->steps_log_t);
         if (c->steps_log_ni) cudaFree(c->steps_log_ni);
+        if (c->steps_log_ns) cudaFree(c->steps_log_ns);
         c->steps_log_t = nullptr;
         c->steps_log_ni = nullptr;
+        c->steps_log_ns = nullptr;
         c->steps_log_cap = 0;
         if (cudaMalloc(&c->steps_log_t, (size_t)k * 8) != cudaSuccess ||
-            cudaMalloc(&c->steps_log_ni, (size_t)k * 8) != cudaSuccess) {
+            cudaMalloc(&c->steps_log_ni, (size_t)k * 8) != cudaSuccess ||
+            cudaMalloc(&c->steps_log_ns, (size_t)(k + 1) * 8) != cudaSuccess) {
             cudaGetLastError();
             return NB_ERR_ALLOC;
         }
         c->steps_log_cap = k;
     }
     unsigned long long* status = reinterpret_cast<unsigned long long*>(c->err_pinned) + 4;
-    std::vector<int64_t> host_idx;            // steps that went through nb_step: (index, t, ni)
+    std::vector<int64_t> host_idx;            // steps that went through the host path: (index, t, ni)
     std::vector<double> host_t;
     std::vector<int64_t> host_ni;
     int64_t s = 0;
     int result = NB_OK;
+    bool last_was_host = false;
+    auto launch = [&](int64_t budget) -> int {
+        StepsArgs a{};
+        a.st = c->store;
+        a.dts = c->dts;
+        a.flags = c->flags;
+        a.any_flagged = c->flagged.empty() ? 0 : 1;
+        a.n = c->n;
+        a.slots = c->steps_slots;
+        a.list = c->blk_list;
+        a.cap = c->ni_max;
+        a.part = c->part;
+        a.out = c->blk_out;
+        a.meta = c->steps_meta;
+        a.log_t = c->steps_log_t + s;
+        a.log_ni = c->steps_log_ni + s;
+        a.log_ns = c->steps_log_ns + s;
+        a.budget = budget;
+        a.eps2 = eps2;
+        a.eta = eta;
+        a.dt_min = dt_min;
+        a.dt_max = dt_max;
+        a.t_end = t_end;
+        a.max_pairs = c->steps_max_pairs;
+        a.err = c->err;
+        if (launch_steps(a, c->sm_count, c->stream) != cudaSuccess) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        c->launches += 1;
+        c->predicted = false;
+        return NB_OK;
+    };
     while (s < k) {
-        int reason = STEPS_BIG;
+        double t = 0.0;
+        int64_t ni = 0;
         if (c->steps_ok == 1) {
-            StepsArgs a{};
-            a.st = c->store;
-            a.dts = c->dts;
-            a.flags = c->flags;
-            a.any_flagged = c->flagged.empty() ? 0 : 1;
-            a.n = c->n;
-            a.scratch = c->steps_scratch;
-            a.list = c->blk_list;
-            a.cap = c->ni_max;
-            a.part = c->part;
-            a.out = c->blk_out;
-            a.meta = c->steps_meta;
-            a.log_t = c->steps_log_t + s;
-            a.log_ni = c->steps_log_ni + s;
-            a.budget = k - s;
-            a.eps2 = eps2;
-            a.eta = eta;
-            a.dt_min = dt_min;
-            a.dt_max = dt_max;
-            a.t_end = t_end;
-            a.max_pairs = c->steps_max_pairs;
-            a.err = c->err;
-            if (launch_steps(a, c->sm_count, c->stream) != cudaSuccess) {
-                cudaGetLastError();
-                return NB_ERR_CUDA;
-            }
-            c->launches += 1;
-            c->predicted = false;
+            rc = launch(k - s);
+            if (rc != NB_OK) return rc;
             if (cudaMemcpyAsync(status, c->steps_meta + 4, 32, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
                 cudaStreamSynchronize(c->stream) != cudaSuccess)
                 return NB_ERR_CUDA;
             const int64_t did = (int64_t)status[0];
-            reason = (int)status[1];
-            if (did > 0 && reason != STEPS_BIG) c->blk_ni = (int64_t)status[3];   // for nb_block_forces
+            const int reason = (int)status[1];
+            if (did > 0) {
+                last_was_host = false;
+                if (reason != STEPS_BIG) c->blk_ni = (int64_t)status[3];   // for nb_block_forces
+            }
             s += did;
             if (reason == STEPS_DONE || reason == STEPS_T_END) break;
             if (reason == STEPS_STUCK) {
                 result = NB_ERR_STATE;
                 break;
             }
-        }
-        // one block the persistent kernel does not take: nb_step's launches (packed fp32 pair kernel)
-        double t = 0.0;
-        int64_t ni = 0;
-        if (c->steps_ok != 1) {               // no persistent kernel: nb_step decides everything
+            // one block the persistent kernel does not take.  Its time and size are known, so the
+            // scheduler kernel (it leaves the ascending list on the device) and nb_step's launches
+            // (packed fp32 pair kernel) are queued without another synchronisation.
+            const long long kb = (long long)status[2];
+            const long long bits = kb ^ ((~kb >> 63) | (long long)0x8000000000000000ull);
+            memcpy(&t, &bits, 8);
+            ni = (int64_t)status[3];
+            if (ni > c->ni_max) {
+                result = NB_ERR_ARG;
+                break;
+            }
+            if (launch_select(c->store.f[F_T], c->dts, c->n, c->sel_meta, c->sel_counts, c->blk_list, c->ni_pad,
+                              c->sm_count, c->stream) != cudaSuccess) {
+                cudaGetLastError();
+                return NB_ERR_CUDA;
+            }
+            c->launches += 1;
+            c->blk_t = t;
+            c->blk_ni = ni;
+            rc = step_body(c, t, ni, eps2, eta, dt_min, dt_max);
+        } else {                              // no persistent kernel on this device: nb_step does everything
             rc = nb_next_block(c, &t, &ni, nullptr);
+            if (rc == NB_OK && ni == 0) rc = NB_ERR_STATE;
             if (rc != NB_OK) { result = rc; break; }
-            if (ni == 0) { result = NB_ERR_STATE; break; }
             if (!(t <= t_end)) break;
+            rc = step_body(c, t, ni, eps2, eta, dt_min, dt_max);
         }
-        rc = nb_step(c, eps2, eta, dt_min, dt_max, &t, &ni);
         if (rc != NB_OK) { result = rc; break; }
         host_idx.push_back(s);
         host_t.push_back(t);
         host_ni.push_back(ni);
+        last_was_host = true;
         s += 1;
     }
     *done = s;
-    if (s > 0 && (t_log || ni_log)) {
+    if (s > 0 && (t_log || ni_log || us_log)) {
+        std::vector<unsigned long long> ns;
+        if (us_log && c->steps_ok == 1) {
+            if (last_was_host && launch(0) != NB_OK) return NB_ERR_CUDA;   // closing time stamp after a host block
+            ns.resize((size_t)s + 1);
+            if (cudaMemcpyAsync(ns.data(), c->steps_log_ns, ns.size() * 8, cudaMemcpyDeviceToHost, c->stream) !=
+                cudaSuccess)
+                return NB_ERR_CUDA;
+        }
         if (t_log && cudaMemcpyAsync(t_log, c->steps_log_t, (size_t)s * 8, cudaMemcpyDeviceToHost, c->stream) !=
                          cudaSuccess)
             return NB_ERR_CUDA;
@@ -1100,6 +1147,9 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
             if (t_log) t_log[host_idx[q]] = host_t[q];
             if (ni_log) ni_log[host_idx[q]] = host_ni[q];
         }
+        if (us_log)
+            for (int64_t q = 0; q < s; ++q)
+                us_log[q] = ns.empty() ? 0.0 : (double)(long long)(ns[q + 1] - ns[q]) * 1e-3;
     }
     return result;
 }

@@ -127,24 +127,30 @@ cudaError_t launch_fused(const StorePtrs& st, const uint8_t* flags, const int32_
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
 
 // ---- nb_steps (steps.cu): block steps in one persistent cooperative kernel ---------------------
-constexpr int STEPS_NI_MAX = 256;             // largest block the persistent kernel takes itself
+constexpr int STEPS_NI_MAX = 512;             // largest block the persistent kernel takes itself
+constexpr int STEPS_SLOT = 128;               // most due particles one slice can publish
 enum StepsReason { STEPS_RUNNING = 0, STEPS_DONE, STEPS_BIG, STEPS_T_END, STEPS_STUCK };
+struct StepsSlot {                            // what one CTA publishes about its slice of the particles
+    unsigned long long key;                   // order-preserving key of its earliest t + dt
+    int count, pad;                           // how many of its particles are due then
+    int32_t idx[STEPS_SLOT];                  // their indices, ascending (the first STEPS_SLOT)
+};
 struct StepsArgs {
     StorePtrs st;
     double* dts;
     const uint8_t* flags;
     int any_flagged;
     int64_t n;
-    int32_t* scratch;             // [STEPS_NI_MAX] due particles in the order of the atomics
+    StepsSlot* slots;             // [CTAs]
     int32_t* list;                // the context's block list (ascending), as nb_next_block leaves it
     int64_t cap;                  // ni_max
     double* part;                 // [NOUT][ni][CTAs]
     double* out;                  // the context's block forces [NOUT][ni]
-    unsigned long long* meta;     // [0,1] min keys, [2,3] counters (by step parity); [4..7] exit status:
-                                  // steps done, StepsReason, key of the pending block time, N_i of the
-                                  // pending block (STEPS_BIG) or of the last block completed
+    unsigned long long* meta;     // [4..7] exit status: steps done, StepsReason, key of the pending block
+                                  // time, N_i of the pending block (STEPS_BIG) or of the last one completed
     double* log_t;                // [budget] block times, from this launch's first step
     long long* log_ni;            // [budget] block sizes
+    unsigned long long* log_ns;   // [budget + 1] %globaltimer at the start of each step and at the exit
     int64_t budget;
     double eps2, eta, dt_min, dt_max, t_end;
     int64_t max_pairs;            // a block with ni x n above this is left to the host path

@@ -6,26 +6,29 @@
 // PAPER.md:51 says a handful of active particles cannot hide latencies.  With individual steps most
 // blocks ARE a handful of particles (median 4 at N = 16384), so a block step done as five launches
 // plus a synchronisation (nb_step) is all latency.  Here one grid of at most one 512-thread CTA per
-// SM runs the whole loop and meets at three grid-wide barriers per step:
-//   A  t1 = min_j (t_j + dt_j): each CTA scans its slice of the particles, one atomicMin per CTA  (R21)
-//      -- barrier --
-//   B  particles due at t1 append themselves to a scratch list (atomic counter)                  (R21)
-//      -- barrier --   every CTA now knows N_i; a block that is too large for this kernel ends it
-//   C  every CTA sorts the (short) list by rank in shared memory -- ascending, as R21 states, so the
-//      result does not depend on the order of the atomics --, predicts the due particles (R1, R8),
-//      then streams ITS slice of the j-store once: 512 particles at a time are predicted into shared
-//      memory and the threads, arranged as (i-particle, j-stride), evaluate the pairs in IEEE
-//      double (pair64.h: the same body as nb_force_fused; self pair by index, flagged pairs
-//      unsoftened, R5..R7).  One partial sum per CTA and i-particle, [7][N_i][CTAs].
-//      -- barrier --
+// SM runs the whole loop and meets at TWO grid-wide barriers per step:
+//   A  each CTA scans its slice of the particles (their keys t_j + dt_j sit in shared memory) for
+//      the slice's earliest time and publishes it with the particles due then, ascending   (R21)
+//      -- barrier 1 --
+//   B  every CTA reads the <= 148 published minima: the smallest is the block time t1, the slices
+//      that attain it hold the due particles; concatenated in slice order the list is ascending,
+//      as R21 states, without atomics.  A block that is too large for this kernel ends it here.
+//   C  every CTA predicts the due particles (R1, R8), then streams ITS slice of the j-store once:
+//      512 particles at a time are predicted into shared memory and the threads, arranged as
+//      (i-particle, j-stride), evaluate the pairs in IEEE double (pair64.h: the same body as
+//      nb_force_fused; self pair by index, flagged pairs unsoftened, R5..R7).  One partial sum per
+//      CTA and i-particle, [7][N_i][CTAs].
+//      -- barrier 2 --
 //   D  the CTA that owns a due particle sums its partials (a warp per particle, fixed order:
 //      deterministic, R9), stores the forces for nb_block_forces and runs the corrector and the
-//      step criterion (correct_one: R12, R18..R20).  It then goes straight on to A of the next step:
-//      A and B only read the CTA's own slice.
+//      step criterion (correct_stored: R12, R18..R20; the particle's stored state was fetched while
+//      waiting at barrier 2).  It then goes straight on to A of the next step, which only reads the
+//      CTA's own slice.
 // The kernel stops when its budget of steps is used up, when the next block time exceeds t_end, or
-// when the next block is larger than it handles (N_i > STEPS_NI_MAX or N_i x N above the caller's
-// bound): the host then takes that one block through nb_step's launches, where the packed fp32 pair
-// kernel is faster, and starts the kernel again.  (t1, N_i) of every step go to a device log.
+// when the next block is larger than it handles (N_i > STEPS_NI_MAX, N_i x N above the caller's
+// bound, or more than STEPS_SLOT due particles in one slice): the host then takes that one block
+// through nb_step's launches, where the packed fp32 pair kernel is faster, and starts the kernel
+// again.  (t1, N_i) and a device time stamp of every step go to a device log.
 #include <cooperative_groups.h>
 
 #include "hermite_dev.h"
@@ -41,17 +44,50 @@ namespace {
 constexpr int ST_THREADS = 512;
 constexpr int ST_WARPS = ST_THREADS / 32;
 constexpr int ST_TILE = ST_THREADS;           // j-particles predicted into shared memory at a time
+constexpr int ST_KEYS = 2048;                 // keys of a slice kept in shared memory (else re-read)
+constexpr int ST_GMAX = 256;                  // most CTAs (slices)
+
+// dynamic shared memory: si [NI_MAX][6] | tile [7][512] | keys [ST_KEYS]
+constexpr int ST_SMEM = STEPS_NI_MAX * 6 * 8 + NOUT * ST_TILE * 8 + ST_KEYS * 8;
 
 __device__ __forceinline__ double ldcg(const double* p) { return __ldcg(p); }
+__device__ __forceinline__ unsigned long long gtime()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// block-wide minimum of one key per thread (all threads get the result)
+__device__ __forceinline__ unsigned long long block_min(unsigned long long k, unsigned long long* sw, int lane,
+                                                        int warp)
+{
+#pragma unroll
+    for (int w = 16; w >= 1; w >>= 1) {
+        const unsigned long long o = __shfl_xor_sync(0xffffffffu, k, w);
+        k = o < k ? o : k;
+    }
+    __syncthreads();                          // sw may still be read from the previous use
+    if (lane == 0) sw[warp] = k;
+    __syncthreads();
+    k = sw[0];
+#pragma unroll
+    for (int w = 1; w < ST_WARPS; ++w) k = sw[w] < k ? sw[w] : k;
+    return k;
+}
 
 __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
 {
     cg::grid_group grid = cg::this_grid();
-    __shared__ double si[STEPS_NI_MAX][6];            // predicted state of the due particles
-    __shared__ double tile[NOUT][ST_TILE];            // x y z vx vy vz m of 512 j; later: the slice sums
-    __shared__ int sl_raw[STEPS_NI_MAX], sl[STEPS_NI_MAX];
+    extern __shared__ __align__(16) unsigned char dyn[];
+    double (*si)[6] = reinterpret_cast<double (*)[6]>(dyn);
+    double (*tile)[ST_TILE] = reinterpret_cast<double (*)[ST_TILE]>(dyn + STEPS_NI_MAX * 6 * 8);
+    unsigned long long* keys = reinterpret_cast<unsigned long long*>(dyn + STEPS_NI_MAX * 6 * 8 + NOUT * ST_TILE * 8);
+    __shared__ int sl[STEPS_NI_MAX];
     __shared__ unsigned char sfl[STEPS_NI_MAX], tfl[ST_TILE];
     __shared__ unsigned long long swmin[ST_WARPS];
+    __shared__ int swsum[ST_WARPS];
+    __shared__ int goff[ST_GMAX + 1];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = (int)gridDim.x, b = (int)blockIdx.x;
@@ -59,55 +95,94 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
     const int64_t chunk = (n + G - 1) / G;
     const int64_t lo = (int64_t)b * chunk < n ? (int64_t)b * chunk : n;
     const int64_t hi = lo + chunk < n ? lo + chunk : n;
+    const int cnt_own = (int)(hi - lo);
+    const bool cached = chunk <= ST_KEYS;
     const double* __restrict__ T = P.st.f[F_T];
     volatile unsigned long long* meta = P.meta;
+    StepsSlot* slots = P.slots;
+
+    if (cached)
+        for (int q = tid; q < cnt_own; q += ST_THREADS) keys[q] = key_of(ldcg(T + lo + q) + ldcg(P.dts + lo + q));
+    __syncthreads();
 
     long long last_ni = 0;                    // size of the last block this launch completed
-    for (int64_t s = 0; s < P.budget; ++s) {
-        const int par = (int)(s & 1);
+    for (int64_t s = 0; s <= P.budget; ++s) {
+        if (b == 0 && tid == 0) P.log_ns[s] = gtime();
+        if (s == P.budget) break;
 
-        // ---- A: the next block time (R21) ----------------------------------------------------
+        // ---- A: earliest time of my slice and who is due then (R21) ----------------------------
         unsigned long long k = ~0ull;
-        for (int64_t p = lo + tid; p < hi; p += ST_THREADS) {
-            const unsigned long long q = key_of(ldcg(T + p) + ldcg(P.dts + p));
-            k = q < k ? q : k;
+        for (int q = tid; q < cnt_own; q += ST_THREADS) {
+            const unsigned long long kq = cached ? keys[q] : key_of(ldcg(T + lo + q) + ldcg(P.dts + lo + q));
+            k = kq < k ? kq : k;
         }
+        const unsigned long long kmin = block_min(k, swmin, lane, warp);
+        int base = 0;
+        for (int q0 = 0; q0 < cnt_own; q0 += ST_THREADS) {
+            const int q = q0 + tid;
+            bool due = false;
+            if (q < cnt_own)
+                due = (cached ? keys[q] : key_of(ldcg(T + lo + q) + ldcg(P.dts + lo + q))) == kmin;
+            const unsigned bal = __ballot_sync(0xffffffffu, due);
+            if (lane == 0) swsum[warp] = __popc(bal);
+            __syncthreads();
+            int before = 0, total = 0;
 #pragma unroll
-        for (int w = 16; w >= 1; w >>= 1) {
-            const unsigned long long o = __shfl_xor_sync(0xffffffffu, k, w);
-            k = o < k ? o : k;
-        }
-        if (lane == 0) swmin[warp] = k;
-        __syncthreads();
-        if (tid == 0) {
-            for (int w = 1; w < ST_WARPS; ++w) k = swmin[w] < k ? swmin[w] : k;
-            atomicMin(P.meta + par, k);
-        }
-        grid.sync();
-        const double t1 = of_key(meta[par]);
-        if (b == 0 && tid == 0) {             // the other parity's slots, for the next step
-            meta[par ^ 1] = ~0ull;
-            meta[2 + (par ^ 1)] = 0ull;
-        }
-
-        // ---- B: who is due (R21) ---------------------------------------------------------------
-        for (int64_t p = lo + tid; p < hi; p += ST_THREADS) {
-            if (ldcg(T + p) + ldcg(P.dts + p) == t1) {
-                const unsigned long long pos = atomicAdd(P.meta + 2 + par, 1ull);
-                if (pos < (unsigned long long)STEPS_NI_MAX) P.scratch[pos] = (int32_t)p;
+            for (int w = 0; w < ST_WARPS; ++w) {
+                const int c = swsum[w];
+                total += c;
+                if (w < warp) before += c;
             }
+            if (due) {
+                const int pos = base + before + __popc(bal & ((1u << lane) - 1u));
+                if (pos < STEPS_SLOT) slots[b].idx[pos] = (int32_t)(lo + q);
+            }
+            base += total;
+            __syncthreads();
         }
-        grid.sync();
-        const long long ni64 = (long long)meta[2 + par];
+        if (tid == 0) {
+            slots[b].key = kmin;
+            slots[b].count = base;
+        }
+        grid.sync();                                                            // ---- barrier 1
+
+        // ---- B: the block time and the due list, from the published slices ---------------------
+        unsigned long long kg = ~0ull;
+        int cg_ = 0;
+        if (tid < G) {
+            kg = __ldcg(&slots[tid].key);
+            cg_ = __ldcg(&slots[tid].count);
+        }
+        const unsigned long long kall = block_min(kg, swmin, lane, warp);
+        const int mine = (tid < G && kg == kall && kall != ~0ull) ? cg_ : 0;
+        int incl = mine;                      // inclusive scan over the block
+#pragma unroll
+        for (int w = 1; w < 32; w <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, incl, w);
+            if (lane >= w) incl += o;
+        }
+        if (lane == 31) swsum[warp] = incl;
+        const int trunc = __syncthreads_or(mine > STEPS_SLOT);
+        int wbase = 0, ni_all = 0;
+#pragma unroll
+        for (int w = 0; w < ST_WARPS; ++w) {
+            const int c = swsum[w];
+            ni_all += c;
+            if (w < warp) wbase += c;
+        }
+        if (tid < G) goff[tid] = wbase + incl - mine;
+        if (tid == 0) goff[G] = ni_all;
+        const double t1 = of_key(kall);
+        const long long ni64 = ni_all;
         int reason = STEPS_RUNNING;
-        if (ni64 == 0) reason = STEPS_STUCK;                        // every t + dt is NaN
+        if (ni64 == 0 || t1 != t1) reason = STEPS_STUCK;            // no particle, or every t + dt is NaN
         else if (!(t1 <= P.t_end)) reason = STEPS_T_END;
-        else if (ni64 > STEPS_NI_MAX || ni64 > P.cap || ni64 * n > P.max_pairs) reason = STEPS_BIG;
+        else if (trunc || ni64 > STEPS_NI_MAX || ni64 > P.cap || ni64 * n > P.max_pairs) reason = STEPS_BIG;
         if (reason != STEPS_RUNNING) {        // uniform over the grid: everybody leaves
             if (b == 0 && tid == 0) {
                 meta[4] = (unsigned long long)s;
                 meta[5] = (unsigned long long)reason;
-                meta[6] = key_of(t1);
+                meta[6] = kall;
                 meta[7] = (unsigned long long)(reason == STEPS_BIG ? ni64 : last_ni);
             }
             return;
@@ -117,19 +192,17 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             P.log_t[s] = t1;
             P.log_ni[s] = ni64;
         }
-
-        // ---- C: sorted list, predicted i-particles, one pass over this CTA's j-slice -----------
-        if (tid < ni) sl_raw[tid] = __ldcg(P.scratch + tid);
-        __syncthreads();
+        __syncthreads();                      // goff complete
         if (tid < ni) {
-            const int me = sl_raw[tid];
-            int rank = 0;
-            for (int q = 0; q < ni; ++q) rank += sl_raw[q] < me ? 1 : 0;
-            sl[rank] = me;
-        }
-        __syncthreads();
-        if (tid < ni) {
-            const int64_t i = sl[tid];
+            int g0 = 0, g1 = G;               // the last slice g with goff[g] <= tid holds entry tid
+            while (g1 - g0 > 1) {
+                const int gm = (g0 + g1) >> 1;
+                if (goff[gm] <= tid) g0 = gm;
+                else g1 = gm;
+            }
+            const int64_t i = __ldcg(&slots[g0].idx[tid - goff[g0]]);
+            sl[tid] = (int)i;
+            // ---- C: predicted i-particles ...
             const double dti = t1 - ldcg(T + i);
 #pragma unroll
             for (int c = 0; c < 3; ++c)
@@ -138,11 +211,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             sfl[tid] = P.any_flagged ? (P.flags[i] & 1) : 0;
             if (b == 0) P.list[tid] = (int32_t)i;
         }
+        // ... and one pass over this CTA's j-slice
         const int ii = tid % ni, slice = tid / ni, nsl = ST_THREADS / ni;
         Acc64 A;
         A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.p = 0.0;
-        for (int64_t base = lo; base < hi; base += ST_TILE) {
-            const int64_t p = base + tid;
+        for (int64_t base_j = lo; base_j < hi; base_j += ST_TILE) {
+            const int64_t p = base_j + tid;
             if (p < hi) {
                 const double dtj = t1 - ldcg(T + p);
 #pragma unroll
@@ -153,9 +227,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
                 tfl[tid] = P.any_flagged ? (P.flags[p] & 1) : 0;
             }
             __syncthreads();                  // tile (and, the first time, si / sfl / sl) complete
-            const int cnt = (int)(hi - base < ST_TILE ? hi - base : ST_TILE);
+            const int cnt = (int)(hi - base_j < ST_TILE ? hi - base_j : ST_TILE);
             if (slice < nsl) {
-                const int self = sl[ii] - (int)base;      // position of the own index in this tile, if any
+                const int self = sl[ii] - (int)base_j;    // position of the own index in this tile, if any
 #pragma unroll 2
                 for (int q = slice; q < cnt; q += nsl) {
                     const double e2 = (sfl[ii] && tfl[q]) ? 0.0 : P.eps2;
@@ -187,17 +261,23 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
                 if (lane == 0) P.part[((int64_t)c * ni + i) * G + b] = sum;
             }
         }
-        grid.sync();
 
         // ---- D: the owner of a due particle sums its partials and corrects it ------------------
-        for (int q = warp; q < ni; q += ST_WARPS) {
-            const int64_t i = sl[q];
-            if (i < lo || i >= hi) continue;
+        // my due particles are entries [goff[b], goff[b+1]) of the list when my slice attains t1; a
+        // warp takes one of them at a time and fetches its stored state BEFORE the barrier
+        const int first = goff[b];
+        const int mycnt = goff[b + 1] - first;
+        Stored s0;
+        if (warp < mycnt) s0 = load_stored(P.st, P.dts, sl[first + warp]);
+        grid.sync();                                                            // ---- barrier 2
+        for (int q = warp; q < mycnt; q += ST_WARPS) {
+            const int64_t i = sl[first + q];
+            if (q != warp) s0 = load_stored(P.st, P.dts, i);
             double o[NOUT];
 #pragma unroll
             for (int c = 0; c < NOUT; ++c) {
                 double sum = 0.0;
-                const double* src = P.part + ((int64_t)c * ni + q) * G;
+                const double* src = P.part + ((int64_t)c * ni + first + q) * G;
                 for (int g = lane; g < G; g += 32) sum += ldcg(src + g);
 #pragma unroll
                 for (int w = 16; w >= 1; w >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, w);
@@ -205,11 +285,13 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             }
             if (lane == 0) {
 #pragma unroll
-                for (int c = 0; c < NOUT; ++c) P.out[(int64_t)c * ni + q] = o[c];
-                correct_one(P.st, P.dts, i, t1, o, o + 3, P.eta, P.dt_min, P.dt_max, P.err);
+                for (int c = 0; c < NOUT; ++c) P.out[(int64_t)c * ni + first + q] = o[c];
+                const double d = correct_stored(P.st, P.dts, i, s0, t1, o, o + 3, P.eta, P.dt_min, P.dt_max, P.err);
+                // the particle's new key; after a refused correction (zero step) the store is unchanged
+                if (cached) keys[i - lo] = key_of((t1 - s0.t != 0.0 ? t1 : s0.t) + d);
             }
         }
-        __syncthreads();                      // the new (t, dt) of my slice are visible to my next scan
+        __syncthreads();                      // the new keys / (t, dt) of my slice are visible to my next scan
         last_ni = ni64;
     }
     if (b == 0 && tid == 0) {
@@ -224,22 +306,20 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
 
 cudaError_t steps_kernel_setup(int* blocks_per_sm)
 {
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, steps_kernel, ST_THREADS, 0);
+    cudaError_t e = cudaFuncSetAttribute(steps_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ST_SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, steps_kernel, ST_THREADS, ST_SMEM);
 }
 
-// meta[0] (min key of step 0) and meta[2] (its counter) are preset here; the kernel resets the slots
-// of the other parity itself.  Grid: one CTA per SM, fewer when the set is small.
+// Grid: one CTA per SM, fewer when the set is small (at least 64 particles per slice).
 cudaError_t launch_steps(const StepsArgs& a, int sm_count, cudaStream_t s)
 {
-    const unsigned long long init[4] = {~0ull, ~0ull, 0ull, 0ull};
-    cudaError_t e = cudaMemcpyAsync(a.meta, init, sizeof(init), cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return e;
     int64_t want = (a.n + 63) / 64;
-    int grid = sm_count;
+    int grid = sm_count < ST_GMAX ? sm_count : ST_GMAX;
     if (want < grid) grid = (int)(want > 0 ? want : 1);
     StepsArgs copy = a;
     void* args[] = {(void*)&copy};
-    return cudaLaunchCooperativeKernel((const void*)steps_kernel, dim3(grid), dim3(ST_THREADS), args, 0, s);
+    return cudaLaunchCooperativeKernel((const void*)steps_kernel, dim3(grid), dim3(ST_THREADS), args, ST_SMEM, s);
 }
 
 }  // namespace nb

@@ -56,10 +56,10 @@ def _oracle_steps(k, m, x, v, a, j, t, dt, eps2, eta, lo, hi, flags=None):
     return np.array(log_t), np.array(log_ni), last
 
 
-@pytest.mark.parametrize("n", [1, 2, 200, 256])
+@pytest.mark.parametrize("n", [1, 2, 200, 512])
 def test_steps_all_in_kernel_match_oracle(nbmod, n):
-    """Every block fits the persistent kernel (bound lifted, n <= 256).  The 80 steps pass t = 2^-6,
-    where every particle is due at once (block of n: two j-strides per particle at n = 256)."""
+    """Every block fits the persistent kernel (bound lifted, n <= 512).  The 80 steps pass t = 2^-6,
+    where every particle is due at once (a block of n: one thread per due particle at n = 512)."""
     eps2, eta, lo, hi = 2.0 ** -10, 0.02, 2.0 ** -12, 2.0 ** -6
     m, x, v, a, j, t, dt = _start(n, 900 + n, eps2, eta, lo, hi)
     if n == 1:
@@ -77,7 +77,7 @@ def test_steps_all_in_kernel_match_oracle(nbmod, n):
             assert np.array_equal(gt, rt), (gt, rt)
             assert np.array_equal(gni, rni), (gni, rni)
             g = ctx.state().cpu().numpy()
-            small = rni.max() <= 256
+            small = rni.max() <= 512
             tol = 1e-11 if small else 1e-7
             assert np.array_equal(g[13], t)
             assert np.abs(g[1:4] - x).max() <= tol and np.abs(g[4:7] - v).max() <= tol * 10
@@ -148,7 +148,33 @@ def test_steps_host_path_and_mixed(nbmod):
             if bound == 0:
                 assert launches >= 4 * k            # select, predict, pair, reduce, correct per block
             else:
-                small = int(((gni <= 256) & (gni * n <= bound)).sum())
+                small = int(((gni <= 512) & (gni * n <= bound)).sum())
                 print("mixed run: %d of %d blocks in the persistent kernel, %d launches" % (small, k, launches))
                 assert small > 0 and launches < 6 * (k - small) + 2 * (k - small) + 8
+        ctx.sync()
+
+
+def test_steps_slice_overflow_goes_to_host_path(nbmod):
+    """More than 128 due particles inside ONE slice of the persistent kernel (N = 30000: 148 slices of
+    203): the slice cannot publish them all, the block must be handed to the host path, not truncated.
+    And the device time log adds up."""
+    n, eps2, eta, lo, hi = 30000, 2.0 ** -12, 0.02, 2.0 ** -16, 2.0 ** -6
+    m, x, v = nbgen.plummer(n, 990)
+    il = np.arange(n, dtype=np.int32)
+    a, j, _ = oracle.force(m, x, v, il, eps2)
+    t = np.zeros(n)
+    dt = np.full(n, hi)
+    dt[1000:1150] = lo                      # 150 consecutive particles due first, in one slice
+    dt[20000] = 2 * lo
+    with nbmod.Context(n) as ctx:
+        _load(ctx, m, x, v, a, j, t, dt)
+        done, gt, gni, us = ctx.steps(3, eps2, eta, lo, hi, times=True)
+        rt, rni, _ = _oracle_steps(3, m, x, v, a, j, t, dt, eps2, eta, lo, hi)
+        assert done == 3 and np.array_equal(gt, rt) and np.array_equal(gni, rni), (gt, gni, rt, rni)
+        assert rni[0] == 150
+        g = ctx.state().cpu().numpy()
+        assert np.array_equal(g[13], t)
+        assert np.abs(g[1:4] - x).max() < 1e-9 and np.abs(g[4:7] - v).max() < 1e-7
+        assert (us > 0).all() and us.sum() < 1e6
+        print("device time per step (us):", us)
         ctx.sync()
