@@ -57,9 +57,25 @@ def parse():
     ap.add_argument("--fp64", action="store_true",
                     help="run the step with the full-double pair loop (nb_set_precision 1); the roofline "
                          "is then the FP64 pipe (64 lanes per SM per clock)")
+    ap.add_argument("--order6", action="store_true",
+                    help="run the step with the 6th-order pair loop (nb_set_order 6 + nb_force6: acc, jerk, snap, "
+                         "pot; 64 FP32 lane-operations per interaction instead of 33)")
+    ap.add_argument("--predict", action="store_true",
+                    help="instead of the default line: the Hermite predictor alone against the HBM roofline "
+                         "(config 5's N = 2^22 + 11, and N = 2^20 alternating between two contexts)")
+    ap.add_argument("--shard", default="i", choices=["i", "j"],
+                    help="multi-GPU decomposition: i = active list sharded, j replicated (default); j = the paper's "
+                         "scheme (PAPER.md:55): j sharded, every rank evaluates all active particles by value "
+                         "against its slice, one all_reduce of [7][N_i]")
     ap.add_argument("--kick", action="store_true",
                     help="instead of the default line: time nb_force_ext on config 4's two galaxies "
                          "(stars of B by value against galaxy A as j-set), with jerk and acc + pot only")
+    ap.add_argument("--steps-bound", type=float, default=-1.0,
+                    help="with --blockstep: largest N_i x N the persistent kernel of nb_steps takes itself")
+    ap.add_argument("--detail", action="store_true", help="with --blockstep: add the per-step sizes and device times")
+    ap.add_argument("--fewi", action="store_true",
+                    help="instead of the default line: the force call for a handful of active particles "
+                         "(N_i = 1..64 of config 3, N = 2^20), nb_force and nb_force_fused, against the HBM roofline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target duration of the cpu_baseline sample")
     return ap.parse_args()
@@ -268,9 +284,13 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.shard == "j":
+        return run_shard_j(args, case, il, t, workload, rank, world, local, dev)
     ctx = nbm.Context(n, max(ni, 1), device=local)
     if args.fp64:
         ctx.precision(1)
+    if args.order6:
+        ctx.order(6)
     ctx.load_case(case)
     h = ctx.h
     # device-resident step inputs: the active list and the active particles' corrected state (here:
@@ -282,11 +302,15 @@ def run_ours(args):
     acc = torch.empty((3, ni_loc), dtype=torch.float64, device=dev)
     jrk = torch.empty((3, ni_loc), dtype=torch.float64, device=dev)
     pot = torch.empty((ni_loc,), dtype=torch.float64, device=dev)
+    snp = torch.empty((3, ni_loc), dtype=torch.float64, device=dev) if args.order6 else None
 
     def step():
         nb.nb_update_j(h, d_il_full, ni, *upd)                     # a0
         nb.nb_predict(h, t)                                        # a1
-        nb.nb_force(h, d_il, ni_loc, case.eps2, acc, jrk, pot)     # a2..a5
+        if args.order6:
+            nb.nb_force6(h, d_il, ni_loc, case.eps2, acc, jrk, snp, pot)
+        else:
+            nb.nb_force(h, d_il, ni_loc, case.eps2, acc, jrk, pot) # a2..a5
         if world > 1:
             return sharding.gather_forces(acc, jrk, pot, ni)
         return acc, jrk, pot
@@ -326,7 +350,7 @@ def run_ours(args):
 
     # ---- e2e: the same step through the HOST-buffer entry points of the C-ABI -----------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.order6:
         def pin(a):
             return torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         h_il_full, h_il = pin(il), pin(il_loc)
@@ -348,7 +372,17 @@ def run_ours(args):
         ms_h = timed(step_host, args.steps)
         wall = time.perf_counter() - w0
         assert bool(torch.isfinite(h_pot).all())
+        # the timed host path against the device-resident result of the same step: bit for bit (the
+        # reduction order is fixed, R9); a sample of 256 active particles spread over the list
+        samp = np.unique(np.linspace(0, ni_loc - 1, 256).astype(np.int64))
+        d_samp = torch.from_numpy(samp).to(dev)
+        same = (np.array_equal(h_acc.numpy()[:, samp], acc[:, d_samp].cpu().numpy()) and
+                np.array_equal(h_jrk.numpy()[:, samp], jrk[:, d_samp].cpu().numpy()) and
+                np.array_equal(h_pot.numpy()[samp], pot[d_samp].cpu().numpy()))
+        assert same, "host-buffer path and device-resident path disagree"
         e2e = {"value": float(ni) * n * args.steps / (ms_h * 1e-3), "unit": "interactions/s",
+               "checked": "%d sampled i: outputs of the timed host-buffer path are bit-identical to the "
+                          "device-resident step's (which tests/test_gpu_configs.py checks against the oracle)" % len(samp),
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": ms_h / args.steps, "wall_ms_per_step": wall / args.steps * 1e3,
                "api": "nb_update_j_host + nb_predict + nb_force_host (pinned host buffers)"}
@@ -479,6 +513,8 @@ def run_blockstep(args):
         block (five launches + a synchronisation each), "steps" = one nb_steps call (persistent
         kernel; the host sees only the blocks above the bound)."""
         with nbm.Context(n) as ctx:
+            if args.steps_bound >= 0:
+                ctx.steps_bound(int(args.steps_bound))
             ctx.set_j(m, x, v)
             ctx.predict(0.0)
             ga, gj, gp = ctx.force(il, eps2)
@@ -512,7 +548,7 @@ def run_blockstep(args):
     ms_step, _, launches_step, _, _ = min((r for md, r in runs if md == "step"), key=lambda r: r[0])
     ms, wall, launches, sizes, t = min((r for md, r in runs if md == "steps"), key=lambda r: r[0])
     sizes = np.array(sizes, dtype=np.float64)
-    small = (sizes <= 512) & (sizes * n <= 3.0e7)
+    small = (sizes <= 512) & (sizes * n <= (args.steps_bound if args.steps_bound >= 0 else 3.0e7))
     in_kernel = int(small.sum())
     us = np.minimum(times[0], times[1])                    # per-step device time (%globaltimer), best of 2
     floor_us = sizes * n / 1.2408e12 * 1e6                  # pair work at 100 % of the FP32 peak
@@ -540,6 +576,83 @@ def run_blockstep(args):
                    "launches_per_block_nb_steps": launches / args.steps,
                    "note": "same process, same start and schedule, best of 2 each, interleaved"},
             "gpu_launches": int(launches)}
+    if args.detail:
+        line["steps_detail"] = {"n_i": [int(q) for q in sizes], "us": [float(q) for q in us]}
+    print(json.dumps(line))
+    return 0
+
+
+def run_fewi(args):
+    """a handful of active particles.  The call then streams the predicted j-set once
+    (44 B per particle, nb_force) or the whole j-store (112 B, nb_force_fused, predictor inside) and
+    is bound by HBM and launch latency, not by FP32: reported against the measured copy bandwidth."""
+    import numpy as np
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    import nbgen
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import binding as nb
+    peaks = measured_peaks()
+    case, il_all, t, workload = make_case(args.workload)
+    n = case.n
+    dev = torch.device("cuda", 0)
+    rows = []
+    with nbm.Context(n, 1 << 10) as ctx:
+        ctx.load_case(case)
+        h = ctx.h
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > L2: evicts the pack / store
+        for ni in (1, 2, 4, 8, 16, 64):
+            d_il = torch.from_numpy(np.ascontiguousarray(il_all[:ni])).to(dev)
+            o = [torch.empty((3, ni), dtype=torch.float64, device=dev),
+                 torch.empty((3, ni), dtype=torch.float64, device=dev),
+                 torch.empty((ni,), dtype=torch.float64, device=dev)]
+            for name in ("nb_force", "nb_force_fused"):
+                if name == "nb_force_fused" and ni > nb.NB_FUSED_MAX:
+                    continue
+                if name == "nb_force":
+                    nb.nb_predict(h, t)
+                    call = lambda: nb.nb_force(h, d_il, ni, case.eps2, *o)
+                    nbytes = 44.0 * n
+                else:
+                    call = lambda: nb.nb_force_fused(h, t, d_il, ni, case.eps2, *o)
+                    nbytes = 112.0 * n
+                for _ in range(5):
+                    call()
+                ctx.sync()
+                # (a) back to back, the j data resident in L2 as far as it fits; (b) every call after an
+                # L2 flush, timed alone with events around the call
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                reps = 200
+                e0.record()
+                for _ in range(reps):
+                    call()
+                e1.record()
+                ctx.sync()
+                warm = e0.elapsed_time(e1) / reps * 1e3
+                cold = []
+                for _ in range(20):
+                    flush.fill_(1)
+                    e0.record()
+                    call()
+                    e1.record()
+                    ctx.sync()
+                    cold.append(e0.elapsed_time(e1) * 1e3)
+                cold_us = float(np.median(cold))
+                info = ctx.last_launch()
+                rows.append({"call": name, "n_i": ni, "us_per_call_back_to_back": warm, "us_per_call_after_l2_flush": cold_us,
+                             "bytes_per_call": nbytes, "gbs_after_flush": nbytes / cold_us / 1e3,
+                             "hbm_frac": nbytes / cold_us / 1e3 / peaks["hbm_gbs"],
+                             "gbs_back_to_back": nbytes / warm / 1e3,
+                             "kernels": int(info["kernels"]), "ctas": int(info["ctas"])})
+    best = max(r["hbm_frac"] for r in rows if r["n_i"] == 1)
+    line = {"metric": "GB/s of the j data streamed by one few-i force call", "value": best * peaks["hbm_gbs"],
+            "unit": "GB/s", "n_gpus": 1, "steps": 200, "warmup": 5, "higher_is_better": True, "dtype": "f32/f64",
+            "data": "synthetic", "config": {"workload": workload + "_few_i", "n_j": n,
+                                            "l2": "hbm_frac rows: the L2 is flushed (256 MB fill) before every timed call"},
+            "roofline": {"bound": "hbm", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "unit": "GB/s",
+                         "achieved": best * peaks["hbm_gbs"], "frac": best, "traffic": None},
+            "rows": rows}
     print(json.dumps(line))
     return 0
 
@@ -602,6 +715,8 @@ def main():
         return run_reference(args)
     if args.kick:
         return run_kick(args)
+    if args.fewi:
+        return run_fewi(args)
     if args.blockstep > 0:
         return run_blockstep(args)
     return run_ours(args)

@@ -163,6 +163,18 @@ int nb_force(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
 int nb_force_ext(nb_ctx* c, int64_t ni, const double* x, const double* v, double eps2, double* acc,
                  double* jrk, double* pot);
 
+/* nb_force_ext for i-particles that may be MEMBERS of this context's j-set although they are given by
+ * value -- the call one GPU makes in the paper's multi-GPU scheme, "distributing the j particles over
+ * the various GPUs": every GPU evaluates ALL active particles, received by value,
+ * against its own slice of j, and the partial forces are summed afterwards.  self_idx[k] (DEVICE
+ * int32) = index in THIS context's j-set of the particle that IS i-particle k, or negative if it
+ * belongs to another slice: that pair is excluded by index (R5), exactly as in nb_force.  iflags[k]
+ * (DEVICE uint8, may be NULL) bit 0 = i-particle k carries the unsoftened flag: its pairs with the
+ * flagged members of this j-set are unsoftened (R7) and summed in fp64.  x and v are the predicted
+ * state at the time of the last nb_predict.  Everything else as nb_force_ext with velocities. */
+int nb_force_ext_ids(nb_ctx* c, int64_t ni, const double* x, const double* v, const int32_t* self_idx,
+                     const uint8_t* iflags, double eps2, double* acc, double* jrk, double* pot);
+
 /* Forces at time t on a HANDFUL of members of the j-set (ni <= NB_FUSED_MAX), in one pass over the
  * j-store: the Hermite predictor (R1) runs inside the pair loop, for i and j alike, instead of as a
  * separate nb_predict pass (PAPER.md:55 counts the prediction step among the costs of a step;
@@ -194,6 +206,20 @@ int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,
  * (NB_ERR_STATE otherwise).  The atomics reduce mode and the threads-per-i variants are mode-0
  * only; results of mode 1 are deterministic. */
 int nb_set_precision(nb_ctx* c, int mode);
+
+/* 6th-order variant ("high >= 4th order integrators").  With
+ * order = 6 the predictor also writes force-ready records that carry the predicted acceleration
+ * ap = a + jerk dt (R22; 56 B more per particle, cudaMalloc'ed by this call), and nb_force6 returns the
+ * second time derivative of the acceleration ("snap") next to acc, jerk and pot:
+ *     b = ap_j - ap_i ,  al = (r.w)/s ,  be = (w.w + r.b)/s + al^2
+ *     snp_i = sum m_j ( b s^-3/2 - 6 al J_ij - 3 be A_ij ),  A_ij = r s^-3/2,  J_ij = w s^-3/2 - 3 al A_ij
+ * i.e. d2(acc)/dt2 along orbits with the given relative position, velocity and acceleration.  Same
+ * pair rules (R5, R6, R7), precision scheme, layout ([3][ni] for snp) and errors as nb_force; snp
+ * agrees with exact summation to <= 1e-3 relative.  order = 4 (default) switches the extra records
+ * off.  Changing the order invalidates the predicted state.  nb_force6 is NB_ERR_STATE at order 4. */
+int nb_set_order(nb_ctx* c, int order);
+int nb_force6(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc, double* jrk, double* snp,
+              double* pot);
 
 /* Force-call tuning, for tests and experiments.  j_splits: 0 = let the dispatcher choose the
  * number of j-subsets, >0 = use exactly this many (clamped to what the partial

@@ -17,7 +17,7 @@ NB_MAX_FLAGGED = 1024
 EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
-    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_precision", "nb_set_tuning",
+    "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_ext_ids", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_order", "nb_force6", "nb_set_precision", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_steps", "nb_set_steps_bound", "nb_block_forces", "nb_strerror", "nb_version",
 ]
@@ -50,6 +50,8 @@ for _f in (lib.nb_force, lib.nb_force_host):
     _f.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _vp]
 lib.nb_set_tuning.argtypes = [_vp, _i32, _i32]
 lib.nb_set_precision.argtypes = [_vp, _i32]
+lib.nb_set_order.argtypes = [_vp, _i32]
+lib.nb_force6.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _vp, _vp]
 lib.nb_last_launch.argtypes = [_vp, ctypes.POINTER(_i64)]
 lib.nb_launch_count.argtypes = [_vp]
 lib.nb_launch_count.restype = _i64
@@ -61,6 +63,7 @@ lib.nb_strerror.restype = ctypes.c_char_p
 lib.nb_force_fused.argtypes = [_vp, _dbl, _vp, _i64, _dbl, _vp, _vp, _vp]
 lib.nb_set_fused.argtypes = [_vp, _i32]
 lib.nb_force_ext.argtypes = [_vp, _i64, _vp, _vp, _dbl, _vp, _vp, _vp]
+lib.nb_force_ext_ids.argtypes = [_vp, _i64, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]
 lib.nb_set_dt.argtypes = [_vp, _i64, _i64, _vp]
 lib.nb_get_state.argtypes = [_vp, _i64, _i64, _vp]
 lib.nb_init_steps.argtypes = [_vp, _vp, _i64, _vp, _vp, _dbl, _dbl, _dbl]
@@ -227,6 +230,21 @@ def nb_set_fused(c, on):
 def nb_force_ext(c, ni, x, v, eps2, acc, jrk, pot):
     """DEVICE x, v (3, ni) fp64 (v and jrk both None: acc + pot only)."""
     _check(lib.nb_force_ext(c, ni, _ptr(x), _ptr(v), eps2, _ptr(acc), _ptr(jrk), _ptr(pot)), "nb_force_ext")
+
+
+def nb_force_ext_ids(c, ni, x, v, self_idx, iflags, eps2, acc, jrk, pot):
+    """DEVICE x, v (3, ni) fp64, self_idx int32 (ni,), iflags uint8 (ni,) or None."""
+    _check(lib.nb_force_ext_ids(c, ni, _ptr(x), _ptr(v), _ptr(self_idx), _ptr(iflags), eps2, _ptr(acc), _ptr(jrk),
+                                _ptr(pot)), "nb_force_ext_ids")
+
+
+def nb_set_order(c, order):
+    _check(lib.nb_set_order(c, int(order)), "nb_set_order")
+
+
+def nb_force6(c, i_list, ni, eps2, acc, jrk, snp, pot):
+    """DEVICE: i_list int32 (ni,); outputs acc, jrk, snp fp64 (3, ni), pot fp64 (ni,)."""
+    _check(lib.nb_force6(c, _ptr(i_list), ni, float(eps2), _ptr(acc), _ptr(jrk), _ptr(snp), _ptr(pot)), "nb_force6")
 
 
 def nb_set_precision(c, mode):

@@ -86,6 +86,19 @@ class Context:
         self._keep_i = il
         return acc, jrk, pot
 
+    def order(self, order):
+        """4 (default) or 6: the predictor then also writes the records nb_force6 streams."""
+        nb.nb_set_order(self.h, order)
+
+    def force6(self, i_list, eps2):
+        il = self._dev(i_list, torch.int32)
+        ni = il.shape[0]
+        out = [torch.empty((3, ni), dtype=torch.float64, device=self.device) for _ in range(3)]
+        pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
+        nb.nb_force6(self.h, il, ni, eps2, out[0], out[1], out[2], pot)
+        self._keep_i = il
+        return out[0], out[1], out[2], pot
+
     def precision(self, mode):
         """0 = mixed (48-bit differences, fp32 pair terms), 1 = IEEE double throughout."""
         nb.nb_set_precision(self.h, mode)
@@ -139,6 +152,19 @@ class Context:
         pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
         nb.nb_force_ext(self.h, ni, dx, dv, eps2, acc, jrk, pot)
         self._keep = [dx, dv]
+        return acc, jrk, pot
+
+    def force_ext_ids(self, x, v, self_idx, iflags, eps2):
+        """By value, with the index of the j-set member each i-particle is (or -1) and its flag."""
+        dx, dv = self._dev(x), self._dev(v)
+        ds = self._dev(self_idx, torch.int32)
+        df = self._dev(iflags, torch.uint8) if iflags is not None else None
+        ni = dx.shape[1]
+        acc = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        jrk = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
+        nb.nb_force_ext_ids(self.h, ni, dx, dv, ds, df, eps2, acc, jrk, pot)
+        self._keep = [dx, dv, ds, df]
         return acc, jrk, pot
 
     # -- block-step layer (marshalling only) --------------------------------------------------

@@ -20,13 +20,27 @@ __device__ __forceinline__ double of_key(unsigned long long k)
 
 __device__ __forceinline__ double norm3(double x, double y, double z) { return sqrt(x * x + y * y + z * z); }
 
+// Is t1 a multiple of p (p > 0)?  Steps are powers of two, so t1 / p is exact and the answer is
+// "the quotient is an integer" -- the same truth value as fmod(t1, p) == 0 without its long loop;
+// any other p (a step the caller set by hand) takes fmod.
+__device__ __forceinline__ bool is_multiple(double t1, double p)
+{
+    const long long pb = __double_as_longlong(p);
+    const int e = (int)(pb >> 52);            // biased exponent (p > 0: no sign bit)
+    if ((pb & 0x000fffffffffffffll) == 0 && e > 523 && e < 1523) {      // 2^-500 < p = 2^k < 2^500
+        const double q = t1 * __longlong_as_double(0x7fe0000000000000ll - pb);   // t1 * 2^-k, exact
+        return q == rint(q) && fabs(q) < __longlong_as_double(0x7ff0000000000000ll);
+    }
+    return fmod(t1, p) == 0.0;
+}
+
 // R20: new power-of-two step after a step of d_old that ended at t1, given the wanted step w
 __device__ __forceinline__ double block_rule(double d, double w, double t1, double dt_min, double dt_max)
 {
     d = d < dt_min ? dt_min : d;      // a step that was never set (0) must not stay below the grid
     if (w < d) {
         while (d > w && d * 0.5 >= dt_min) d *= 0.5;
-    } else if (w >= 2.0 * d && 2.0 * d <= dt_max && fmod(t1, 2.0 * d) == 0.0) {
+    } else if (w >= 2.0 * d && 2.0 * d <= dt_max && is_multiple(t1, 2.0 * d)) {
         d *= 2.0;
     }
     return d;

@@ -1,6 +1,7 @@
 // nb_api.cu -- the C-ABI of include/nb.h: context, argument checks, host dispatcher.
 #include <math.h>
 #include <new>
+#include <stdio.h>
 #include <string.h>
 #include <vector>
 
@@ -12,7 +13,8 @@ struct nb_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     int64_t n_max = 0, ni_max = 0, n_cap = 0, n = 0;
-    int sm_count = 148, blocks_per_sm = 1, blocks_per_sm_guard = 1;
+    int sm_count = 148;
+    int blocks_per_sm[4] = {1, 1, 1, 1};   // all-i kernel, its guarded form, few-i kernel, its guarded form
 
     // device memory: either one cudaMalloc'ed slab or the caller's workspace
     bool allocated = false, own_slab = false;
@@ -27,6 +29,7 @@ struct nb_ctx {
     double* part = nullptr;
     size_t part_bytes = 0;
     int* err = nullptr;
+    unsigned* ticket = nullptr;         // the few-i kernel's reduction ticket (zero between calls)
     int32_t* h_ilist = nullptr;   // device staging for the *_host force call
     double* h_out = nullptr;      // [7][ni_max]
     double* h_in = nullptr;       // [14][ni_pad] staging of nb_update_j_host
@@ -53,6 +56,11 @@ struct nb_ctx {
     int precision = 0;
     double* pack64 = nullptr;
     int blocks_per_sm64 = 1;
+
+    // 6th-order pair loop (force6.cu): tiles with the predicted acceleration, allocated when selected
+    int order = 4;
+    float* pack6 = nullptr;
+    int blocks_per_sm6 = 1;
 
     int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy; 32..63: nb_steps status
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
@@ -117,7 +125,7 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.part_bytes = (size_t)NOUT * sizeof(double) * (size_t)ni_pad * 4;
     if (L.part_bytes < ((size_t)32 << 20)) L.part_bytes = (size_t)32 << 20;
     L.part = off; off += up(L.part_bytes);
-    L.err = off; off += up(sizeof(int));
+    L.err = off; off += up(2 * sizeof(int));           // error latch, reduction ticket
     L.ilist = off; off += up((size_t)ni_pad * 4);
     L.out = off; off += up((size_t)NOUT * ni_pad * sizeof(double));
     L.in = off; off += up((size_t)NFIELD * ni_pad * sizeof(double));
@@ -160,6 +168,7 @@ int ensure_alloc(nb_ctx* c)
     c->part = reinterpret_cast<double*>(c->slab + L.part);
     c->part_bytes = L.part_bytes;
     c->err = reinterpret_cast<int*>(c->slab + L.err);
+    c->ticket = reinterpret_cast<unsigned*>(c->slab + L.err) + 1;
     c->h_ilist = reinterpret_cast<int32_t*>(c->slab + L.ilist);
     c->h_out = reinterpret_cast<double*>(c->slab + L.out);
     c->h_in = reinterpret_cast<double*>(c->slab + L.in);
@@ -272,9 +281,11 @@ int choose_splits(nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad, size_t pa
     return ans;
 }
 
-// ext_x != NULL: i-particles by value (nb_force_ext); ext_v == NULL then means acc + pot only
+// ext_x != NULL: i-particles by value (nb_force_ext); ext_v == NULL then means acc + pot only;
+// ext_self / ext_flags: which member of the j-set each one is, and its flag (nb_force_ext_ids)
 int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc, double* jrk,
-               double* pot, const double* ext_x = nullptr, const double* ext_v = nullptr)
+               double* pot, const double* ext_x = nullptr, const double* ext_v = nullptr,
+               const int32_t* ext_self = nullptr, const uint8_t* ext_flags = nullptr)
 {
     const int kmode = ext_x ? (ext_v ? 1 : 2) : 0;
     const bool f64 = c->precision == 1;
@@ -282,11 +293,14 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     c->last[0] = c->last[1] = c->last[2] = 0;
     if (ni == 0) return NB_OK;
     const int64_t n_launch = c->n > 0 ? c->n : 0;
+    const bool ids = kmode == 1 && ext_self != nullptr;
     ForceArgs a{};
     a.pack = c->pack;
     a.i_list = i_list;
     a.ext_x = ext_x;
     a.ext_v = ext_v;
+    a.ext_self = ext_self;
+    a.ext_flags = ext_flags;
     a.flags = c->flags;
     a.tileflag = c->tileflag;
     a.err = c->err;
@@ -294,16 +308,20 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     a.n = (int)n_launch;
     a.ntiles = (int)((n_launch + TJ - 1) / TJ);
     a.eps2 = (float)eps2;
-    a.any_flagged = (c->flagged.empty() || kmode != 0) ? 0 : 1;
+    a.any_flagged = (c->flagged.empty() || !(kmode == 0 || ids)) ? 0 : 1;
     a.pack64 = c->pack64;
     a.eps2d = eps2;
     const int mode = (c->tune_reduce && kmode == 0 && !f64) ? 1 : 0;
-    // few active i: several threads share one i-particle and split the j of a tile
-    const int jl = f64 ? 1 : (ni <= ITILE / JL_MAX ? JL_MAX : (ni <= ITILE / JL_MID ? JL_MID : 1));
-    const int itile = ITILE / jl;
+    // few active i: 2, 4, .. 32 threads share one i-slot and split the j of a tile, so
+    // that one CTA's 256 slots hold the smallest power of two >= ni particles (down to 8)
+    int jsh = 0;
+    if (!f64)
+        while (jsh < JSH_MAX && (ITILE >> (jsh + 1)) >= ni) ++jsh;
+    a.jsh = jsh;
+    const int itile = ITILE >> jsh;
     const int n_itiles = (int)((ni + itile - 1) / itile);
-    const int resident = c->sm_count * (f64 ? c->blocks_per_sm64
-                                            : ((float)eps2 < EPS2_GUARD ? c->blocks_per_sm_guard : c->blocks_per_sm));
+    const bool guard = (float)eps2 < EPS2_GUARD;
+    const int resident = c->sm_count * (f64 ? c->blocks_per_sm64 : c->blocks_per_sm[(jsh > 0 ? 2 : 0) + (guard ? 1 : 0)]);
 
     // the i-tiles are cut in two segments.  A = the largest multiple of the resident CTA
     // count, one j-subset each (whole waves of equal CTAs); B = the rest, whose j is split in S
@@ -313,45 +331,12 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     int splits_a = tiles_a > 0 ? 1 : 0, splits_b = 0;
     const int64_t pad_a = (int64_t)tiles_a * itile, pad_b = (int64_t)tiles_b * itile;
     double* part_b = c->part + (size_t)NOUT * pad_a;
-    int launched = 0;
-    nb_ctx::Rec* rec = nullptr;
-    if (a.ntiles > 0) {
-        if (tiles_b > 0) {
-            const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a;
-            splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left, resident);
-        }
-        if (mode) {
-            if (launch_zero_out(acc, jrk, pot, ni, c->stream) != cudaSuccess) return NB_ERR_CUDA;
-            ++launched;
-        }
-        rec = prof_next(c);
-        if (rec) cudaEventRecord(rec->e[0], c->stream);
-        if (tiles_a > 0) {
-            a.k0 = 0;
-            a.n_itiles = tiles_a;
-            a.ni_pad = (int)pad_a;
-            a.splits = 1;
-            a.part = c->part;
-            if ((f64 ? launch_force64(a, kmode, c->stream)
-                     : launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
-                return NB_ERR_CUDA;
-            ++launched;
-        }
-        if (tiles_b > 0) {
-            a.k0 = (int)pad_a;
-            a.n_itiles = tiles_b;
-            a.ni_pad = (int)pad_b;
-            a.splits = splits_b;
-            a.part = part_b;
-            if ((f64 ? launch_force64(a, kmode, c->stream)
-                     : launch_force(a, jl, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
-                return NB_ERR_CUDA;
-            ++launched;
-        }
-        if (rec) cudaEventRecord(rec->e[1], c->stream);
-    } else {
-        splits_a = splits_b = 0;   // n == 0: the reduction of zero partials writes zeros
+    if (a.ntiles > 0 && tiles_b > 0) {
+        const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a;
+        splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left, resident);
     }
+    if (a.ntiles == 0) splits_a = splits_b = 0;   // n == 0: the reduction of zero partials writes zeros
+
     ReduceArgs r{};
     r.part = c->part;
     r.part_b = part_b;
@@ -365,20 +350,99 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     r.store = c->store;
     r.flags = c->flags;
     r.flag_list = c->flag_list;
-    r.nflag = f64 ? 0 : (int)c->flagged.size();      // the fp64 kernel handles flagged pairs itself
+    // the fp64 kernel handles flagged pairs itself; by-value calls have them only with ids
+    r.nflag = (f64 || !(kmode == 0 || ids)) ? 0 : (int)c->flagged.size();
     r.ni = (int)ni;
     r.ni_pad = (int)pad_a;
     r.splits = splits_a;
     r.n = (int)n_launch;
     r.t_pred = c->t_pred;
     r.atomic_mode = (mode && a.ntiles > 0) ? 1 : 0;
-    if (launch_reduce(r, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    r.ext_x = ext_x;
+    r.ext_v = ext_v;
+    r.ext_self = ext_self;
+    r.ext_flags = ext_flags;
+    r.counter = c->ticket;
+    // a handful of i: the few-i kernel's last CTA also reduces, the call is one launch
+    const bool reduce_here = jsh > 0 && !mode && !f64 && a.ntiles > 0 && tiles_a == 0 && ni <= 16;
+    a.reduce_here = reduce_here ? 1 : 0;
+
+    int launched = 0;
+    nb_ctx::Rec* rec = nullptr;
+    // a handful of members of the j-set: the direct kernel (direct.cu) streams the pack once, one
+    // launch; it keeps whole per-thread sums in fp32, so only while they stay within R17's 64 terms
+    if (kmode == 0 && !f64 && !mode && c->tune_splits == 0 && ni <= DIRECT_NI_MAX && a.ntiles > 0) {
+        const int grid = direct_grid(a.ntiles, c->sm_count);
+        if (direct_terms_per_lane(a.ntiles, grid) <= 64) {
+            const int nip = ni <= 1 ? 1 : (ni <= 2 ? 2 : (ni <= 4 ? 4 : 8));
+            a.jsh = 0;
+            a.k0 = 0;
+            a.n_itiles = 1;
+            a.ni_pad = nip;
+            a.splits = grid;
+            a.part = c->part;
+            r.part = c->part;
+            r.part_b = c->part;
+            r.kA = (int)ni;
+            r.ni_pad = nip;
+            r.splits = grid;
+            rec = prof_next(c);
+            if (rec) cudaEventRecord(rec->e[0], c->stream);
+            if (launch_direct(a, r, grid, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            if (rec) {
+                cudaEventRecord(rec->e[1], c->stream);
+                cudaEventRecord(rec->e[2], c->stream);
+                rec->kind = 1;
+                c->ring_used += 1;
+            }
+            c->last[0] = grid;
+            c->last[1] = grid;
+            c->last[2] = 1;
+            c->last[3] = 0;
+            c->launches += 1;
+            return NB_OK;
+        }
+    }
+    if (a.ntiles > 0) {
+        if (mode) {
+            if (launch_zero_out(acc, jrk, pot, ni, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+            ++launched;
+        }
+        rec = prof_next(c);
+        if (rec) cudaEventRecord(rec->e[0], c->stream);
+        if (tiles_a > 0) {
+            a.k0 = 0;
+            a.n_itiles = tiles_a;
+            a.ni_pad = (int)pad_a;
+            a.splits = 1;
+            a.part = c->part;
+            if ((f64 ? launch_force64(a, kmode, c->stream)
+                     : launch_force(a, r, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
+                return NB_ERR_CUDA;
+            ++launched;
+        }
+        if (tiles_b > 0) {
+            a.k0 = (int)pad_a;
+            a.n_itiles = tiles_b;
+            a.ni_pad = (int)pad_b;
+            a.splits = splits_b;
+            a.part = part_b;
+            if ((f64 ? launch_force64(a, kmode, c->stream)
+                     : launch_force(a, r, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
+                return NB_ERR_CUDA;
+            ++launched;
+        }
+        if (rec) cudaEventRecord(rec->e[1], c->stream);
+    }
+    if (!reduce_here) {
+        if (launch_reduce(r, c->stream) != cudaSuccess) return NB_ERR_CUDA;
+        ++launched;
+    }
     if (rec) {
         cudaEventRecord(rec->e[2], c->stream);
         rec->kind = 1;
         c->ring_used += 1;
     }
-    ++launched;
     c->last[0] = tiles_b > 0 ? splits_b : splits_a;
     c->last[1] = (int64_t)tiles_a * splits_a + (int64_t)tiles_b * splits_b;
     c->last[2] = launched;
@@ -436,8 +500,8 @@ int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* str
     c->ni_max = ni_max;
     c->sm_count = prop.multiProcessorCount;
     DeviceGuard g(device);
-    if (force_kernel_setup(&c->blocks_per_sm, &c->blocks_per_sm_guard) != cudaSuccess || c->blocks_per_sm < 1 ||
-        c->blocks_per_sm_guard < 1) {
+    if (force_kernel_setup(c->blocks_per_sm) != cudaSuccess || c->blocks_per_sm[0] < 1 || c->blocks_per_sm[1] < 1 ||
+        c->blocks_per_sm[2] < 1 || c->blocks_per_sm[3] < 1) {
         cudaGetLastError();
         delete c;
         return NB_ERR_CUDA;
@@ -458,6 +522,7 @@ int nb_destroy(nb_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->own_slab && c->slab) cudaFree(c->slab);
     if (c->pack64) cudaFree(c->pack64);
+    if (c->pack6) cudaFree(c->pack6);
     if (c->steps_log_t) cudaFree(c->steps_log_t);
     if (c->steps_log_ni) cudaFree(c->steps_log_ni);
     if (c->steps_log_ns) cudaFree(c->steps_log_ns);
@@ -656,8 +721,8 @@ int nb_predict(nb_ctx* c, double t)
     if (rc != NB_OK) return rc;
     nb_ctx::Rec* rec = c->n > 0 ? prof_next(c) : nullptr;
     if (rec) cudaEventRecord(rec->e[0], c->stream);
-    if (launch_predict(c->store, c->flags, c->pack, c->precision == 1 ? c->pack64 : nullptr, c->n, t,
-                       c->stream) != cudaSuccess)
+    if (launch_predict(c->store, c->flags, c->pack, c->precision == 1 ? c->pack64 : nullptr,
+                       c->order == 6 ? c->pack6 : nullptr, c->n, t, c->stream) != cudaSuccess)
         return NB_ERR_CUDA;
     if (rec) {
         cudaEventRecord(rec->e[1], c->stream);
@@ -698,6 +763,15 @@ int nb_force_ext(nb_ctx* c, int64_t ni, const double* x, const double* v, double
     if ((v == nullptr) != (jrk == nullptr)) return NB_ERR_ARG;     // jerk needs velocities, and only then
     DeviceGuard g(c->device);
     return force_impl(c, nullptr, ni, eps2, acc, jrk, pot, x, v);
+}
+
+int nb_force_ext_ids(nb_ctx* c, int64_t ni, const double* x, const double* v, const int32_t* self_idx,
+                     const uint8_t* iflags, double eps2, double* acc, double* jrk, double* pot)
+{
+    if (!c || ni < 0 || ni > c->ni_max || !isfinite(eps2) || eps2 < 0.0) return NB_ERR_ARG;
+    if (ni > 0 && (!x || !v || !self_idx || !acc || !jrk || !pot)) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    return force_impl(c, nullptr, ni, eps2, acc, jrk, pot, x, v, self_idx, iflags);
 }
 
 int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc,
@@ -745,6 +819,67 @@ int nb_set_precision(nb_ctx* c, int mode)
     }
     c->precision = mode;
     c->predicted = false;      // the tiles of the new mode are written by the next nb_predict
+    return NB_OK;
+}
+
+int nb_set_order(nb_ctx* c, int order)
+{
+    if (!c || (order != 4 && order != 6)) return NB_ERR_ARG;
+    if (order == c->order) return NB_OK;
+    DeviceGuard g(c->device);
+    if (order == 6 && !c->pack6) {
+        int rc = ensure_alloc(c);
+        if (rc != NB_OK) return rc;
+        if (force6_kernel_setup(&c->blocks_per_sm6) != cudaSuccess || c->blocks_per_sm6 < 1) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        if (cudaMalloc(&c->pack6, (size_t)(c->n_cap / TJ) * TILE6_BYTES) != cudaSuccess) {
+            cudaGetLastError();
+            c->pack6 = nullptr;
+            return NB_ERR_ALLOC;
+        }
+    }
+    c->order = order;
+    c->predicted = false;      // the tiles of the new order are written by the next nb_predict
+    return NB_OK;
+}
+
+int nb_force6(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc, double* jrk, double* snp,
+              double* pot)
+{
+    if (!c || ni < 0 || ni > c->ni_max || !isfinite(eps2) || eps2 < 0.0) return NB_ERR_ARG;
+    if (ni > 0 && (!i_list || !acc || !jrk || !snp || !pot)) return NB_ERR_ARG;
+    if (c->order != 6 || !c->predicted) return NB_ERR_STATE;
+    if (ni == 0) return NB_OK;
+    DeviceGuard g(c->device);
+    const int64_t n_launch = c->n > 0 ? c->n : 0;
+    Force6Args a{};
+    a.pack6 = c->pack6;
+    a.i_list = i_list;
+    a.part = c->part;
+    a.flags = c->flags;
+    a.err = c->err;
+    a.ni = (int)ni;
+    a.n = (int)n_launch;
+    a.ntiles = (int)((n_launch + TJ - 1) / TJ);
+    a.n_itiles = (int)((ni + ITILE - 1) / ITILE);
+    a.ni_pad = a.n_itiles * ITILE;
+    a.eps2 = (float)eps2;
+    a.any_flagged = c->flagged.empty() ? 0 : 1;
+    // j split in subsets while the i-tiles alone do not fill the chip; 10 sums per i
+    const int resident = c->sm_count * c->blocks_per_sm6;
+    a.splits = 1;
+    if (a.ntiles > 0 && a.n_itiles < resident)
+        a.splits = choose_splits(c, a.n_itiles, a.ntiles, a.ni_pad, c->part_bytes * NOUT / 10, resident);
+    if (launch_force6(a, c->store, c->flag_list, (int)c->flagged.size(), c->t_pred, acc, jrk, snp, pot, c->stream) !=
+        cudaSuccess)
+        return NB_ERR_CUDA;
+    c->last[0] = a.splits;
+    c->last[1] = (int64_t)a.n_itiles * a.splits;
+    c->last[2] = 2;
+    c->last[3] = 0;
+    c->launches += 2;
     return NB_OK;
 }
 
@@ -1063,6 +1198,7 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
         a.t_end = t_end;
         a.max_pairs = c->steps_max_pairs;
         a.err = c->err;
+        a.trace = reinterpret_cast<unsigned long long*>(c->part) + (c->part_bytes / 8 - (size_t)8 * 4096);
         if (launch_steps(a, c->sm_count, c->stream) != cudaSuccess) {
             cudaGetLastError();
             return NB_ERR_CUDA;
@@ -1082,6 +1218,20 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
                 return NB_ERR_CUDA;
             const int64_t did = (int64_t)status[0];
             const int reason = (int)status[1];
+#ifdef NB_STEPS_TRACE
+            {   // development builds: dump CTA 0's phase stamps of this launch (ns since its first stamp)
+                std::vector<unsigned long long> tr((size_t)8 * (did < 4096 ? did : 4096));
+                cudaMemcpy(tr.data(), reinterpret_cast<unsigned long long*>(c->part) + (c->part_bytes / 8 - (size_t)8 * 4096),
+                           tr.size() * 8, cudaMemcpyDeviceToHost);
+                if (FILE* f = fopen("gpurun_out/steps_trace.txt", "a")) {
+                    for (int64_t q = 0; q < (int64_t)tr.size() / 8; ++q) {
+                        for (int w = 1; w < 7; ++w) fprintf(f, "%lld ", (long long)(tr[q * 8 + w] - tr[q * 8 + w - 1]));
+                        fprintf(f, "\n");
+                    }
+                    fclose(f);
+                }
+            }
+#endif
             if (did > 0) {
                 last_was_host = false;
                 if (reason != STEPS_BIG) c->blk_ni = (int64_t)status[3];   // for nb_block_forces
@@ -1092,9 +1242,9 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
                 result = NB_ERR_STATE;
                 break;
             }
-            // one block the persistent kernel does not take.  Its time and size are known, so the
-            // scheduler kernel (it leaves the ascending list on the device) and nb_step's launches
-            // (packed fp32 pair kernel) are queued without another synchronisation.
+            // one block the persistent kernel does not take.  It left the block's ascending list on
+            // the device and its time and size are known, so nb_step's launches (predictor, packed
+            // fp32 pair kernel, reduction, corrector) are queued without another synchronisation.
             const long long kb = (long long)status[2];
             const long long bits = kb ^ ((~kb >> 63) | (long long)0x8000000000000000ull);
             memcpy(&t, &bits, 8);
@@ -1103,12 +1253,6 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
                 result = NB_ERR_ARG;
                 break;
             }
-            if (launch_select(c->store.f[F_T], c->dts, c->n, c->sel_meta, c->sel_counts, c->blk_list, c->ni_pad,
-                              c->sm_count, c->stream) != cudaSuccess) {
-                cudaGetLastError();
-                return NB_ERR_CUDA;
-            }
-            c->launches += 1;
             c->blk_t = t;
             c->blk_ni = ni;
             rc = step_body(c, t, ni, eps2, eta, dt_min, dt_max);

@@ -38,7 +38,7 @@ constexpr int FORCE_THREADS = 128;
 constexpr int NWARPS = FORCE_THREADS / 32;
 constexpr int IPT = 2;                        // i-particles per thread
 constexpr int ITILE = FORCE_THREADS * IPT;    // i-slots per CTA (= i-particles when JL = 1)
-constexpr int JL_MID = 4, JL_MAX = 32;        // threads per i in the few-i variants (force.cu)
+constexpr int JSH_MAX = 5;                    // up to 2^5 = 32 threads per i-slot in the few-i kernel (force.cu)
 constexpr int STAGES = NB_STAGES;             // j-tile ring depth
 constexpr int NOUT = 7;                       // ax ay az jx jy jz pot
 
@@ -46,6 +46,12 @@ constexpr int NOUT = 7;                       // ax ay az jx jy jz pot
 enum Pack64Field { Q_X = 0, Q_Y, Q_Z, Q_VX, Q_VY, Q_VZ, Q_M, Q_FLAG, NQF };
 constexpr int TILE64_DOUBLES = TJ * NQF;      // 1024
 constexpr int TILE64_BYTES = TILE64_DOUBLES * 8;   // 8192
+
+// pack6: the tiles of the 6th-order pair loop (force6.cu): 14 float arrays of TJ: two-float position,
+// velocity, predicted acceleration, mass, flag
+constexpr int NPF6 = 14;
+constexpr int TILE6_FLOATS = TJ * NPF6;       // 1792
+constexpr int TILE6_BYTES = TILE6_FLOATS * 4; // 7168
 
 // calls with eps2 below this (zero included) drop r = 0 pairs inside the packed pair (force.cu GUARD):
 // the self pair's m eps^-3 would leave the fp32 range (m up to ~1e8 is safe at the threshold)
@@ -65,6 +71,10 @@ struct ForceArgs {
     const int32_t* i_list;    // [ni] (by-index calls, nb_force)
     const double* ext_x;      // [3][ni]: i-particles by value (nb_force_ext), else unused
     const double* ext_v;      // [3][ni], or NULL for acc + pot only
+    const int32_t* ext_self;  // [ni] by value: index of the j-set member this i-particle is (or < 0), or NULL
+    const uint8_t* ext_flags; // [ni] by value: bit 0 = it carries the unsoftened flag, or NULL
+    int jsh;                  // few-i kernel: log2 of the threads per i-slot (0 = all-i kernel)
+    int reduce_here;          // few-i kernel: the last CTA to finish also reduces (one launch per call)
     double* part;             // [S][NOUT][ni_pad] partial sums (reduce_mode 0)
     const uint8_t* flags;     // [n_cap] bit 0: unsoftened among flagged
     const uint32_t* tileflag; // bit t: tile t holds a flagged particle
@@ -92,6 +102,10 @@ struct ReduceArgs {
     int ni, ni_pad, splits, n;
     double t_pred;
     int atomic_mode;          // 1: acc/jrk/pot already hold the sums (atomics); only fix-ups here
+    const double *ext_x, *ext_v;      // by-value calls: the i-particles (for their flagged pairs)
+    const int32_t* ext_self;
+    const uint8_t* ext_flags;
+    unsigned* counter;        // ticket counter of the few-i kernel's own reduction (zero between calls)
 };
 
 // kernel launchers (each returns the cudaError of the launch)
@@ -100,16 +114,21 @@ cudaError_t launch_set_j(const StorePtrs& dst, const SrcPtrs& src, int64_t first
 cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int32_t* idx,
                             int64_t count, int64_t n, int* err, cudaStream_t s);
 cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int count, cudaStream_t s);
-cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64, int64_t n,
-                           double t, cudaStream_t s);
+cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64, float* pack6,
+                           int64_t n, double t, cudaStream_t s);
 cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
                                  double* out, cudaStream_t s);
-cudaError_t force_kernel_setup(int* blocks_per_sm, int* blocks_per_sm_guard);
+cudaError_t force_kernel_setup(int* blocks_per_sm /*[4]*/);
 cudaError_t force64_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_force64(const ForceArgs& a, int mode, cudaStream_t s);
-cudaError_t launch_force(const ForceArgs& a, int jl, int mode, int atomic_mode, double* acc, double* jrk,
-                         double* pot, cudaStream_t s);
+cudaError_t launch_force(const ForceArgs& a, const ReduceArgs& r, int mode, int atomic_mode, double* acc,
+                         double* jrk, double* pot, cudaStream_t s);
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s);
+// direct.cu: the one-launch force call for a handful of active particles
+constexpr int DIRECT_NI_MAX = 8;
+int direct_grid(int ntiles, int sm_count);
+int64_t direct_terms_per_lane(int ntiles, int grid);
+cudaError_t launch_direct(const ForceArgs& a, const ReduceArgs& r, int grid, cudaStream_t s);
 constexpr int SEL_MAX_BLOCKS = 1024;          // most CTAs the cooperative scheduler kernel uses
 cudaError_t launch_select(const double* t, const double* dt, int64_t n, unsigned long long* meta,
                           int* counts, int32_t* list, int64_t cap, int sm_count, cudaStream_t s);
@@ -125,6 +144,20 @@ cudaError_t launch_fused(const StorePtrs& st, const uint8_t* flags, const int32_
                          double t, double eps2, int any_flagged, double* part, int* err, int sm_count,
                          int* grid_out, int* ni_pad_out, cudaStream_t s);
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s);
+
+struct Force6Args {
+    const float* pack6;       // [ntiles][NPF6][TJ]
+    const int32_t* i_list;
+    double* part;             // [10][ni_pad][splits]
+    const uint8_t* flags;
+    int* err;
+    int ni, ni_pad, n_itiles, n, ntiles, splits;
+    float eps2;
+    int any_flagged;
+};
+cudaError_t force6_kernel_setup(int* blocks_per_sm);
+cudaError_t launch_force6(const Force6Args& a, const StorePtrs& st, const int32_t* flag_list, int nflag, double t_pred,
+                          double* acc, double* jrk, double* snp, double* pot, cudaStream_t s);
 
 // ---- nb_steps (steps.cu): block steps in one persistent cooperative kernel ---------------------
 constexpr int STEPS_NI_MAX = 512;             // largest block the persistent kernel takes itself
@@ -155,6 +188,7 @@ struct StepsArgs {
     double eps2, eta, dt_min, dt_max, t_end;
     int64_t max_pairs;            // a block with ni x n above this is left to the host path
     int* err;
+    unsigned long long* trace;    // NB_STEPS_TRACE builds only
 };
 cudaError_t steps_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_steps(const StepsArgs& a, int sm_count, cudaStream_t s);

@@ -64,11 +64,13 @@ __device__ __forceinline__ void split(double x, float& hi, float& lo)
 // One thread = particles 2q, 2q+1.  n_pad = ntiles * TJ; particles in [n, n_pad) become m = 0
 // padding records far away.  Store arrays are n_cap >= n_pad long, so loads never leave them.
 // P64: also write the fp64 tiles of the full-double pair loop (force64.cu; 64 B more per particle).
-template <bool P64>
+// P6: also write the tiles of the 6th-order pair loop (force6.cu; 56 B more), which carry the
+// predicted acceleration a + jerk dt (R22).
+template <bool P64, bool P6>
 __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_t* __restrict__ flags,
                                                       float* __restrict__ pack,
-                                                      double* __restrict__ pack64, int64_t n,
-                                                      int64_t n_pad, double t)
+                                                      double* __restrict__ pack64, float* __restrict__ pack6,
+                                                      int64_t n, int64_t n_pad, double t)
 {
     const int64_t p = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
     if (p >= n_pad) return;
@@ -76,6 +78,7 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
     const double dt0 = t - tj.x, dt1 = t - tj.y;
     float2 out[NPF];
     double2 o64[NQF];
+    float2 oa[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const double2 x = ld2(st.f[F_X + c], p), v = ld2(st.f[F_VX + c], p);
@@ -86,6 +89,7 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
         split(xp0, out[P_XH + c].x, out[P_XL + c].x);
         split(xp1, out[P_XH + c].y, out[P_XL + c].y);
         out[P_VX + c] = make_float2(__double2float_rn(vp0), __double2float_rn(vp1));
+        if (P6) oa[c] = make_float2(__double2float_rn(fma(j.x, dt0, a.x)), __double2float_rn(fma(j.y, dt1, a.y)));
         if (P64) {
             o64[Q_X + c] = make_double2(xp0, xp1);
             o64[Q_VX + c] = make_double2(vp0, vp1);
@@ -119,6 +123,20 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
     float* base = pack + (p / TJ) * TILE_FLOATS + (p % TJ);
 #pragma unroll
     for (int f = 0; f < NPF; ++f) *reinterpret_cast<float2*>(base + f * TJ) = out[f];
+    if (P6) {
+        // same records with the acceleration between velocity and mass: xh xl v | a | m flag
+        float* b6 = pack6 + (p / TJ) * TILE6_FLOATS + (p % TJ);
+#pragma unroll
+        for (int f = 0; f < 9; ++f) *reinterpret_cast<float2*>(b6 + f * TJ) = out[f];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            if (p >= n) oa[c].x = 0.0f;
+            if (p + 1 >= n) oa[c].y = 0.0f;
+            *reinterpret_cast<float2*>(b6 + (9 + c) * TJ) = oa[c];
+        }
+        *reinterpret_cast<float2*>(b6 + 12 * TJ) = out[P_M];
+        *reinterpret_cast<float2*>(b6 + 13 * TJ) = out[P_FLAG];
+    }
 }
 
 __global__ void __launch_bounds__(256) get_predicted_kernel(StorePtrs st, int64_t first,
@@ -170,14 +188,16 @@ cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int co
 }
 
 cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64,
-                           int64_t n, double t, cudaStream_t s)
+                           float* pack6, int64_t n, double t, cudaStream_t s)
 {
     if (n == 0) return cudaSuccess;
     const int64_t n_pad = (n + TJ - 1) / TJ * TJ;
     const int64_t threads = n_pad / 2;
     const unsigned grid = (unsigned)((threads + 127) / 128);
-    if (pack64) predict_kernel<true><<<grid, 128, 0, s>>>(store, flags, pack, pack64, n, n_pad, t);
-    else predict_kernel<false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, n, n_pad, t);
+    if (pack64 && pack6) predict_kernel<true, true><<<grid, 128, 0, s>>>(store, flags, pack, pack64, pack6, n, n_pad, t);
+    else if (pack64) predict_kernel<true, false><<<grid, 128, 0, s>>>(store, flags, pack, pack64, nullptr, n, n_pad, t);
+    else if (pack6) predict_kernel<false, true><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, pack6, n, n_pad, t);
+    else predict_kernel<false, false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, nullptr, n, n_pad, t);
     return cudaGetLastError();
 }
 

@@ -50,6 +50,14 @@ constexpr int ST_GMAX = 256;                  // most CTAs (slices)
 // dynamic shared memory: si [NI_MAX][6] | tile [7][512] | keys [ST_KEYS]
 constexpr int ST_SMEM = STEPS_NI_MAX * 6 * 8 + NOUT * ST_TILE * 8 + ST_KEYS * 8;
 
+// NB_STEPS_TRACE (development builds only): CTA 0 stamps %globaltimer at the phase boundaries of every
+// step into the partial buffer's tail, 8 words per step
+#ifdef NB_STEPS_TRACE
+#define TRACE(k) do { if (b == 0 && tid == 0) P.trace[s * 8 + (k)] = gtime(); } while (0)
+#else
+#define TRACE(k) do { } while (0)
+#endif
+
 __device__ __forceinline__ double ldcg(const double* p) { return __ldcg(p); }
 __device__ __forceinline__ unsigned long long gtime()
 {
@@ -74,6 +82,37 @@ __device__ __forceinline__ unsigned long long block_min(unsigned long long k, un
 #pragma unroll
     for (int w = 1; w < ST_WARPS; ++w) k = sw[w] < k ? sw[w] : k;
     return k;
+}
+
+// The particles of this CTA's slice whose key equals kmin, ascending, to dst[0 .. cap_dst): ordered
+// compaction by ballots, 512 particles at a time.  Returns how many there are (may exceed cap_dst).
+__device__ __forceinline__ int compact_due(const unsigned long long* keys, bool cached, const double* T,
+                                           const double* dts, int64_t lo, int cnt_own, unsigned long long kmin,
+                                           int32_t* dst, int cap_dst, int* swsum, int tid, int lane, int warp)
+{
+    int base = 0;
+    for (int q0 = 0; q0 < cnt_own; q0 += ST_THREADS) {
+        const int q = q0 + tid;
+        bool due = false;
+        if (q < cnt_own) due = (cached ? keys[q] : key_of(ldcg(T + lo + q) + ldcg(dts + lo + q))) == kmin;
+        const unsigned bal = __ballot_sync(0xffffffffu, due);
+        if (lane == 0) swsum[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < ST_WARPS; ++w) {
+            const int c = swsum[w];
+            total += c;
+            if (w < warp) before += c;
+        }
+        if (due) {
+            const int pos = base + before + __popc(bal & ((1u << lane) - 1u));
+            if (pos < cap_dst) dst[pos] = (int32_t)(lo + q);
+        }
+        base += total;
+        __syncthreads();
+    }
+    return base;
 }
 
 __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
@@ -109,6 +148,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
     for (int64_t s = 0; s <= P.budget; ++s) {
         if (b == 0 && tid == 0) P.log_ns[s] = gtime();
         if (s == P.budget) break;
+        TRACE(0);
 
         // ---- A: earliest time of my slice and who is due then (R21) ----------------------------
         unsigned long long k = ~0ull;
@@ -117,34 +157,15 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             k = kq < k ? kq : k;
         }
         const unsigned long long kmin = block_min(k, swmin, lane, warp);
-        int base = 0;
-        for (int q0 = 0; q0 < cnt_own; q0 += ST_THREADS) {
-            const int q = q0 + tid;
-            bool due = false;
-            if (q < cnt_own)
-                due = (cached ? keys[q] : key_of(ldcg(T + lo + q) + ldcg(P.dts + lo + q))) == kmin;
-            const unsigned bal = __ballot_sync(0xffffffffu, due);
-            if (lane == 0) swsum[warp] = __popc(bal);
-            __syncthreads();
-            int before = 0, total = 0;
-#pragma unroll
-            for (int w = 0; w < ST_WARPS; ++w) {
-                const int c = swsum[w];
-                total += c;
-                if (w < warp) before += c;
-            }
-            if (due) {
-                const int pos = base + before + __popc(bal & ((1u << lane) - 1u));
-                if (pos < STEPS_SLOT) slots[b].idx[pos] = (int32_t)(lo + q);
-            }
-            base += total;
-            __syncthreads();
-        }
+        const int base = compact_due(keys, cached, T, P.dts, lo, cnt_own, kmin, slots[b].idx, STEPS_SLOT, swsum, tid,
+                                     lane, warp);
         if (tid == 0) {
             slots[b].key = kmin;
             slots[b].count = base;
         }
+        TRACE(1);
         grid.sync();                                                            // ---- barrier 1
+        TRACE(2);
 
         // ---- B: the block time and the due list, from the published slices ---------------------
         unsigned long long kg = ~0ull;
@@ -179,6 +200,14 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         else if (!(t1 <= P.t_end)) reason = STEPS_T_END;
         else if (trunc || ni64 > STEPS_NI_MAX || ni64 > P.cap || ni64 * n > P.max_pairs) reason = STEPS_BIG;
         if (reason != STEPS_RUNNING) {        // uniform over the grid: everybody leaves
+            if (reason == STEPS_BIG && ni64 <= P.cap) {
+                // leave the whole ascending list for the host path: each slice that attains t1 writes
+                // its due particles at its offset (the published lists stop at STEPS_SLOT entries)
+                __syncthreads();              // goff complete
+                if (__ldcg(&slots[b].key) == kall)
+                    compact_due(keys, cached, T, P.dts, lo, cnt_own, kall, P.list + goff[b], (int)(P.cap - goff[b]),
+                                swsum, tid, lane, warp);
+            }
             if (b == 0 && tid == 0) {
                 meta[4] = (unsigned long long)s;
                 meta[5] = (unsigned long long)reason;
@@ -191,6 +220,22 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         if (b == 0 && tid == 0) {
             P.log_t[s] = t1;
             P.log_ni[s] = ni64;
+        }
+        // the stored state of my j-particle of the first tile is requested before anything else
+        double rx[3], rv[3], ra[3], rj[3], rt = 0.0, rm = 0.0;
+        int rfl = 0;
+        if (lo + tid < hi) {
+            const int64_t p = lo + tid;
+            rt = ldcg(T + p);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                rx[c] = ldcg(P.st.f[F_X + c] + p);
+                rv[c] = ldcg(P.st.f[F_VX + c] + p);
+                ra[c] = ldcg(P.st.f[F_AX + c] + p);
+                rj[c] = ldcg(P.st.f[F_JX + c] + p);
+            }
+            rm = ldcg(P.st.f[F_M] + p);
+            rfl = P.any_flagged ? (P.flags[p] & 1) : 0;
         }
         __syncthreads();                      // goff complete
         if (tid < ni) {
@@ -211,6 +256,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             sfl[tid] = P.any_flagged ? (P.flags[i] & 1) : 0;
             if (b == 0) P.list[tid] = (int32_t)i;
         }
+        TRACE(3);
         // ... and one pass over this CTA's j-slice
         const int ii = tid % ni, slice = tid / ni, nsl = ST_THREADS / ni;
         Acc64 A;
@@ -218,13 +264,23 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         for (int64_t base_j = lo; base_j < hi; base_j += ST_TILE) {
             const int64_t p = base_j + tid;
             if (p < hi) {
-                const double dtj = t1 - ldcg(T + p);
+                if (base_j != lo) {           // later tiles: fetched here
+                    rt = ldcg(T + p);
 #pragma unroll
-                for (int c = 0; c < 3; ++c)
-                    predict1(ldcg(P.st.f[F_X + c] + p), ldcg(P.st.f[F_VX + c] + p), ldcg(P.st.f[F_AX + c] + p),
-                             ldcg(P.st.f[F_JX + c] + p), dtj, tile[c][tid], tile[3 + c][tid]);
-                tile[6][tid] = ldcg(P.st.f[F_M] + p);
-                tfl[tid] = P.any_flagged ? (P.flags[p] & 1) : 0;
+                    for (int c = 0; c < 3; ++c) {
+                        rx[c] = ldcg(P.st.f[F_X + c] + p);
+                        rv[c] = ldcg(P.st.f[F_VX + c] + p);
+                        ra[c] = ldcg(P.st.f[F_AX + c] + p);
+                        rj[c] = ldcg(P.st.f[F_JX + c] + p);
+                    }
+                    rm = ldcg(P.st.f[F_M] + p);
+                    rfl = P.any_flagged ? (P.flags[p] & 1) : 0;
+                }
+                const double dtj = t1 - rt;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) predict1(rx[c], rv[c], ra[c], rj[c], dtj, tile[c][tid], tile[3 + c][tid]);
+                tile[6][tid] = rm;
+                tfl[tid] = (unsigned char)rfl;
             }
             __syncthreads();                  // tile (and, the first time, si / sfl / sl) complete
             const int cnt = (int)(hi - base_j < ST_TILE ? hi - base_j : ST_TILE);
@@ -269,20 +325,34 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         const int mycnt = goff[b + 1] - first;
         Stored s0;
         if (warp < mycnt) s0 = load_stored(P.st, P.dts, sl[first + warp]);
+        TRACE(4);
         grid.sync();                                                            // ---- barrier 2
+        TRACE(5);
         for (int q = warp; q < mycnt; q += ST_WARPS) {
             const int64_t i = sl[first + q];
             if (q != warp) s0 = load_stored(P.st, P.dts, i);
             double o[NOUT];
 #pragma unroll
-            for (int c = 0; c < NOUT; ++c) {
-                double sum = 0.0;
-                const double* src = P.part + ((int64_t)c * ni + first + q) * G;
-                for (int g = lane; g < G; g += 32) sum += ldcg(src + g);
+            for (int c = 0; c < NOUT; ++c) o[c] = 0.0;
+            // four partials per lane and component in flight (28 loads): the sum is all load latency
+            for (int g0 = 0; g0 < G; g0 += 128) {
+                double pv[4][NOUT];
 #pragma unroll
-                for (int w = 16; w >= 1; w >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, w);
-                o[c] = sum;
+                for (int w = 0; w < 4; ++w) {
+                    const int g = g0 + 32 * w + lane;
+#pragma unroll
+                    for (int c = 0; c < NOUT; ++c)
+                        pv[w][c] = g < G ? ldcg(P.part + ((int64_t)c * ni + first + q) * G + g) : 0.0;
+                }
+#pragma unroll
+                for (int w = 0; w < 4; ++w)
+#pragma unroll
+                    for (int c = 0; c < NOUT; ++c) o[c] += pv[w][c];
             }
+#pragma unroll
+            for (int c = 0; c < NOUT; ++c)
+#pragma unroll
+                for (int w = 16; w >= 1; w >>= 1) o[c] += __shfl_xor_sync(0xffffffffu, o[c], w);
             if (lane == 0) {
 #pragma unroll
                 for (int c = 0; c < NOUT; ++c) P.out[(int64_t)c * ni + first + q] = o[c];
@@ -292,6 +362,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             }
         }
         __syncthreads();                      // the new keys / (t, dt) of my slice are visible to my next scan
+        TRACE(6);
         last_ni = ni64;
     }
     if (b == 0 && tid == 0) {

@@ -59,14 +59,16 @@ def gather_forces(acc, jrk, pot, ni, group=None):
 # ... and the second kernel sums these."  Rank r stores and predicts only particles
 # [lo_r, hi_r) (contiguous blocks: the sum is order-free, so this equals the paper's round-robin).
 # One force call on a global active list:
-#   1. every rank takes the predicted state and mass of the active particles it OWNS;
-#   2. one all_gather gives every rank the state of all active particles (7 fp64 each);
-#   3. every rank evaluates them BY VALUE against its own j-slice (nb_force_ext): partial forces;
-#   4. one all_reduce(sum) of [7][ni] fp64 -- the paper's "second kernel", across GPUs;
-#   5. the self pair was included by the owner's slice (by-value calls skip nothing): with
-#      eps2 > 0 it added nothing to acc and jerk and -m_i/eps to pot, which is taken back here;
-#      with eps2 = 0 a coincident pair contributes nothing (R6), so nothing is to be undone.
-# Unsoftened flagged pairs (R7) are not available on this path.
+#   1. every rank takes the predicted state of the active particles it OWNS, with their flag;
+#   2. one all_gather gives every rank the state of all active particles (6 fp64 + flag + global
+#      index each);
+#   3. every rank evaluates them BY VALUE against its own j-slice, telling the kernel which member of
+#      the slice each active particle is (nb_force_ext_ids: self_idx = global index - lo for the
+#      particles it owns, -1 for the others): the owner excludes the self pair by index (R5) and
+#      every rank treats the pairs between a flagged active particle and the flagged members of
+#      its slice as unsoftened (R7) -- exactly what nb_force does on one GPU;
+#   4. one all_reduce(sum) of [7][ni] fp64 -- the paper's "second kernel", across GPUs.
+# Nothing is added or taken back on the host: the sum of the ranks' partial forces IS the force.
 
 
 def owned(i_list, lo, hi):
@@ -76,36 +78,42 @@ def owned(i_list, lo, hi):
 
 
 def gather_active_state(state_local, pos_local, ni, group=None):
-    """state_local: (7, n_owned) fp64 = predicted x, y, z, vx, vy, vz and mass of the owned active
-    particles, pos_local: their positions in the global active list.  Returns (7, ni) on every
-    rank, in active-list order.  One all_gather of padded blocks + one of the positions."""
+    """state_local: (R, n_owned) fp64 rows of the owned active particles (predicted x, y, z, vx, vy,
+    vz, then whatever else travels: flag, global index), pos_local: their positions in the global
+    active list.  Returns (R, ni) on every rank, in active-list order.  One all_gather of the
+    counts + one of padded blocks."""
     world = dist.get_world_size(group)
     dev = state_local.device
+    rows = state_local.shape[0]
     counts = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(world)]
     dist.all_gather(counts, torch.tensor([state_local.shape[1]], dtype=torch.int64, device=dev), group=group)
     width = max(int(c.item()) for c in counts)
-    block = torch.zeros((8, max(width, 1)), dtype=torch.float64, device=dev)
+    block = torch.zeros((rows + 1, max(width, 1)), dtype=torch.float64, device=dev)
     k = state_local.shape[1]
-    block[:7, :k] = state_local
-    block[7, :k] = pos_local.to(torch.float64)           # positions < 2^53: exact in fp64
+    block[:rows, :k] = state_local
+    block[rows, :k] = pos_local.to(torch.float64)        # positions < 2^53: exact in fp64
     blocks = [torch.empty_like(block) for _ in range(world)]
     dist.all_gather(blocks, block, group=group)
-    out = torch.empty((7, ni), dtype=torch.float64, device=dev)
+    out = torch.empty((rows, ni), dtype=torch.float64, device=dev)
     for r in range(world):
         kr = int(counts[r].item())
         if kr:
-            out[:, blocks[r][7, :kr].to(torch.int64)] = blocks[r][:7, :kr]
+            out[:, blocks[r][rows, :kr].to(torch.int64)] = blocks[r][:rows, :kr]
     return out
 
 
-def force_j_sharded(force_by_value, state_local, pos_local, ni, eps2, group=None):
-    """Steps 2-5 above.  force_by_value(x (3, ni), v (3, ni)) -> (acc (3, ni), jrk (3, ni),
-    pot (ni,)) against the CALLING rank's j-slice (Context.force_ext on a GPU).  Returns the
-    complete acc, jrk, pot of the active list on every rank."""
+def force_j_sharded(force_by_value_ids, state_local, pos_local, ni, lo, hi, group=None):
+    """Steps 2-4 above.  state_local: (8, n_owned) = predicted x, y, z, vx, vy, vz, flag (0/1) and
+    GLOBAL index of the owned active particles.  force_by_value_ids(x (3, ni), v (3, ni), self_idx
+    int32 (ni,), iflags uint8 (ni,)) -> (acc (3, ni), jrk (3, ni), pot (ni,)) against the CALLING
+    rank's j-slice [lo, hi) (Context.force_ext_ids on a GPU).  Returns the complete acc, jrk, pot of
+    the active list on every rank."""
     st = gather_active_state(state_local, pos_local, ni, group)
-    acc, jrk, pot = force_by_value(st[0:3].contiguous(), st[3:6].contiguous())
+    gidx = st[7].to(torch.int64)
+    mine = (gidx >= lo) & (gidx < hi)
+    self_idx = torch.where(mine, gidx - lo, torch.full_like(gidx, -1)).to(torch.int32)
+    iflags = st[6].to(torch.uint8)
+    acc, jrk, pot = force_by_value_ids(st[0:3].contiguous(), st[3:6].contiguous(), self_idx, iflags)
     part = torch.cat([acc, jrk, pot.reshape(1, -1)], dim=0).contiguous()
     dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
-    if eps2 > 0.0:
-        part[6] += st[6] / (eps2 ** 0.5)
     return part[0:3], part[3:6], part[6]

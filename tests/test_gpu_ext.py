@@ -135,9 +135,43 @@ def test_bridge_kick_two_galaxies(nbmod):
     assert np.abs(pa + pb).max() <= 1e-7 * np.abs(pa).max()
 
 
+def test_by_value_members_of_a_j_slice(nbmod):
+    """nb_force_ext_ids: the call one GPU makes in the j-sharded scheme.  The context holds
+    a SLICE of the particles; the active particles come by value, some of them members of the slice
+    (self pair excluded by index, also at a softening where it would swamp pot), some flagged
+    (unsoftened pairs with the flagged members of the slice, R7).  Oracle: the full set with the
+    masses outside the slice zeroed."""
+    n, lo, hi, t = 3000, 1000, 2500, 0.2
+    m, x, v, a, j, tj = _j_set(n, 730)
+    flags = np.zeros(n, np.uint8)
+    flags[[40, 1100, 1105, 2400, 2900]] = 1
+    x[:, 1105] = x[:, 40] + 2e-3                       # flagged i outside the slice, flagged j inside, close
+    v[:, 1105], a[:, 1105], j[:, 1105], tj[1105] = v[:, 40], a[:, 40], j[:, 40], tj[40]    # and staying close
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    mm = m.copy()
+    mm[:lo] = 0.0
+    mm[hi:] = 0.0
+    for ni, eps2 in ((300, 2.0 ** -14), (12, 1e-12), (5, 0.0), (300, 1e-12)):
+        il = nbgen.permutation(731, n)[:ni].astype(np.int32)
+        il[:5] = [40, 1100, 1105, 2400, 2900]
+        ref = oracle.force(mm, xp, vp, il, eps2, flags)
+        self_idx = np.where((il >= lo) & (il < hi), il - lo, -1).astype(np.int32)
+        with nbmod.Context(hi - lo, ni) as ctx:
+            ctx.set_j(m[lo:hi], x[:, lo:hi], v[:, lo:hi], a[:, lo:hi], j[:, lo:hi], tj[lo:hi])
+            fl = np.flatnonzero(flags[lo:hi]).astype(np.int32)
+            ctx.set_flags(fl, np.ones(len(fl), np.uint8))
+            ctx.predict(t)
+            got = [q.cpu().numpy() for q in ctx.force_ext_ids(xp[:, il], vp[:, il], self_idx, flags[il], eps2)]
+            ctx.sync()
+        print("ids ni=%d eps2=%g" % (ni, eps2), check_parity(got, ref))
+    soft = oracle.force(mm, xp, vp, il, 2.0 ** -14)
+    hard = oracle.force(mm, xp, vp, il, 2.0 ** -14, flags)
+    assert rel_err_vec(soft[0][:, [0]], hard[0][:, [0]]).max() > 0.5       # the flags matter here
+
+
 def test_j_sharded_path_on_one_gpu(nbmod):
-    """sharding.force_j_sharded with the real kernel behind it (world size 1 over NCCL): the
-    by-value partial forces + self-term correction reproduce the by-index force call."""
+    """sharding.force_j_sharded with the real kernel behind it (world size 1 over NCCL): by-value
+    partial forces with member indices and flags reproduce the by-index force call."""
     import socket
     import torch.distributed as dist
     from paper_1409_5474_b200 import sharding
@@ -148,17 +182,23 @@ def test_j_sharded_path_on_one_gpu(nbmod):
     try:
         n, ni, t, eps2 = 5000, 700, 0.3, 2.0 ** -14
         m, x, v, a, j, tj = _j_set(n, 720)
+        flags = np.zeros(n, np.uint8)
+        flags[[7, 4000]] = 1
         il = nbgen.permutation(721, n)[:ni].astype(np.int32)
+        il[:2] = [7, 4000]
         xp, vp = oracle.predict(t, x, v, a, j, tj)
-        ref = oracle.force(m, xp, vp, il, eps2)
+        ref = oracle.force(m, xp, vp, il, eps2, flags)
         with nbmod.Context(n, ni) as ctx:
             ctx.set_j(m, x, v, a, j, tj)
+            ctx.set_flags(np.array([7, 4000], np.int32), np.ones(2, np.uint8))
             ctx.predict(t)
             px, pv = ctx.predicted()
             pos = sharding.owned(il, 0, n).to(ctx.device)
             idx = torch.from_numpy(il.astype(np.int64)).to(ctx.device)
-            state = torch.cat([px[:, idx], pv[:, idx], torch.from_numpy(m).to(ctx.device)[None, idx]], 0)
-            got = sharding.force_j_sharded(lambda xi, vi: ctx.force_ext(xi, vi, eps2), state, pos, ni, eps2)
+            fl = torch.from_numpy(flags.astype(np.float64)).to(ctx.device)
+            state = torch.cat([px[:, idx], pv[:, idx], fl[None, idx], idx[None].to(torch.float64)], 0)
+            got = sharding.force_j_sharded(lambda xi, vi, si, fi: ctx.force_ext_ids(xi, vi, si, fi, eps2),
+                                           state, pos, ni, 0, n)
             got = [q.cpu().numpy() for q in got]
             ctx.sync()
         check_parity(got, ref)

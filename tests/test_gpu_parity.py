@@ -172,11 +172,12 @@ def test_j_split_variants_agree(nbmod):
     assert all((p == q).all() for p, q in zip(again, outs[2]))    # deterministic (R9)
 
 
-@pytest.mark.parametrize("ni", [1, 3, 8, 9, 64, 65, 200])
+@pytest.mark.parametrize("ni", [1, 3, 8, 9, 16, 17, 32, 33, 64, 65, 128, 129, 200])
 def test_few_active_i_share_threads(nbmod, ni):
-    """few i active -> several threads per i split the j of a tile (32 threads per i
-    up to 8 i, 4 up to 64), shuffle butterfly, warp-per-i reduction.  Includes a flagged i, its own
-    tile, and the self pair of every i."""
+    """few i active -> 32, 16, .. 2 threads per i split the j-quads of a tile (the 256
+    slots of a CTA hold the next power of two >= N_i particles), shuffle butterfly; up to 16 i the
+    pair kernel's last CTA also reduces (one launch).  Includes a flagged i, its own tile, and the
+    self pair of every i."""
     c = _random_case(6000, 94, eps2=2.0 ** -14)
     c.flags[[11, 4000]] = 1
     il = nbgen.permutation(95, c.n)[:ni].astype(np.int32)

@@ -90,36 +90,46 @@ def _worker_j(rank, world, port, ni, eps2, out_q):
     try:
         c = nbgen.config1(777)
         c.m = c.m * (0.5 + nbgen.Streams(9, c.n).uniform())
-        il = nbgen.permutation(6, c.n)[:ni]
+        c.flags[[5, 300, 390, 776]] = 1                              # flagged on both sides of the cut
+        c.x[:, 390] = c.x[:, 5] + 1e-3                               # a tight flagged pair ACROSS ranks
+        il = nbgen.permutation(6, c.n)[:ni].copy()
+        il[:min(ni, 4)] = [5, 390, 300, 776][:min(ni, 4)]
         lo, hi = sharding.shard_bounds(c.n, rank, world)             # this rank's j-slice
         pos = sharding.owned(il, lo, hi)
         mine = il[pos.numpy()]
-        state = torch.from_numpy(np.concatenate([c.x[:, mine], c.v[:, mine], c.m[None, mine]], 0))
+        state = torch.from_numpy(np.concatenate([c.x[:, mine], c.v[:, mine], c.flags[None, mine].astype(np.float64),
+                                                 mine[None].astype(np.float64)], 0))
 
-        def by_value(x, v):
-            # the rank's "nb_force_ext": the oracle on its j-slice, i-particles appended massless
-            xi, vi = x.numpy(), v.numpy()
+        def by_value_ids(x, v, self_idx, iflags):
+            # the rank's "nb_force_ext_ids": the oracle on its j-slice with the i-particles appended
+            # massless; an i-particle that IS a member of the slice is evaluated in place (by index)
+            xi, vi, sidx, ifl = x.numpy(), v.numpy(), self_idx.numpy(), iflags.numpy()
             k = xi.shape[1]
             mm = np.concatenate([c.m[lo:hi], np.zeros(k)])
             xx = np.concatenate([c.x[:, lo:hi], xi], 1)
             vv = np.concatenate([c.v[:, lo:hi], vi], 1)
-            a, j, p = oracle.force(mm, xx, vv, np.arange(hi - lo, hi - lo + k, dtype=np.int32), eps2)
+            ff = np.concatenate([c.flags[lo:hi], ifl]).astype(np.uint8)
+            who = np.where(sidx >= 0, sidx, hi - lo + np.arange(k)).astype(np.int32)
+            a, j, p = oracle.force(mm, xx, vv, who, eps2, ff)
             return torch.from_numpy(a), torch.from_numpy(j), torch.from_numpy(p)
 
-        acc, jrk, pot = sharding.force_j_sharded(by_value, state, pos, len(il), eps2)
-        ra, rj, rp = oracle.force(c.m, c.x, c.v, il, eps2)
+        acc, jrk, pot = sharding.force_j_sharded(by_value_ids, state, pos, len(il), lo, hi)
+        ra, rj, rp = oracle.force(c.m, c.x, c.v, il, eps2, c.flags)
         ea = np.abs(acc.numpy() - ra).max() / np.abs(ra).max()
         ej = np.abs(jrk.numpy() - rj).max() / np.abs(rj).max()
         ep = np.abs(pot.numpy() - rp).max() / np.abs(rp).max()
-        out_q.put((rank, float(max(ea, ej, ep))))
+        soft = oracle.force(c.m, c.x, c.v, il, eps2)                 # the flags must matter in this case
+        differs = bool(np.abs(soft[0] - ra).max() > 1e-3 * np.abs(ra).max()) or eps2 != 1e-4
+        out_q.put((rank, float(max(ea, ej, ep)), differs))
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("ni,eps2", [(301, 1e-4), (5, 1e-4), (64, 0.0)])
+@pytest.mark.parametrize("ni,eps2", [(301, 1e-4), (5, 1e-4), (64, 0.0), (301, 1e-12)])
 def test_force_j_sharded_world2_gloo(ni, eps2):
     """j distributed over the ranks, partial forces summed.  Equal to the unsharded
-    sum up to the order of the fp64 additions (and the self term taken back when eps2 > 0)."""
+    sum up to the order of the fp64 additions, including unsoftened flagged pairs across the cut
+    and a softening small enough that a self pair left in would dominate pot."""
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
@@ -133,3 +143,4 @@ def test_force_j_sharded_world2_gloo(ni, eps2):
         assert p.exitcode == 0
     assert sorted(r[0] for r in res) == [0, 1]
     assert all(r[1] < 1e-12 for r in res), res
+    assert all(r[2] for r in res), res
