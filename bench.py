@@ -251,6 +251,9 @@ def measured_peaks():
 # no DRAM counters for the call's second, shorter launch.)  Algorithmic bytes of that launch: the
 # 46 MB pack once + 51 MB of partial sums.
 FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": 94.69e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one predict_kernel launch by particle count, from the
+# committed capture profiles/r2_predict_full.md (filled in when that capture exists)
+PREDICT_DRAM_TRAFFIC = {}
 
 
 def run_ours(args):
@@ -445,6 +448,19 @@ def run_ours(args):
                               (props.multi_processor_count * FFMA2_LANES_PER_CLK_SM * sm_max * 1e6),
         "note": "the pair body executes 33 FP32 lane-ops per interaction (DESIGN.md 7.2); "
                 "frac_of_ffma2_rate = executed lane-ops/s over the measured packed-FMA rate"}
+    if args.order6:
+        # 64 FP32 lane-operations per interaction (force6.cu) against 128 lanes per SM per clock
+        lane_peak = props.multi_processor_count * FP32_LANES_PER_SM * sm_max * 1e6
+        rate6 = ni_loc * n / (pair_ms * 1e-3)
+        roofline.update({"kernel": "force6_kernel (+ its reduction)", "lane_ops_per_interaction": 64,
+                         "frac_of_fp32_lanes": 64.0 * rate6 / lane_peak,
+                         "note": "achieved / frac are in 60-flop interactions as for the 4th-order kernel; the "
+                                 "6th-order body executes 64 lane-ops per interaction instead of 33, so its "
+                                 "ceiling in interactions is 33/64 of that kernel's",
+                         "traffic": None})
+        roofline["fma_probe"]["frac_of_ffma2_rate"] = (64.0 * rate6) / (
+            props.multi_processor_count * FFMA2_LANES_PER_CLK_SM * sm_max * 1e6)
+        roofline["fma_probe"]["note"] = "64 lane-ops per interaction (force6.cu)"
     if args.fp64:
         # FP64 pipe: 64 lanes per SM per clock (measured DFMA/DADD rate, profiles/r1_pipe_probes.md)
         p64 = fp32_peak_tflops / 2.0
@@ -467,8 +483,9 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": "f64" if args.fp64 else "f32",
         "data": "synthetic", "gflops": value * FLOP_PER_INTERACTION / 1e9,
-        "config": {"workload": workload, "n_j": n, "n_i": ni, "eps2": case.eps2,
-                   "step": "nb_update_j(active) + nb_predict + nb_force (gather, pairs, reduce)",
+        "config": {"workload": workload + ("_order6" if args.order6 else ""), "n_j": n, "n_i": ni, "eps2": case.eps2,
+                   "step": "nb_update_j(active) + nb_predict + %s (gather, pairs, reduce)" % (
+                       "nb_force6: acc, jerk, snap, pot" if args.order6 else "nb_force"),
                    "parallelism": "i-sharded x%d, j replicated" % world,
                    "l2": "no flush: per-step working set (j-store %.0f MB + pack %.0f MB + outputs "
                          "%.0f MB) exceeds the L2" % (112e-6 * n, 44e-6 * n, 56e-6 * ni),
@@ -601,7 +618,7 @@ def run_fewi(args):
     with nbm.Context(n, 1 << 10) as ctx:
         ctx.load_case(case)
         h = ctx.h
-        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > L2: evicts the pack / store
+        flush = torch.zeros(256 << 20, dtype=torch.uint8, device=dev)      # > L2: reading it evicts the pack / store
         for ni in (1, 2, 4, 8, 16, 64):
             d_il = torch.from_numpy(np.ascontiguousarray(il_all[:ni])).to(dev)
             o = [torch.empty((3, ni), dtype=torch.float64, device=dev),
@@ -632,7 +649,7 @@ def run_fewi(args):
                 warm = e0.elapsed_time(e1) / reps * 1e3
                 cold = []
                 for _ in range(20):
-                    flush.fill_(1)
+                    flush.sum()                 # a READ pass: the L2 then holds clean lines of this buffer only
                     e0.record()
                     call()
                     e1.record()
@@ -649,11 +666,150 @@ def run_fewi(args):
     line = {"metric": "GB/s of the j data streamed by one few-i force call", "value": best * peaks["hbm_gbs"],
             "unit": "GB/s", "n_gpus": 1, "steps": 200, "warmup": 5, "higher_is_better": True, "dtype": "f32/f64",
             "data": "synthetic", "config": {"workload": workload + "_few_i", "n_j": n,
-                                            "l2": "hbm_frac rows: the L2 is flushed (256 MB fill) before every timed call"},
+                                            "l2": "hbm_frac rows: the L2 is flushed (a 256 MB buffer is read) before every timed call"},
             "roofline": {"bound": "hbm", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "unit": "GB/s",
                          "achieved": best * peaks["hbm_gbs"], "frac": best, "traffic": None},
             "rows": rows}
     print(json.dumps(line))
+    return 0
+
+
+def run_predict(args):
+    """The Hermite predictor (a1) against the HBM roofline, where its working set cannot sit in the L2:
+    (a) config 5's N = 2^22 + 11 (470 MB of j-store, 185 MB of packed records), (b) config 3's
+    N = 2^20 alternating between two contexts (2 x 163 MB > 126 MB of L2).  GB/s at the contract's
+    152 B per particle and at the 157 B the kernel moves (112 B + 1 flag byte read,
+    44 B written)."""
+    import numpy as np
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    import nbgen
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import binding as nb
+    peaks = measured_peaks()
+    reps = max(args.steps, 20)
+
+    def time_calls(ctxs, t):
+        e = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        for _ in range(max(args.warmup, 3)):
+            for c in ctxs:
+                nb.nb_predict(c.h, t)
+        torch.cuda.synchronize()
+        for r in range(reps):
+            c = ctxs[r % len(ctxs)]
+            e[r][0].record()
+            nb.nb_predict(c.h, t)
+            e[r][1].record()
+        torch.cuda.synchronize()
+        ms = np.array([a.elapsed_time(b) for a, b in e])
+        return float(np.median(ms)), float(ms.min())
+
+    rows = []
+    c5 = nbgen.config5()
+    with nbm.Context(c5.n, 1) as ctx:
+        ctx.load_case(c5)
+        med, best = time_calls([ctx], 2.0 ** -7)
+        rows.append({"case": "cfg5_N%d_one_context" % c5.n, "n": c5.n, "ms_median": med, "ms_min": best})
+    del c5
+    c3 = nbgen.config3(sizes=(1,))
+    with nbm.Context(c3.n, 1) as a, nbm.Context(c3.n, 1) as b:
+        a.load_case(c3)
+        b.load_case(c3)
+        med, best = time_calls([a, b], c3.t_now)
+        rows.append({"case": "cfg3_N%d_two_contexts_alternating" % c3.n, "n": c3.n, "ms_median": med, "ms_min": best})
+    for r in rows:
+        r["gbs_152"] = 152.0 * r["n"] / (r["ms_median"] * 1e-3) / 1e9
+        r["gbs_157"] = 157.0 * r["n"] / (r["ms_median"] * 1e-3) / 1e9
+        r["frac_152"] = r["gbs_152"] / peaks["hbm_gbs"]
+        r["frac_157"] = r["gbs_157"] / peaks["hbm_gbs"]
+        # DRAM bytes of this launch from the committed ncu capture (profiles/r2_predict_full.md)
+        r["traffic"] = PREDICT_DRAM_TRAFFIC.get(r["n"])
+    top = rows[0]
+    line = {"metric": "GB/s of the Hermite predictor (152 B per particle)", "value": top["gbs_152"], "unit": "GB/s",
+            "n_gpus": 1, "steps": reps, "warmup": max(args.warmup, 3), "ms_per_step": top["ms_median"],
+            "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "predictor_" + top["case"],
+                       "l2": "working set 655 MB (one context) / 2 x 163 MB (two contexts) exceeds the 126 MB L2"},
+            "roofline": {"kernel": "predict_kernel", "bound": "hbm", "achieved": top["gbs_152"], "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": top["frac_152"], "traffic": top["traffic"],
+                         "peak_source": peaks["source"], "achieved_at_157_bytes": top["gbs_157"],
+                         "frac_at_157_bytes": top["frac_157"]},
+            "rows": rows}
+    print(json.dumps(line))
+    return 0
+
+
+def run_shard_j(args, case, il, t, workload, rank, world, local, dev):
+    """The paper's own multi-GPU scheme: rank r stores and predicts only its slice of j,
+    evaluates ALL active particles, received by value, against it (nb_force_ext_ids), and the partial
+    forces are summed by one all_reduce of [7][N_i] fp64.  World size 1 runs the same code path."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import binding as nb, sharding
+    if world == 1 and not dist.is_initialized():
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1, device_id=dev)
+    n, ni = case.n, len(il)
+    lo, hi = sharding.shard_bounds(n, rank, world)               # this rank's j-slice
+    ctx = nbm.Context(hi - lo, ni, device=local)
+    sl = slice(lo, hi)
+    ctx.set_j(case.m[sl], case.x[:, sl], case.v[:, sl], case.a[:, sl], case.j[:, sl], case.t[sl])
+    fl = np.flatnonzero(case.flags[sl]).astype(np.int32)
+    if fl.size:
+        ctx.set_flags(fl, np.ones(fl.size, np.uint8))
+    h = ctx.h
+    pos = sharding.owned(il, lo, hi).to(dev)                     # active particles this rank owns
+    mine = torch.from_numpy(il.astype(np.int64)).to(dev)[pos]
+    flags_dev = torch.from_numpy(case.flags.astype(np.float64)).to(dev)
+
+    def step():
+        nb.nb_predict(h, t)
+        px, pv = ctx.predicted()
+        loc = mine - lo
+        state = torch.cat([px[:, loc], pv[:, loc], flags_dev[None, mine], mine[None].to(torch.float64)], 0)
+        return sharding.force_j_sharded(lambda x, v, s_, f_: ctx.force_ext_ids(x, v, s_, f_, case.eps2),
+                                        state, pos, ni, lo, hi)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        out = step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.launch_count()
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        out = step()
+    e1.record()
+    barrier()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms = float(ms.item())
+    launches = ctx.launch_count() - l0
+    assert bool(torch.isfinite(out[2]).all())
+    if rank == 0:
+        value = float(ni) * n * args.steps / (ms * 1e-3)
+        line = {"metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "gflops": value * FLOP_PER_INTERACTION / 1e9,
+                "config": {"workload": workload, "n_j": n, "n_i": ni, "eps2": case.eps2,
+                           "step": "nb_predict(slice) + all_gather(active state) + nb_force_ext_ids(slice) + "
+                                   "all_reduce([7][N_i])",
+                           "parallelism": "j-sharded x%d (PAPER.md:55), active particles by value" % world},
+                "gpu_launches": int(launches),
+                "bytes_all_reduce_per_step": 56 * ni, "bytes_all_gather_per_step": 72 * ni}
+        print(json.dumps(line))
+    ctx.close()
+    dist.destroy_process_group()
     return 0
 
 
@@ -717,6 +873,8 @@ def main():
         return run_kick(args)
     if args.fewi:
         return run_fewi(args)
+    if args.predict:
+        return run_predict(args)
     if args.blockstep > 0:
         return run_blockstep(args)
     return run_ours(args)

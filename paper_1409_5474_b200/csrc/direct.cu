@@ -66,40 +66,56 @@ direct_kernel(ForceArgs P, ReduceArgs R)
     const float2 eps2 = dup(P.eps2);
     const float2 m3 = dup(-3.0f);
 
-    // a3: my j-quads, strided over the grid (a warp reads 512 contiguous bytes of each tile array)
+    // a3: my j-quads, strided over the grid (a warp reads 512 contiguous bytes of each tile array).
+    // UNR quads are fetched before the first is evaluated, so that a thread has 10 x UNR 128-bit
+    // loads in flight: with a cold L2 the loop is DRAM latency otherwise.
+    constexpr int UNR = NI <= 2 ? 4 : (NI <= 4 ? 2 : 1);
     const int64_t nquads = (int64_t)P.ntiles * (TJ / 4);
     const int64_t stride = (int64_t)gridDim.x * DIRECT_THREADS;
-    for (int64_t qd = (int64_t)blockIdx.x * DIRECT_THREADS + tid; qd < nquads; qd += stride) {
-        const int64_t tile = qd / (TJ / 4);
-        const int p = (int)(qd % (TJ / 4)) * 4;
-        const float* T = P.pack + tile * TILE_FLOATS + p;
-        float4 f[10];
+    for (int64_t qd0 = (int64_t)blockIdx.x * DIRECT_THREADS + tid; qd0 < nquads; qd0 += UNR * stride) {
+        float4 fa[UNR][10];
 #pragma unroll
-        for (int c = 0; c < 10; ++c) f[c] = __ldg(reinterpret_cast<const float4*>(T + c * TJ));
-        const int j0 = (int)(tile * TJ) + p;                      // index of the quad's first particle
-        unsigned jfl = 0u;                                        // flag bits of the four j (only if needed)
-        if (iflagged && ((P.tileflag[tile >> 5] >> (tile & 31)) & 1u)) {
-            const float4 ff = __ldg(reinterpret_cast<const float4*>(T + P_FLAG * TJ));
-            jfl = (__float_as_uint(ff.x) & 1u) | ((__float_as_uint(ff.y) & 1u) << 1) |
-                  ((__float_as_uint(ff.z) & 1u) << 2) | ((__float_as_uint(ff.w) & 1u) << 3);
+        for (int r = 0; r < UNR; ++r) {
+            const int64_t qd = qd0 + r * stride;
+            if (qd < nquads) {
+                const float* T = P.pack + (qd / (TJ / 4)) * TILE_FLOATS + (int)(qd % (TJ / 4)) * 4;
+#pragma unroll
+                for (int c = 0; c < 10; ++c) fa[r][c] = __ldg(reinterpret_cast<const float4*>(T + c * TJ));
+            }
         }
 #pragma unroll
-        for (int k = 0; k < NI; ++k) {
-            if (k < P.ni) {
-                const int self = sself[k] - j0;                   // 0..3: my own index is in this quad
-                const bool fl = ((iflagged >> k) & 1u) && jfl;
-                if ((unsigned)self < 4u || fl) {
-                    const float xs[4][10] = {
-                        {f[0].x, f[1].x, f[2].x, f[3].x, f[4].x, f[5].x, f[6].x, f[7].x, f[8].x, f[9].x},
-                        {f[0].y, f[1].y, f[2].y, f[3].y, f[4].y, f[5].y, f[6].y, f[7].y, f[8].y, f[9].y},
-                        {f[0].z, f[1].z, f[2].z, f[3].z, f[4].z, f[5].z, f[6].z, f[7].z, f[8].z, f[9].z},
-                        {f[0].w, f[1].w, f[2].w, f[3].w, f[4].w, f[5].w, f[6].w, f[7].w, f[8].w, f[9].w}};
+        for (int r = 0; r < UNR; ++r) {
+            const int64_t qd = qd0 + r * stride;
+            if (qd >= nquads) break;
+            const float4* f = fa[r];
+            const int64_t tile = qd / (TJ / 4);
+            const int p = (int)(qd % (TJ / 4)) * 4;
+            const int j0 = (int)(tile * TJ) + p;                      // index of the quad's first particle
+            unsigned jfl = 0u;                                        // flag bits of the four j (only if needed)
+            if (iflagged && ((P.tileflag[tile >> 5] >> (tile & 31)) & 1u)) {
+                const float4 ff = __ldg(reinterpret_cast<const float4*>(P.pack + tile * TILE_FLOATS + p + P_FLAG * TJ));
+                jfl = (__float_as_uint(ff.x) & 1u) | ((__float_as_uint(ff.y) & 1u) << 1) |
+                      ((__float_as_uint(ff.z) & 1u) << 2) | ((__float_as_uint(ff.w) & 1u) << 3);
+            }
 #pragma unroll
-                    for (int e = 0; e < 4; ++e)
-                        pair1_vals(sI[k], A[k], xs[e][0], xs[e][1], xs[e][2], xs[e][3], xs[e][4], xs[e][5], xs[e][6],
-                                   xs[e][7], xs[e][8], xs[e][9], e == self || (fl && ((jfl >> e) & 1u)), P.eps2);
-                } else {
-                    quad<true, GUARD>(sI[k], A[k], f, eps2, m3);
+            for (int k = 0; k < NI; ++k) {
+                if (k < P.ni) {
+                    const int self = sself[k] - j0;                   // 0..3: my own index is in this quad
+                    const bool fl = ((iflagged >> k) & 1u) && jfl;
+                    if ((unsigned)self < 4u || fl) {
+                        const float xs[4][10] = {
+                            {f[0].x, f[1].x, f[2].x, f[3].x, f[4].x, f[5].x, f[6].x, f[7].x, f[8].x, f[9].x},
+                            {f[0].y, f[1].y, f[2].y, f[3].y, f[4].y, f[5].y, f[6].y, f[7].y, f[8].y, f[9].y},
+                            {f[0].z, f[1].z, f[2].z, f[3].z, f[4].z, f[5].z, f[6].z, f[7].z, f[8].z, f[9].z},
+                            {f[0].w, f[1].w, f[2].w, f[3].w, f[4].w, f[5].w, f[6].w, f[7].w, f[8].w, f[9].w}};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            pair1_vals(sI[k], A[k], xs[e][0], xs[e][1], xs[e][2], xs[e][3], xs[e][4], xs[e][5],
+                                       xs[e][6], xs[e][7], xs[e][8], xs[e][9],
+                                       e == self || (fl && ((jfl >> e) & 1u)), P.eps2);
+                    } else {
+                        quad<true, GUARD>(sI[k], A[k], f, eps2, m3);
+                    }
                 }
             }
         }

@@ -872,9 +872,17 @@ int nb_force6(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double*
     a.splits = 1;
     if (a.ntiles > 0 && a.n_itiles < resident)
         a.splits = choose_splits(c, a.n_itiles, a.ntiles, a.ni_pad, c->part_bytes * NOUT / 10, resident);
+    nb_ctx::Rec* rec = prof_next(c);
+    if (rec) cudaEventRecord(rec->e[0], c->stream);
     if (launch_force6(a, c->store, c->flag_list, (int)c->flagged.size(), c->t_pred, acc, jrk, snp, pot, c->stream) !=
         cudaSuccess)
         return NB_ERR_CUDA;
+    if (rec) {                                // pair kernel and its reduction are timed together here
+        cudaEventRecord(rec->e[1], c->stream);
+        cudaEventRecord(rec->e[2], c->stream);
+        rec->kind = 1;
+        c->ring_used += 1;
+    }
     c->last[0] = a.splits;
     c->last[1] = (int64_t)a.n_itiles * a.splits;
     c->last[2] = 2;

@@ -204,3 +204,20 @@ def test_j_sharded_path_on_one_gpu(nbmod):
         check_parity(got, ref)
     finally:
         dist.destroy_process_group()
+
+
+def test_bench_shard_j_runs_on_one_gpu():
+    """bench.py --shard j (the arm a multi-GPU scaling run of the paper's scheme would use) on one GPU:
+    world size 1 goes through the same all_gather / nb_force_ext_ids / all_reduce path."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--shard", "j", "--workload", "small",
+                          "--steps", "2", "--warmup", "3"], capture_output=True, text=True, timeout=600, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["n_gpus"] == 1 and line["value"] > 1e10
+    assert "j-sharded" in line["config"]["parallelism"]
