@@ -44,7 +44,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg2", "cfg4", "cfg5", "small"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg1", "cfg2", "cfg4", "cfg5", "small"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sweep", action="store_true",
@@ -88,6 +88,10 @@ def make_case(name):
     if name == "cfg3":
         c = nbgen.config3()
         return c, c.i_lists[-1], c.t_now, "cfg3_plummer_N1048576_blockstep_all_active"
+    if name == "cfg1":
+        c = nbgen.config1()
+        c.a, c.j = nbgen.mean_field(c.x, c.v)
+        return c, c.i_lists[1], 2.0 ** -6, "cfg1_plummer_N1024_all_active"
     if name == "cfg2":
         c = nbgen.config2()
         c.a, c.j = nbgen.mean_field(c.x, c.v)
@@ -245,15 +249,17 @@ def measured_peaks():
         return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant force_kernel launch of the default
-# workload (the whole-wave segment, 3552 of the call's CTAs and 86 % of its time), from the committed
-# `ncu --set full` capture profiles/r1_cfg3_full.md: 56.97 MB read + 37.72 MB written.  (ncu returned
-# no DRAM counters for the call's second, shorter launch.)  Algorithmic bytes of that launch: the
-# 46 MB pack once + 51 MB of partial sums.
-FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": 94.69e6}
-# dram__bytes_read.sum + dram__bytes_write.sum of one predict_kernel launch by particle count, from the
-# committed capture profiles/r2_predict_full.md (filled in when that capture exists)
-PREDICT_DRAM_TRAFFIC = {}
+# DRAM bytes per launch cannot be measured inside a timed run (they need ncu's counters), so `traffic`
+# is quoted from the committed `ncu --set full` captures of this same command, per launch:
+# force_kernel, default workload (profiles/r2_cfg3_full.md): the whole-wave launch (3552 of the call's
+# CTAs, 87 % of its time) moved 57.76 MB read + 38.44 MB written = 96.2 MB -- the 46 MB pack once plus
+# the 51 MB of partial sums it writes; ncu returned no DRAM counters (NaN) for the call's second,
+# shorter launch in round 1 and again in round 2, so the figure covers 87 % of the call.
+FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": 96.20e6}
+# predict_kernel (profiles/r2_predict_full.md, profiles/r2_cfg3_full.md), by particle count:
+# N = 2^22 + 11: 474.04 MB read (= 113 B x N exactly) + 150.20 MB written of the 184.5 MB the kernel
+# stores (the rest was still in the L2 when the kernel ended) = 624.2 MB; N = 2^20: 118.5 + 18.3 MB.
+PREDICT_DRAM_TRAFFIC = {4194315: 624.25e6, 1048576: 136.84e6}
 
 
 def run_ours(args):
@@ -475,7 +481,7 @@ def run_ours(args):
     pred_gbs = PREDICT_BYTES_PER_PARTICLE * n / (pred_ms * 1e-3) / 1e9
     roofline_predict = {"kernel": "predict_kernel", "bound": "hbm", "achieved": pred_gbs,
                         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": pred_gbs / peaks["hbm_gbs"],
-                        "traffic": None, "peak_source": peaks["source"], "ms_per_launch": pred_ms,
+                        "traffic": PREDICT_DRAM_TRAFFIC.get(n), "peak_source": peaks["source"], "ms_per_launch": pred_ms,
                         "bytes_per_particle": PREDICT_BYTES_PER_PARTICLE}
     line = {
         "metric": "interactions/s", "value": value, "unit": "interactions/s", "n_gpus": world,

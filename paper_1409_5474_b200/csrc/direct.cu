@@ -37,6 +37,23 @@ direct_kernel(ForceArgs P, ReduceArgs R)
     __shared__ int s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
+    // a3 starts here: the first UNR quads of this thread are requested before anything else -- they do
+    // not depend on the i-particles, whose gather (two dependent loads) then runs under their latency
+    constexpr int UNR = NI <= 2 ? 4 : (NI <= 4 ? 2 : 1);
+    const int64_t nquads = (int64_t)P.ntiles * (TJ / 4);
+    const int64_t stride = (int64_t)gridDim.x * DIRECT_THREADS;
+    const int64_t qfirst = (int64_t)blockIdx.x * DIRECT_THREADS + threadIdx.x;
+    float4 fa[UNR][10];
+#pragma unroll
+    for (int r = 0; r < UNR; ++r) {
+        const int64_t qd = qfirst + r * stride;
+        if (qd < nquads) {
+            const float* T = P.pack + (qd / (TJ / 4)) * TILE_FLOATS + (int)(qd % (TJ / 4)) * 4;
+#pragma unroll
+            for (int c = 0; c < 10; ++c) fa[r][c] = __ldg(reinterpret_cast<const float4*>(T + c * TJ));
+        }
+    }
+
     // a2: the active particles, from the pack (two-float position, fp32 velocity; R8, R17)
     if (tid == 0) sflagged = 0u;
     __syncthreads();
@@ -68,19 +85,17 @@ direct_kernel(ForceArgs P, ReduceArgs R)
 
     // a3: my j-quads, strided over the grid (a warp reads 512 contiguous bytes of each tile array).
     // UNR quads are fetched before the first is evaluated, so that a thread has 10 x UNR 128-bit
-    // loads in flight: with a cold L2 the loop is DRAM latency otherwise.
-    constexpr int UNR = NI <= 2 ? 4 : (NI <= 4 ? 2 : 1);
-    const int64_t nquads = (int64_t)P.ntiles * (TJ / 4);
-    const int64_t stride = (int64_t)gridDim.x * DIRECT_THREADS;
-    for (int64_t qd0 = (int64_t)blockIdx.x * DIRECT_THREADS + tid; qd0 < nquads; qd0 += UNR * stride) {
-        float4 fa[UNR][10];
+    // loads in flight: with a cold L2 the loop is DRAM latency otherwise.  (First round: see above.)
+    for (int64_t qd0 = qfirst; qd0 < nquads; qd0 += UNR * stride) {
+        if (qd0 != qfirst) {
 #pragma unroll
-        for (int r = 0; r < UNR; ++r) {
-            const int64_t qd = qd0 + r * stride;
-            if (qd < nquads) {
-                const float* T = P.pack + (qd / (TJ / 4)) * TILE_FLOATS + (int)(qd % (TJ / 4)) * 4;
+            for (int r = 0; r < UNR; ++r) {
+                const int64_t qd = qd0 + r * stride;
+                if (qd < nquads) {
+                    const float* T = P.pack + (qd / (TJ / 4)) * TILE_FLOATS + (int)(qd % (TJ / 4)) * 4;
 #pragma unroll
-                for (int c = 0; c < 10; ++c) fa[r][c] = __ldg(reinterpret_cast<const float4*>(T + c * TJ));
+                    for (int c = 0; c < 10; ++c) fa[r][c] = __ldg(reinterpret_cast<const float4*>(T + c * TJ));
+                }
             }
         }
 #pragma unroll

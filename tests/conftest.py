@@ -20,3 +20,18 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "slow" in it.keywords:
             it.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _fresh_library_on_a_gpu_box(request):
+    """On a box with a GPU the library is rebuilt from the sources of this tree before the first
+    test, so that what the GPU tests load is what the tree says (the shipped .so is a convenience)."""
+    try:
+        import torch
+        have_gpu = torch.cuda.is_available()
+    except ImportError:
+        have_gpu = False
+    if have_gpu and os.environ.get("NB_NO_REBUILD") != "1":
+        import __graft_entry__ as g
+        g.build(force=True)
+    yield

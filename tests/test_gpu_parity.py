@@ -320,3 +320,37 @@ def test_lent_workspace(nbmod):
         nb.nb_set_workspace(ctx.h, ws.data_ptr() + off, nbytes)     # too late
     ctx.close()
     check_parity(got, _oracle_force(c, 0.0, np.arange(c.n)))
+
+
+def test_bitwise_repeatability_of_every_kernel_path(nbmod):
+    """compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md), so races in the tile
+    ring (release counter, refill by the last warp out, mbarrier phases), in the ticket reduction and
+    in the persistent kernel's slots are hunted the other way round: every path is deterministic by
+    construction (R9), so 12 back-to-back repeats under different timing (a second stream keeps the
+    chip busy for half of them) must give bit-identical results -- and the first of them matches the
+    oracle."""
+    c = _random_case(20000, 130, eps2=2.0 ** -16)
+    c.flags[[17, 9000]] = 1
+    perm = nbgen.permutation(131, c.n)
+    side = torch.cuda.Stream()
+    noise = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+    for ni in (3, 8, 12, 100, 300, 20000):             # direct, few-i (in-kernel and separate reduce), all-i
+        il = perm[:ni].astype(np.int32)
+        il[0] = 17
+        ref = _oracle_force(c, 0.1, il)
+        with nbmod.Context(c.n, ni) as ctx:
+            ctx.load_case(c)
+            ctx.predict(0.1)
+            first = None
+            for rep in range(12):
+                if rep % 2:
+                    with torch.cuda.stream(side):
+                        noise.fill_(rep)
+                got = _np(ctx.force(il, c.eps2))
+                if first is None:
+                    first = got
+                    check_parity(got, ref)
+                else:
+                    assert all(np.array_equal(p, q) for p, q in zip(first, got)), (ni, rep)
+            ctx.sync()
+        side.synchronize()
