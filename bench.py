@@ -422,6 +422,7 @@ def run_ours(args):
             ctx.profiling(False)
             sweep.append({"n_i": ns, "ms_per_call": best, "interactions_per_s": ns * n / (best * 1e-3),
                           "frac_fp32_peak": None, "pack_gbs": 44.0 * n / (best * 1e-3) / 1e9,
+                          "hbm_frac": 44.0 * n / (best * 1e-3) / 1e9 / measured_peaks()["hbm_gbs"],
                           "j_splits": int(info["j_splits"]), "ctas": int(info["ctas"]),
                           "pair_ms": kts["pair_ms"] / max(kts["n_pair"], 1),
                           "reduce_ms": kts["reduce_ms"] / max(kts["n_reduce"], 1)})

@@ -285,11 +285,17 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
             __syncthreads();                  // tile (and, the first time, si / sfl / sl) complete
             const int cnt = (int)(hi - base_j < ST_TILE ? hi - base_j : ST_TILE);
             if (slice < nsl) {
+                // my i-particle in registers: read from shared memory inside the loop its six doubles
+                // (48-byte rows: bank conflicts) would make the pair loop shared-memory-bound
+                double xi[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) xi[c] = si[ii][c];
+                const bool ifl = sfl[ii] != 0;
                 const int self = sl[ii] - (int)base_j;    // position of the own index in this tile, if any
 #pragma unroll 2
                 for (int q = slice; q < cnt; q += nsl) {
-                    const double e2 = (sfl[ii] && tfl[q]) ? 0.0 : P.eps2;
-                    pair64<true>(si[ii], A, tile[0][q], tile[1][q], tile[2][q], tile[3][q], tile[4][q], tile[5][q],
+                    const double e2 = (ifl && tfl[q]) ? 0.0 : P.eps2;
+                    pair64<true>(xi, A, tile[0][q], tile[1][q], tile[2][q], tile[3][q], tile[4][q], tile[5][q],
                                  tile[6][q], e2, q == self);
                 }
             }
