@@ -539,6 +539,7 @@ def run_blockstep(args):
         with nbm.Context(n) as ctx:
             if args.steps_bound >= 0:
                 ctx.steps_bound(int(args.steps_bound))
+            ctx.steps_queue({"steps_host": 0, "steps_rounds": 1}.get(mode, 2))
             ctx.set_j(m, x, v)
             ctx.predict(0.0)
             ga, gj, gp = ctx.force(il, eps2)
@@ -560,16 +561,18 @@ def run_blockstep(args):
                 done, tl, sz, us = ctx.steps(args.steps, eps2, eta, lo, hi, times=True)
                 assert done == args.steps
                 t = float(tl[-1])
-                times.append(np.array(us))
+                {"steps": times, "steps_host": times_host}.get(mode, []).append(np.array(us))
             e1.record()
             ctx.sync()
             return e0.elapsed_time(e1), time.perf_counter() - w0, ctx.launch_count() - l0, list(sz), t
 
     # A/B inside one process, interleaved: numbers from different gpurun calls differ by +-20 % for a
     # latency-bound loop and must not be compared with each other
-    times = []
-    runs = [(md, run(md)) for md in ("step", "steps", "step", "steps")]
+    times, times_host = [], []
+    runs = [(md, run(md)) for md in ("step", "steps_host", "steps_rounds", "steps") * 2]
+    ms_rounds, _, launches_rounds, _, _ = min((r for md, r in runs if md == "steps_rounds"), key=lambda r: r[0])
     ms_step, _, launches_step, _, _ = min((r for md, r in runs if md == "step"), key=lambda r: r[0])
+    ms_host, _, launches_host, _, _ = min((r for md, r in runs if md == "steps_host"), key=lambda r: r[0])
     ms, wall, launches, sizes, t = min((r for md, r in runs if md == "steps"), key=lambda r: r[0])
     sizes = np.array(sizes, dtype=np.float64)
     small = (sizes <= 512) & (sizes * n <= (args.steps_bound if args.steps_bound >= 0 else 3.0e7))
@@ -583,7 +586,9 @@ def run_blockstep(args):
             "data": "synthetic",
             "config": {"workload": "blockstep_plummer_N%d" % n, "eta": eta, "eps2": eps2,
                        "step": "nb_steps: scheduler + predictor-in-pair-loop + reduce + corrector per block in "
-                               "one persistent kernel; blocks above 256 particles or 3e7 pairs via nb_step"},
+                               "one persistent kernel; blocks above 512 particles or 3e7 pairs: launch shape planned "
+                               "on the device, predictor + packed fp32 pair kernel + reduction + corrector queued "
+                               "ahead of time (no host round trip)"},
             "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),
                       "min_n_i": int(sizes.min()), "max_n_i": int(sizes.max()),
                       "in_persistent_kernel": in_kernel,
@@ -595,10 +600,18 @@ def run_blockstep(args):
                       "us_pair_work_at_fp32_peak_host_path": float(floor_us[~small].sum()),
                       "particle_steps_per_s": float(sizes.sum() / (ms * 1e-3)), "t_end": t},
             "ab": {"us_per_block_step_nb_step": ms_step / args.steps * 1e3,
+                   "us_per_block_step_nb_steps_host_handover": ms_host / args.steps * 1e3,
+                   "us_per_block_step_nb_steps_stream_rounds": ms_rounds / args.steps * 1e3,
                    "us_per_block_step_nb_steps": ms / args.steps * 1e3,
+                   "launches_per_block_nb_steps_stream_rounds": launches_rounds / args.steps,
                    "launches_per_block_nb_step": launches_step / args.steps,
+                   "launches_per_block_nb_steps_host_handover": launches_host / args.steps,
                    "launches_per_block_nb_steps": launches / args.steps,
-                   "note": "same process, same start and schedule, best of 2 each, interleaved"},
+                   "us_total_host_path_host_handover": float(np.minimum(times_host[0], times_host[1])[~small].sum()),
+                   "note": "same process, same start and schedule, best of 2 each, interleaved; "
+                           "nb_steps = large blocks planned on the device, rounds in the WHILE node of one graph "
+                           "(nb_set_steps_queue 2, default), stream_rounds = the same rounds queued on the stream (1), "
+                           "host_handover = one host synchronisation per large block (queue 0)"},
             "gpu_launches": int(launches)}
     if args.detail:
         line["steps_detail"] = {"n_i": [int(q) for q in sizes], "us": [float(q) for q in us]}

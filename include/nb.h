@@ -318,6 +318,21 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
  * nb_step's launches; for tests and experiments). */
 int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs);
 
+/* How nb_steps takes a handed-over (large) block (the host link is the bottleneck).
+ * mode 2 (default): the block's launch shape is planned ON THE DEVICE and one "round" -- persistent
+ *   kernel, plan, predictor, packed fp32 pair kernel (both thread mappings), reduction, corrector,
+ *   each of which exits at once when it has nothing to do -- is the body of a WHILE node of a CUDA
+ *   graph whose condition the plan kernel sets: one graph launch and one synchronisation per
+ *   nb_steps call, however many large blocks there are.  Falls back to mode 1 if the driver cannot
+ *   build that graph.
+ * mode 1: the same rounds queued on the stream ahead of time, in batches; the host reads one
+ *   progress record per batch (rounds queued beyond the end of the run are wasted launches).
+ * mode 0: the host synchronises at every large block and takes it through nb_step's launches (the
+ *   only way in the IEEE-double mode, with the atomics reduction and with forced j-splits; these
+ *   select it by themselves).
+ * NB_ERR_ARG for any other mode. */
+int nb_set_steps_queue(nb_ctx* c, int mode);
+
 /* nb_step takes blocks of <= NB_FUSED_MAX particles through nb_force_fused (default on).  on = 0
  * switches this off. */
 int nb_set_fused(nb_ctx* c, int on);

@@ -19,7 +19,7 @@ EXPORTS = [
     "nb_set_j", "nb_update_j", "nb_update_j_host", "nb_set_j_host", "nb_clear", "nb_count", "nb_set_flags",
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_ext_ids", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_order", "nb_force6", "nb_set_precision", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync",
-    "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_steps", "nb_set_steps_bound", "nb_block_forces", "nb_strerror", "nb_version",
+    "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_steps", "nb_set_steps_bound", "nb_set_steps_queue", "nb_block_forces", "nb_strerror", "nb_version",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -72,6 +72,7 @@ lib.nb_correct.argtypes = [_vp, _vp, _i64, _dbl, _vp, _vp, _dbl, _dbl, _dbl]
 lib.nb_step.argtypes = [_vp, _dbl, _dbl, _dbl, _dbl, ctypes.POINTER(_dbl), ctypes.POINTER(_i64)]
 lib.nb_steps.argtypes = [_vp, _i64, _dbl, _dbl, _dbl, _dbl, _dbl, _vp, _vp, _vp, ctypes.POINTER(_i64)]
 lib.nb_set_steps_bound.argtypes = [_vp, _i64]
+lib.nb_set_steps_queue.argtypes = [_vp, _i32]
 lib.nb_block_forces.argtypes = [_vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp), ctypes.POINTER(_vp)]
 lib.nb_version.restype = ctypes.c_char_p
 
@@ -301,6 +302,10 @@ def nb_steps(c, k, eps2, eta, dt_min, dt_max, t_end=float("inf"), log=True, time
 
 def nb_set_steps_bound(c, max_pairs):
     _check(lib.nb_set_steps_bound(c, int(max_pairs)), "nb_set_steps_bound")
+
+
+def nb_set_steps_queue(c, on):
+    _check(lib.nb_set_steps_queue(c, int(on)), "nb_set_steps_queue")
 
 
 def nb_block_forces(c):

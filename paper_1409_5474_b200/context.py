@@ -207,6 +207,9 @@ class Context:
     def steps_bound(self, max_pairs):
         nb.nb_set_steps_bound(self.h, max_pairs)
 
+    def steps_queue(self, on):
+        nb.nb_set_steps_queue(self.h, on)
+
     # -- measurement --------------------------------------------------------------------------
     def profiling(self, on=True):
         nb.nb_set_profiling(self.h, on)

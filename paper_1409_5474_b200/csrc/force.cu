@@ -37,10 +37,14 @@ __host__ __device__ constexpr int stages_for(bool few) { return few ? 2 * STAGES
 // packed pair (R5, R6), so no tile needs the self-pair treatment.
 // The few-i kernel also does the reduction (a4/a5): the last CTA to finish -- a ticket counter --
 // sums the partials of all CTAs, so that such a call is ONE launch.
-template <bool ATOMIC, bool FEW, int MODE, bool GUARD>
-__global__ void __launch_bounds__(FORCE_THREADS, NB_MINB)
-force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __restrict__ ojrk,
-             double* __restrict__ opot)
+// The body takes the CTA's work item `work` (i-tile x j-subset) as an argument: force_kernel passes
+// blockIdx.x, force_dyn_kernel (block steps queued without the host, nb_steps) loops over the items
+// of a launch shape that was decided on the device.  DYN: the second form (the item is then carried
+// in a register through the pair loop instead of being read from %ctaid again).
+template <bool ATOMIC, bool FEW, int MODE, bool GUARD, bool DYN>
+__device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs& R, const unsigned work,
+                                           double* __restrict__ oacc, double* __restrict__ ojrk,
+                                           double* __restrict__ opot)
 {
     constexpr int STG = stages_for(FEW);
     constexpr bool JERK = (MODE != 2);
@@ -59,8 +63,8 @@ force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __res
     const int jsh = FEW ? P.jsh : 0;              // log2 of the threads per i-slot
     const int jl = 1 << jsh;
     const int jlane = tid & (jl - 1);
-    const int it = blockIdx.x % P.n_itiles;       // neighbouring CTAs share the j-subset (L2 reuse)
-    const int sp = blockIdx.x / P.n_itiles;
+    const int it = work % P.n_itiles;             // neighbouring CTAs share the j-subset (L2 reuse)
+    const int sp = work / P.n_itiles;
     const int t0 = (int)(((int64_t)P.ntiles * sp) / P.splits);
     const int t1 = (int)(((int64_t)P.ntiles * (sp + 1)) / P.splits);
 
@@ -250,8 +254,8 @@ force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __res
 
     // the CTA's place in the grid is read again here, so that it does not hold registers through
     // the pair loop (the all-i kernel then fits 128 registers unspilled: 4 CTAs per SM)
-    unsigned bid;
-    asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(bid));
+    unsigned bid = work;
+    if (!DYN) asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(bid));
     const int it2 = bid % P.n_itiles, sp2 = bid / P.n_itiles;
 
     // a4: partial sums of this j-subset (second kernel adds them), or atomics (:63)
@@ -296,6 +300,42 @@ force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __res
             if (tid == 0) *R.counter = 0u;    // ready for the next call on this stream
         }
     }
+    if (DYN) {
+        // the CTA goes on to its next work item, which sets the ring up again: every warp is done
+        // with this one first, and a barrier is invalidated before it is initialised anew
+        __syncthreads();
+        if (tid == 0)
+            for (int s = 0; s < STG; ++s) mbar_inval(smem_u32(&bars[s]));
+    }
+}
+
+template <bool ATOMIC, bool FEW, int MODE, bool GUARD>
+__global__ void __launch_bounds__(FORCE_THREADS, NB_MINB)
+force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __restrict__ ojrk,
+             double* __restrict__ opot)
+{
+    force_body<ATOMIC, FEW, MODE, GUARD, false>(P, R, blockIdx.x, oacc, ojrk, opot);
+}
+
+// The pair kernel of a block whose size is only known on the device (nb_steps, steps.cu): the launch
+// shape -- threads per i, i-tiles, j-subsets -- was written to *plan by plan_kernel; a fixed grid of
+// resident CTAs loops over the work items.  Exits at once when no block is pending or when the plan
+// asks for the other instantiation.
+template <bool FEW, bool GUARD>
+__global__ void __launch_bounds__(FORCE_THREADS, NB_DYN_MINB) force_dyn_kernel(const DynPlan* __restrict__ plan)
+{
+    if (!plan->go || (plan->fa.jsh > 0) != FEW) return;
+    __shared__ ForceArgs sP;
+    __shared__ ReduceArgs sR;
+    if (threadIdx.x == 0) {
+        sP = plan->fa;
+        sR = plan->ra;
+    }
+    __syncthreads();
+    const unsigned items = (unsigned)sP.n_itiles * (unsigned)sP.splits;
+    for (unsigned w = blockIdx.x; w < items; w += gridDim.x) {
+        force_body<false, FEW, 0, GUARD, true>(sP, sR, w, nullptr, nullptr, nullptr);
+    }
 }
 
 // a4/a5 as a kernel of its own (all-i calls, atomics mode, fp64 and fused kernels)
@@ -306,6 +346,23 @@ __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
     const int k = WARP ? gt / 32 : gt;
     if (k >= R.ni) return;
     reduce_row<WARP>(R, k, threadIdx.x & 31);
+}
+
+// the reduction of a block planned on the device: one warp per i while the block is small and its
+// j-subsets many, else one thread per i; the grid is sized for the largest block and exits early
+__global__ void __launch_bounds__(128) reduce_dyn_kernel(const DynPlan* __restrict__ plan)
+{
+    if (!plan->go) return;
+    __shared__ ReduceArgs sR;
+    if (threadIdx.x == 0) sR = plan->ra;
+    __syncthreads();
+    const int64_t gt = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (sR.splits > 8 && sR.ni <= 4096) {
+        const int64_t k = gt / 32;
+        if (k < sR.ni) reduce_row<true>(sR, (int)k, threadIdx.x & 31);
+    } else if (gt < sR.ni) {
+        reduce_row<false>(sR, (int)gt, threadIdx.x & 31);
+    }
 }
 
 __global__ void __launch_bounds__(256) zero_out_kernel(double* acc, double* jrk, double* pot, int64_t ni)
@@ -330,7 +387,7 @@ __host__ __device__ constexpr int force_smem(bool few)
 }  // namespace
 
 template <bool FEW>
-cudaError_t setup_one(int* blocks, int* blocks_guard)
+cudaError_t setup_one(int* blocks, int* blocks_guard, int* blocks_dyn, int* blocks_dyn_guard)
 {
     const void* k[8] = {(const void*)force_kernel<false, FEW, 0, false>, (const void*)force_kernel<true, FEW, 0, false>,
                         (const void*)force_kernel<false, FEW, 1, false>, (const void*)force_kernel<false, FEW, 2, false>,
@@ -345,6 +402,17 @@ cudaError_t setup_one(int* blocks, int* blocks_guard)
         if (e != cudaSuccess) return e;
         if (q == 0 || b < least) least = b;
     }
+    {
+        const void* kd[2] = {(const void*)force_dyn_kernel<FEW, false>, (const void*)force_dyn_kernel<FEW, true>};
+        int* out[2] = {blocks_dyn, blocks_dyn_guard};
+        for (int q = 0; q < 2; ++q) {
+            cudaError_t e = cudaFuncSetAttribute(kd[q], cudaFuncAttributeMaxDynamicSharedMemorySize, force_smem(FEW));
+            if (e != cudaSuccess) return e;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(out[q], kd[q], FORCE_THREADS, force_smem(FEW));
+            if (e != cudaSuccess) return e;
+            if (*out[q] < least) least = *out[q];
+        }
+    }
     // the dispatcher sizes whole waves with the by-index kernels' residency; the others only need >= 1
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks, k[0], FORCE_THREADS, force_smem(FEW));
     if (e == cudaSuccess)
@@ -352,12 +420,13 @@ cudaError_t setup_one(int* blocks, int* blocks_guard)
     return (e == cudaSuccess && least < 1) ? cudaErrorLaunchOutOfResources : e;
 }
 
-// blocks_per_sm[0..3]: CTAs per SM of the all-i kernel, its guarded form, the few-i kernel, its guarded form
+// blocks_per_sm[0..3]: CTAs per SM of the all-i kernel, its guarded form, the few-i kernel, its guarded
+// form; [4..7]: the same for the device-planned kernels of nb_steps (force_dyn_kernel)
 cudaError_t force_kernel_setup(int* blocks_per_sm)
 {
-    cudaError_t e = setup_one<false>(blocks_per_sm + 0, blocks_per_sm + 1);
+    cudaError_t e = setup_one<false>(blocks_per_sm + 0, blocks_per_sm + 1, blocks_per_sm + 4, blocks_per_sm + 5);
     if (e != cudaSuccess) return e;
-    return setup_one<true>(blocks_per_sm + 2, blocks_per_sm + 3);
+    return setup_one<true>(blocks_per_sm + 2, blocks_per_sm + 3, blocks_per_sm + 6, blocks_per_sm + 7);
 }
 
 // mode: 0 = by index (nb_force), 1 = by value with jerk, 2 = by value, acc + pot only (nb_force_ext;
@@ -389,6 +458,28 @@ cudaError_t launch_force(const ForceArgs& a, const ReduceArgs& r, int mode, int 
         if (guard) launch_one<false, true>(a, r, mode, atomic_mode, acc, jrk, pot, s);
         else launch_one<false, false>(a, r, mode, atomic_mode, acc, jrk, pot, s);
     }
+    return cudaGetLastError();
+}
+
+// both instantiations are queued; the plan decides on the device which one works
+cudaError_t launch_force_dyn(const DynPlan* plan, float eps2, int resident_all, int resident_few, cudaStream_t s)
+{
+    if (eps2 < EPS2_GUARD) {
+        force_dyn_kernel<true, true><<<resident_few, FORCE_THREADS, force_smem(true), s>>>(plan);
+        force_dyn_kernel<false, true><<<resident_all, FORCE_THREADS, force_smem(false), s>>>(plan);
+    } else {
+        force_dyn_kernel<true, false><<<resident_few, FORCE_THREADS, force_smem(true), s>>>(plan);
+        force_dyn_kernel<false, false><<<resident_all, FORCE_THREADS, force_smem(false), s>>>(plan);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_dyn(const DynPlan* plan, int64_t ni_max, cudaStream_t s)
+{
+    // one thread per i up to ni_max, or one warp per i up to 4096: the larger of the two grids
+    int64_t grid = (ni_max + 127) / 128;
+    if (grid < 1024 && ni_max > 128) grid = ni_max < 4096 ? (ni_max * 32 + 127) / 128 : 1024;
+    reduce_dyn_kernel<<<(unsigned)grid, 128, 0, s>>>(plan);
     return cudaGetLastError();
 }
 

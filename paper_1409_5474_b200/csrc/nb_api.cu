@@ -14,7 +14,7 @@ struct nb_ctx {
     cudaStream_t stream = nullptr;
     int64_t n_max = 0, ni_max = 0, n_cap = 0, n = 0;
     int sm_count = 148;
-    int blocks_per_sm[4] = {1, 1, 1, 1};   // all-i kernel, its guarded form, few-i kernel, its guarded form
+    int blocks_per_sm[8] = {1, 1, 1, 1, 1, 1, 1, 1};   // all-i kernel, its guarded form, few-i kernel, its guarded form; [4..7] the same for nb_steps' device-planned kernels
 
     // device memory: either one cudaMalloc'ed slab or the caller's workspace
     bool allocated = false, own_slab = false;
@@ -49,6 +49,17 @@ struct nb_ctx {
     int64_t steps_log_cap = 0;
     int64_t steps_max_pairs = 30000000; // blocks with ni x n above this go through nb_step's launches
     int steps_ok = -1;                  // -1 unknown, 0 the cooperative kernel cannot be resident, 1 fine
+    DynPlan* steps_plan = nullptr;      // the device-planned launch shape of a handed-over block
+    StepsProgress* steps_prog = nullptr;   // where a queued batch of nb_steps stands
+    int steps_queue = 2;                // 0: host handover; 1: rounds queued ahead on the stream; 2: one graph with a WHILE node
+    // the graph of mode 2 (built on first use, rebuilt when an argument baked into its kernels changes)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraph_t steps_graph = nullptr;
+    cudaGraphExec_t steps_exec = nullptr;
+    int steps_graph_state = 0;          // 0 none yet, 1 usable, -1 cannot be built here (mode 1 is used)
+    double steps_key[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const void* steps_key_ptr[3] = {nullptr, nullptr, nullptr};
+    void* steps_pinned = nullptr;       // pinned: StepsProgress in / out, the exit words of the last kernel
     double blk_t = 0.0;                 // what the last nb_next_block returned
     int64_t blk_ni = -1;
 
@@ -62,7 +73,8 @@ struct nb_ctx {
     float* pack6 = nullptr;
     int blocks_per_sm6 = 1;
 
-    int* err_pinned = nullptr;          // pinned: [0] error latch copy; bytes 8..23: sel_meta copy; 32..63: nb_steps status
+    int* err_pinned = nullptr;          // pinned, 256 B: [0] error latch copy; bytes 8..23: sel_meta copy; 32..63: nb_steps status;
+                                        // 64..: StepsProgress sent, 128..: StepsProgress read back, 192..: exit words
     std::vector<int32_t> flagged;   // host copy of the flagged set (sorted)
 
     struct SplitMemo {
@@ -101,7 +113,7 @@ inline size_t up(size_t x, size_t a = ALIGN) { return (x + a - 1) / a * a; }
 
 struct Layout {
     size_t store, pack, flags, tileflag, flag_list, flag_stage, part, err, ilist, out, in, dts, blk_list, blk_out,
-        sel_meta, sel_counts, steps_slots, steps_meta, total;
+        sel_meta, sel_counts, steps_slots, steps_meta, steps_plan, steps_prog, total;
     int64_t ni_pad;
     size_t part_bytes;
     int64_t n_cap;
@@ -136,6 +148,8 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.sel_counts = off; off += up((size_t)SEL_MAX_BLOCKS * 4);
     L.steps_slots = off; off += up((size_t)256 * sizeof(StepsSlot));
     L.steps_meta = off; off += up(8 * 8);
+    L.steps_plan = off; off += up(sizeof(DynPlan));
+    L.steps_prog = off; off += up(sizeof(StepsProgress));
     L.ni_pad = ni_pad;
     L.total = off;
     return L;
@@ -179,6 +193,8 @@ int ensure_alloc(nb_ctx* c)
     c->sel_counts = reinterpret_cast<int*>(c->slab + L.sel_counts);
     c->steps_slots = reinterpret_cast<StepsSlot*>(c->slab + L.steps_slots);
     c->steps_meta = reinterpret_cast<unsigned long long*>(c->slab + L.steps_meta);
+    c->steps_plan = reinterpret_cast<DynPlan*>(c->slab + L.steps_plan);
+    c->steps_prog = reinterpret_cast<StepsProgress*>(c->slab + L.steps_prog);
     c->ni_pad = L.ni_pad;
     c->allocated = true;
     return NB_OK;
@@ -506,7 +522,7 @@ int nb_create(nb_ctx** out, int64_t n_max, int64_t ni_max, int device, void* str
         delete c;
         return NB_ERR_CUDA;
     }
-    if (cudaMallocHost(&c->err_pinned, 64) != cudaSuccess) {
+    if (cudaMallocHost(&c->err_pinned, 256) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return NB_ERR_ALLOC;
@@ -526,6 +542,9 @@ int nb_destroy(nb_ctx* c)
     if (c->steps_log_t) cudaFree(c->steps_log_t);
     if (c->steps_log_ni) cudaFree(c->steps_log_ni);
     if (c->steps_log_ns) cudaFree(c->steps_log_ns);
+    if (c->steps_exec) cudaGraphExecDestroy(c->steps_exec);
+    if (c->steps_graph) cudaGraphDestroy(c->steps_graph);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
     for (nb_ctx::Rec& R : c->ring)
         for (cudaEvent_t e : R.e)
@@ -1141,6 +1160,215 @@ int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs)
     c->steps_max_pairs = max_pairs;
     return NB_OK;
 }
+int nb_set_steps_queue(nb_ctx* c, int on)
+{
+    if (!c) return NB_ERR_ARG;
+    if (on < 0 || on > 2) return NB_ERR_ARG;
+    c->steps_queue = on;
+    return NB_OK;
+}
+
+// nb_steps with handed-over blocks planned ON THE DEVICE (steps.cu plan_kernel): the host queues
+// rounds of [persistent kernel, plan, predictor, pair kernel (both mappings), reduction, corrector]
+// without knowing how large the block of a round is, or whether there is one -- every kernel of a
+// round reads the plan and exits at once when it has nothing to do -- and looks at the progress
+// record once per batch of rounds.  No host round trip per large block.
+static int steps_queued(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, double dt_max, double t_end,
+                        bool want_us, int64_t* done)
+{
+    unsigned char* pin = reinterpret_cast<unsigned char*>(c->err_pinned);
+    StepsProgress* p_in = reinterpret_cast<StepsProgress*>(pin + 64);
+    StepsProgress* p_out = reinterpret_cast<StepsProgress*>(pin + 128);
+    unsigned long long* meta_out = reinterpret_cast<unsigned long long*>(pin + 192);
+    memset(p_in, 0, sizeof(StepsProgress));
+    p_in->k = k;
+    p_in->reason = STEPS_RUNNING;
+    if (cudaMemcpyAsync(c->steps_prog, p_in, sizeof(StepsProgress), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemsetAsync(c->steps_plan, 0, sizeof(int), c->stream) != cudaSuccess)
+        return NB_ERR_CUDA;
+
+    StepsArgs a{};
+    a.st = c->store;
+    a.dts = c->dts;
+    a.flags = c->flags;
+    a.any_flagged = c->flagged.empty() ? 0 : 1;
+    a.n = c->n;
+    a.slots = c->steps_slots;
+    a.list = c->blk_list;
+    a.cap = c->ni_max;
+    a.part = c->part;
+    a.out = c->blk_out;
+    a.meta = c->steps_meta;
+    a.log_t = c->steps_log_t;
+    a.log_ni = c->steps_log_ni;
+    a.log_ns = c->steps_log_ns;
+    a.budget = 0;
+    a.eps2 = eps2;
+    a.eta = eta;
+    a.dt_min = dt_min;
+    a.dt_max = dt_max;
+    a.t_end = t_end;
+    a.max_pairs = c->steps_max_pairs;
+    a.err = c->err;
+    a.trace = nullptr;
+    a.prog = c->steps_prog;
+
+    // what the plan cannot know: the fixed arguments of the pair kernel and of the reduction
+    ForceArgs fa{};
+    fa.pack = c->pack;
+    fa.i_list = c->blk_list;
+    fa.part = c->part;
+    fa.flags = c->flags;
+    fa.tileflag = c->tileflag;
+    fa.err = c->err;
+    fa.n = (int)c->n;
+    fa.ntiles = (int)((c->n + TJ - 1) / TJ);
+    fa.eps2 = (float)eps2;
+    fa.any_flagged = a.any_flagged;
+    fa.pack64 = nullptr;
+    fa.eps2d = eps2;
+    ReduceArgs ra{};
+    ra.part = c->part;
+    ra.part_b = c->part;
+    ra.i_list = c->blk_list;
+    ra.acc = c->blk_out;
+    ra.store = c->store;
+    ra.flags = c->flags;
+    ra.flag_list = c->flag_list;
+    ra.nflag = (int)c->flagged.size();
+    ra.n = (int)c->n;
+    ra.counter = c->ticket;
+    const bool guard = (float)eps2 < EPS2_GUARD;
+    const int resident_all = c->sm_count * c->blocks_per_sm[guard ? 5 : 4];
+    const int resident_few = c->sm_count * c->blocks_per_sm[guard ? 7 : 6];
+
+    // one round on stream st; cond/loop: the plan kernel also drives the WHILE node of the graph
+    auto round = [&](cudaStream_t st, unsigned long long cond, int loop) -> bool {
+        return launch_steps(a, c->sm_count, st) == cudaSuccess &&
+               launch_plan(a, c->steps_plan, c->steps_prog, fa, ra, resident_all, resident_few, c->part_bytes, st, cond,
+                           loop) == cudaSuccess &&
+               launch_predict(c->store, c->flags, c->pack, nullptr, nullptr, c->n, 0.0, st, c->steps_plan) ==
+                   cudaSuccess &&
+               launch_force_dyn(c->steps_plan, (float)eps2, resident_all, resident_few, st) == cudaSuccess &&
+               launch_reduce_dyn(c->steps_plan, c->ni_max, st) == cudaSuccess &&
+               launch_correct_dyn(c->store, c->dts, c->steps_plan, c->n, c->ni_max, eta, dt_min, dt_max, c->err, st) ==
+                   cudaSuccess;
+    };
+
+    // Mode 2: the rounds are the body of a WHILE node of ONE graph (the plan kernel sets the loop
+    // condition on the device), followed by a launch that closes the last time stamp: one graph launch
+    // per nb_steps call, no empty rounds, nothing for the host to do until the end.
+    if (c->steps_queue == 2 && c->steps_graph_state >= 0) {
+        const double key[8] = {eps2, eta, dt_min, dt_max, t_end, (double)c->steps_max_pairs, (double)c->n,
+                               (double)c->flagged.size()};
+        const void* kp[3] = {c->steps_log_t, c->steps_log_ni, c->steps_log_ns};
+        const bool same = c->steps_graph_state == 1 && memcmp(key, c->steps_key, sizeof(key)) == 0 &&
+                          memcmp(kp, c->steps_key_ptr, sizeof(kp)) == 0;
+        if (!same) {
+            if (c->steps_exec) cudaGraphExecDestroy(c->steps_exec);
+            if (c->steps_graph) cudaGraphDestroy(c->steps_graph);
+            c->steps_exec = nullptr;
+            c->steps_graph = nullptr;
+            c->steps_graph_state = -1;
+            bool ok = c->cap_stream || cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
+            cudaGraphConditionalHandle handle = 0;
+            cudaGraphNode_t wnode = nullptr;
+            cudaGraph_t body = nullptr, tmp = nullptr;
+            ok = ok && cudaGraphCreate(&c->steps_graph, 0) == cudaSuccess;
+            ok = ok && cudaGraphConditionalHandleCreate(&handle, c->steps_graph, 1, cudaGraphCondAssignDefault) ==
+                           cudaSuccess;
+            if (ok) {
+                cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+                memset(&np, 0, sizeof(np));
+                np.type = cudaGraphNodeTypeConditional;
+                np.conditional.handle = handle;
+                np.conditional.type = cudaGraphCondTypeWhile;
+                np.conditional.size = 1;
+                ok = cudaGraphAddNode(&wnode, c->steps_graph, nullptr, 0, &np) == cudaSuccess;
+                if (ok) body = np.conditional.phGraph_out[0];
+            }
+            if (ok && cudaStreamBeginCaptureToGraph(c->cap_stream, body, nullptr, nullptr, 0,
+                                                     cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+                const bool queued_ok = round(c->cap_stream, (unsigned long long)handle, 1);
+                ok = cudaStreamEndCapture(c->cap_stream, &tmp) == cudaSuccess && queued_ok;
+            } else {
+                ok = false;
+            }
+            if (ok && cudaStreamBeginCaptureToGraph(c->cap_stream, c->steps_graph, &wnode, nullptr, 1,
+                                                     cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+                const bool queued_ok = launch_steps(a, c->sm_count, c->cap_stream) == cudaSuccess;
+                ok = cudaStreamEndCapture(c->cap_stream, &tmp) == cudaSuccess && queued_ok;
+            } else {
+                ok = false;
+            }
+            ok = ok && cudaGraphInstantiate(&c->steps_exec, c->steps_graph, 0) == cudaSuccess;
+            if (ok) {
+                c->steps_graph_state = 1;
+                memcpy(c->steps_key, key, sizeof(key));
+                memcpy(c->steps_key_ptr, kp, sizeof(kp));
+            } else {
+                cudaGetLastError();               // this driver cannot build it: stream-queued rounds from now on
+                if (c->steps_exec) cudaGraphExecDestroy(c->steps_exec);
+                if (c->steps_graph) cudaGraphDestroy(c->steps_graph);
+                c->steps_exec = nullptr;
+                c->steps_graph = nullptr;
+            }
+        }
+    }
+
+    int result = NB_OK;
+    if (c->steps_queue == 2 && c->steps_graph_state == 1) {
+        if (cudaGraphLaunch(c->steps_exec, c->stream) != cudaSuccess) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        c->launches += 1;                         // one graph launch; its kernels are counted from the log below
+        c->predicted = false;
+        if (cudaMemcpyAsync(p_out, c->steps_prog, sizeof(StepsProgress), cudaMemcpyDeviceToHost, c->stream) !=
+                cudaSuccess ||
+            cudaMemcpyAsync(meta_out, c->steps_meta + 4, 32, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        c->launches += 7 * (int64_t)p_out->rounds;
+    } else {
+    int64_t rounds = k < 4 ? k : 4;           // rounds in the first batch
+    int64_t rounds_total = 0;
+    for (;;) {
+        for (int64_t r = 0; r < rounds; ++r) {
+            if (!round(c->stream, 0ull, 0)) {
+                cudaGetLastError();
+                return NB_ERR_CUDA;
+            }
+            c->launches += 7;
+        }
+        c->predicted = false;
+        if (cudaMemcpyAsync(p_out, c->steps_prog, sizeof(StepsProgress), cudaMemcpyDeviceToHost, c->stream) !=
+                cudaSuccess ||
+            cudaMemcpyAsync(meta_out, c->steps_meta + 4, 32, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        if (p_out->final || p_out->done >= k) break;
+        // every round of the batch ended at a large block: size the next batch by the rate seen so far
+        rounds_total += rounds;
+        const double per_step = (double)rounds_total / (double)(p_out->done > 0 ? p_out->done : 1);
+        int64_t want = (int64_t)(per_step * (double)(k - p_out->done) * 1.1) + 1;
+        rounds = want < 2 ? 2 : (want > 64 ? 64 : want);
+    }
+    }
+    *done = p_out->done;
+    if (p_out->pending_ni > 0) result = NB_ERR_ARG;            // a block above ni_max: the list was truncated
+    else if (p_out->final && p_out->reason == STEPS_STUCK) result = NB_ERR_STATE;
+    if (p_out->done > 0) c->blk_ni = (int64_t)meta_out[3];     // for nb_block_forces
+    if (want_us && !p_out->closed && p_out->pending_ni == 0 && !(c->steps_queue == 2 && c->steps_graph_state == 1)) {
+        // the batch ended with a device-planned block: one more (empty) launch stamps the closing time
+        if (launch_steps(a, c->sm_count, c->stream) != cudaSuccess) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        c->launches += 1;
+    }
+    return result;
+}
 
 int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, double dt_max, double t_end,
              double* t_log, int64_t* ni_log, double* us_log, int64_t* done)
@@ -1167,15 +1395,23 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
         c->steps_log_ni = nullptr;
         c->steps_log_ns = nullptr;
         c->steps_log_cap = 0;
-        if (cudaMalloc(&c->steps_log_t, (size_t)k * 8) != cudaSuccess ||
-            cudaMalloc(&c->steps_log_ni, (size_t)k * 8) != cudaSuccess ||
-            cudaMalloc(&c->steps_log_ns, (size_t)(k + 1) * 8) != cudaSuccess) {
+        // (re)allocation synchronises the device: at least 4096 entries, then doubling
+        int64_t cap = c->steps_log_cap > 0 ? c->steps_log_cap : 4096;
+        while (cap < k) cap *= 2;
+        if (cudaMalloc(&c->steps_log_t, (size_t)cap * 8) != cudaSuccess ||
+            cudaMalloc(&c->steps_log_ni, (size_t)cap * 8) != cudaSuccess ||
+            cudaMalloc(&c->steps_log_ns, (size_t)(cap + 1) * 8) != cudaSuccess) {
             cudaGetLastError();
             return NB_ERR_ALLOC;
         }
-        c->steps_log_cap = k;
+        c->steps_log_cap = cap;
     }
     unsigned long long* status = reinterpret_cast<unsigned long long*>(c->err_pinned) + 4;
+    // handed-over blocks are planned on the device and queued, unless the mode was switched off, the
+    // pair loop is the IEEE-double one (its launch shapes are not planned on the device) or the
+    // reduction runs by atomics
+    const bool queued = c->steps_ok == 1 && c->steps_queue && c->precision == 0 && c->tune_reduce == 0 &&
+                        c->tune_splits == 0;
     std::vector<int64_t> host_idx;            // steps that went through the host path: (index, t, ni)
     std::vector<double> host_t;
     std::vector<int64_t> host_ni;
@@ -1215,7 +1451,11 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
         c->predicted = false;
         return NB_OK;
     };
-    while (s < k) {
+    if (queued) {
+        result = steps_queued(c, k, eps2, eta, dt_min, dt_max, t_end, us_log != nullptr, &s);
+        if (result == NB_ERR_CUDA) return result;
+    }
+    while (!queued && s < k) {
         double t = 0.0;
         int64_t ni = 0;
         if (c->steps_ok == 1) {

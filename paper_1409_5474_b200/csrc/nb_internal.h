@@ -25,6 +25,9 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 #ifndef NB_MINB
 #define NB_MINB 3
 #endif
+#ifndef NB_DYN_MINB
+#define NB_DYN_MINB 3
+#endif
 #ifndef NB_UNROLL
 #define NB_UNROLL 2
 #endif
@@ -115,10 +118,10 @@ cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int3
                             int64_t count, int64_t n, int* err, cudaStream_t s);
 cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int count, cudaStream_t s);
 cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64, float* pack6,
-                           int64_t n, double t, cudaStream_t s);
+                           int64_t n, double t, cudaStream_t s, const struct DynPlan* plan = nullptr);
 cudaError_t launch_get_predicted(const StorePtrs& store, int64_t first, int64_t count, double t,
                                  double* out, cudaStream_t s);
-cudaError_t force_kernel_setup(int* blocks_per_sm /*[4]*/);
+cudaError_t force_kernel_setup(int* blocks_per_sm /*[8]*/);
 cudaError_t force64_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_force64(const ForceArgs& a, int mode, cudaStream_t s);
 cudaError_t launch_force(const ForceArgs& a, const ReduceArgs& r, int mode, int atomic_mode, double* acc,
@@ -189,8 +192,38 @@ struct StepsArgs {
     int64_t max_pairs;            // a block with ni x n above this is left to the host path
     int* err;
     unsigned long long* trace;    // NB_STEPS_TRACE builds only
+    struct StepsProgress* prog;   // non-NULL: budget and log offset come from here (queued batches)
+};
+// A block that the persistent kernel hands over, planned ON THE DEVICE so that the host can queue its
+// kernels without knowing its size (steps.cu plan_kernel -> predict / force_dyn / reduce_dyn /
+// correct_dyn, all of which exit at once while go == 0).
+struct DynPlan {
+    int go;                       // 1: a block is pending and planned
+    int pad;
+    double t1;                    // its time
+    long long ni;                 // its size
+    ForceArgs fa;                 // launch shape and arguments of the pair kernel
+    ReduceArgs ra;                // ... and of the reduction
+};
+struct StepsProgress {            // where a batch of queued kernels stands (device memory)
+    long long done;               // block steps completed since nb_steps was called
+    long long k;                  // steps asked for
+    int final;                    // 1: stop (t_end reached, nothing schedulable, an error)
+    int reason;                   // StepsReason of the last persistent-kernel exit
+    long long pending_ni;         // size of a block that could not be planned (ni > ni_max)
+    int closed;                   // 1: log_ns[done] holds the time stamp that closes the last step
+    int rounds;                   // rounds (persistent kernel + plan + block kernels) run so far
 };
 cudaError_t steps_kernel_setup(int* blocks_per_sm);
+// one round of the device-planned path for a handed-over block; every kernel is a no-op while no block
+// is pending.  resident = CTAs of the pair kernel that fit the chip (grid of force_dyn_kernel).
+cudaError_t launch_plan(const StepsArgs& a, DynPlan* plan, StepsProgress* prog, const ForceArgs& fa_base,
+                        const ReduceArgs& ra_base, int resident_all, int resident_few, size_t part_bytes,
+                        cudaStream_t s, unsigned long long cond_handle = 0, int loop = 0);
+cudaError_t launch_force_dyn(const DynPlan* plan, float eps2, int resident_all, int resident_few, cudaStream_t s);
+cudaError_t launch_reduce_dyn(const DynPlan* plan, int64_t ni_max, cudaStream_t s);
+cudaError_t launch_correct_dyn(const StorePtrs& st, double* dts, const DynPlan* plan, int64_t n, int64_t ni_max,
+                               double eta, double dt_min, double dt_max, int* err, cudaStream_t s);
 cudaError_t launch_steps(const StepsArgs& a, int sm_count, cudaStream_t s);
 
 // Hermite predictor of one component (R1), shared by predict / get_predicted / the flagged-pair

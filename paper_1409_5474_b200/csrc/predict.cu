@@ -70,8 +70,13 @@ template <bool P64, bool P6>
 __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_t* __restrict__ flags,
                                                       float* __restrict__ pack,
                                                       double* __restrict__ pack64, float* __restrict__ pack6,
-                                                      int64_t n, int64_t n_pad, double t)
+                                                      int64_t n, int64_t n_pad, double t,
+                                                      const DynPlan* __restrict__ plan)
 {
+    if (plan) {                   // a block planned on the device (nb_steps): its time, or nothing to do
+        if (!plan->go) return;
+        t = plan->t1;
+    }
     const int64_t p = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
     if (p >= n_pad) return;
     const double2 tj = ld2(st.f[F_T], p);
@@ -188,16 +193,16 @@ cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int co
 }
 
 cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* pack, double* pack64,
-                           float* pack6, int64_t n, double t, cudaStream_t s)
+                           float* pack6, int64_t n, double t, cudaStream_t s, const DynPlan* plan)
 {
     if (n == 0) return cudaSuccess;
     const int64_t n_pad = (n + TJ - 1) / TJ * TJ;
     const int64_t threads = n_pad / 2;
     const unsigned grid = (unsigned)((threads + 127) / 128);
-    if (pack64 && pack6) predict_kernel<true, true><<<grid, 128, 0, s>>>(store, flags, pack, pack64, pack6, n, n_pad, t);
-    else if (pack64) predict_kernel<true, false><<<grid, 128, 0, s>>>(store, flags, pack, pack64, nullptr, n, n_pad, t);
-    else if (pack6) predict_kernel<false, true><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, pack6, n, n_pad, t);
-    else predict_kernel<false, false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, nullptr, n, n_pad, t);
+    if (pack64 && pack6) predict_kernel<true, true><<<grid, 128, 0, s>>>(store, flags, pack, pack64, pack6, n, n_pad, t, plan);
+    else if (pack64) predict_kernel<true, false><<<grid, 128, 0, s>>>(store, flags, pack, pack64, nullptr, n, n_pad, t, plan);
+    else if (pack6) predict_kernel<false, true><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, pack6, n, n_pad, t, plan);
+    else predict_kernel<false, false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, nullptr, n, n_pad, t, plan);
     return cudaGetLastError();
 }
 

@@ -144,10 +144,28 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         for (int q = tid; q < cnt_own; q += ST_THREADS) keys[q] = key_of(ldcg(T + lo + q) + ldcg(P.dts + lo + q));
     __syncthreads();
 
+    // queued batches (nb_steps): how many steps are left and where the log continues is read from
+    // device memory, because the host queued this launch before it knew; every CTA reads the same
+    // values (they were written before this launch)
+    int64_t budget = P.budget;
+    if (P.prog) {
+        const long long done0 = P.prog->done;
+        budget = P.prog->final ? 0 : P.prog->k - done0;
+        if (budget <= 0) {                    // nothing left: close the last step's time stamp once
+            if (b == 0 && tid == 0 && !P.prog->closed) {
+                P.log_ns[done0] = gtime();
+                P.prog->closed = 1;
+            }
+            return;
+        }
+        P.log_t += done0;
+        P.log_ni += done0;
+        P.log_ns += done0;
+    }
     long long last_ni = 0;                    // size of the last block this launch completed
-    for (int64_t s = 0; s <= P.budget; ++s) {
+    for (int64_t s = 0; s <= budget; ++s) {
         if (b == 0 && tid == 0) P.log_ns[s] = gtime();
-        if (s == P.budget) break;
+        if (s == budget) break;
         TRACE(0);
 
         // ---- A: earliest time of my slice and who is due then (R21) ----------------------------
@@ -213,6 +231,14 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
                 meta[5] = (unsigned long long)reason;
                 meta[6] = kall;
                 meta[7] = (unsigned long long)(reason == STEPS_BIG ? ni64 : last_ni);
+                if (P.prog) {
+                    P.prog->done += s;
+                    P.prog->reason = reason;
+                    if (reason != STEPS_BIG) {
+                        P.prog->final = 1;
+                        P.prog->closed = 1;   // log_ns[s] was stamped when this step began
+                    }
+                }
             }
             return;
         }
@@ -372,11 +398,130 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         last_ni = ni64;
     }
     if (b == 0 && tid == 0) {
-        meta[4] = (unsigned long long)P.budget;
+        meta[4] = (unsigned long long)budget;
         meta[5] = (unsigned long long)STEPS_DONE;
         meta[6] = 0ull;
         meta[7] = (unsigned long long)last_ni;
+        if (P.prog) {
+            P.prog->done += budget;
+            P.prog->reason = STEPS_DONE;
+            P.prog->closed = 1;
+        }
     }
+}
+
+// After the persistent kernel: if it stopped at a block it does not take itself, plan that block's
+// kernels -- threads per i, i-tiles, j-subsets, buffers -- in device memory, log it and count it as
+// done (its kernels are queued right behind this one).  One thread.
+__device__ __forceinline__ bool plan_block(const StepsArgs& P, DynPlan* plan, ForceArgs& fa, ReduceArgs& ra,
+                                           int resident_all, int resident_few, size_t part_bytes);
+
+// loop != 0: the kernel sits in the body of a graph's WHILE node and decides whether the body runs
+// again (another round is needed while steps are left and nothing stopped the run)
+__global__ void plan_kernel(StepsArgs P, DynPlan* plan, ForceArgs fa, ReduceArgs ra, int resident_all,
+                            int resident_few, size_t part_bytes, cudaGraphConditionalHandle handle, int loop)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    P.prog->rounds += 1;
+    plan_block(P, plan, fa, ra, resident_all, resident_few, part_bytes);
+    if (loop) {
+        const StepsProgress* g = P.prog;
+        cudaGraphSetConditional(handle, (!g->final && g->done < g->k) ? 1u : 0u);
+    }
+}
+
+__device__ __forceinline__ bool plan_block(const StepsArgs& P, DynPlan* plan, ForceArgs& fa, ReduceArgs& ra,
+                                           int resident_all, int resident_few, size_t part_bytes)
+{
+    plan->go = 0;
+    StepsProgress* g = P.prog;
+    if (g->final || g->reason != STEPS_BIG || g->done >= g->k) return false;
+    const long long ni = (long long)P.meta[7];
+    if (ni > P.cap) {                         // the list was truncated: the host reports the error
+        g->final = 1;
+        g->pending_ni = ni;
+        return false;
+    }
+    const double t1 = of_key(P.meta[6]);
+    // launch shape (nb_api.cu force_impl does the same on the host for nb_force)
+    int jsh = 0;
+    while (jsh < JSH_MAX && (ITILE >> (jsh + 1)) >= ni) ++jsh;
+    const int itile = ITILE >> jsh;
+    const int n_itiles = (int)((ni + itile - 1) / itile);
+    const int resident = jsh > 0 ? resident_few : resident_all;
+    long long smax = (long long)(part_bytes / (NOUT * sizeof(double) * (size_t)n_itiles * itile));
+    if (smax > fa.ntiles) smax = fa.ntiles;
+    if (smax > 4096) smax = 4096;
+    // j-subsets: the resident CTAs loop over n_itiles x S work items, so for every
+    // number of waves w the best S is the largest one that still fits w waves; of those the one with
+    // the best useful-tile fraction wins (each item also pays about two tiles of gather, pipeline fill
+    // and partial store -- the model nb_api.cu choose_splits uses on the host)
+    long long splits = 1;
+    double best = -1.0;
+    const long long w0 = (n_itiles + resident - 1) / resident;
+    for (long long w = w0; w < w0 + 12; ++w) {
+        long long sw = w * resident / n_itiles;
+        if (sw > smax) sw = smax;
+        if (sw < 1) sw = 1;
+        const long long items = (long long)n_itiles * sw;
+        const long long waves = (items + resident - 1) / resident;
+        const long long per = (fa.ntiles + sw - 1) / sw;
+        const double eff = (double)n_itiles * fa.ntiles / ((double)waves * resident * (double)(per + 2));
+        if (eff > best * 1.004) {
+            best = eff;
+            splits = sw;
+        }
+        if (sw == smax) break;
+    }
+    fa.ni = (int)ni;
+    fa.jsh = jsh;
+    fa.k0 = 0;
+    fa.n_itiles = n_itiles;
+    fa.ni_pad = n_itiles * itile;
+    fa.splits = (int)splits;
+    fa.reduce_here = 0;
+    ra.kA = (int)ni;
+    ra.ni = (int)ni;
+    ra.ni_pad = fa.ni_pad;
+    ra.splits = (int)splits;
+    ra.jrk = ra.acc + 3 * ni;                 // the context's block forces: [7][ni]
+    ra.pot = ra.acc + 6 * ni;
+    ra.t_pred = t1;
+    plan->fa = fa;
+    plan->ra = ra;
+    plan->t1 = t1;
+    plan->ni = ni;
+    plan->go = 1;
+    P.log_t[g->done] = t1;
+    P.log_ni[g->done] = ni;
+    g->done += 1;
+    g->closed = 0;                            // the step's closing time stamp is the next launch's first
+    g->reason = STEPS_RUNNING;                // taken: a kernel that starts with nothing left must not see it again
+    P.meta[7] = (unsigned long long)ni;       // for nb_block_forces after the batch
+    return true;
+}
+
+// corrector of a device-planned block (hermite.cu correct_kernel with its arguments read from the plan)
+__global__ void __launch_bounds__(128)
+correct_dyn_kernel(StorePtrs st, double* __restrict__ dts, const DynPlan* __restrict__ plan, int64_t n, double eta,
+                   double dt_min, double dt_max, int* err)
+{
+    if (!plan->go) return;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t ni = plan->ni;
+    if (k >= ni) return;
+    const int64_t i = plan->ra.i_list[k];
+    if (i < 0 || i >= n) {
+        atomicOr(err, 1);
+        return;
+    }
+    double a1[3], j1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        a1[c] = plan->ra.acc[(int64_t)c * ni + k];
+        j1[c] = plan->ra.jrk[(int64_t)c * ni + k];
+    }
+    correct_one(st, dts, i, plan->t1, a1, j1, eta, dt_min, dt_max, err);
 }
 
 }  // namespace
@@ -397,6 +542,24 @@ cudaError_t launch_steps(const StepsArgs& a, int sm_count, cudaStream_t s)
     StepsArgs copy = a;
     void* args[] = {(void*)&copy};
     return cudaLaunchCooperativeKernel((const void*)steps_kernel, dim3(grid), dim3(ST_THREADS), args, ST_SMEM, s);
+}
+
+cudaError_t launch_plan(const StepsArgs& a, DynPlan* plan, StepsProgress* prog, const ForceArgs& fa_base,
+                        const ReduceArgs& ra_base, int resident_all, int resident_few, size_t part_bytes,
+                        cudaStream_t s, unsigned long long cond_handle, int loop)
+{
+    StepsArgs copy = a;
+    copy.prog = prog;
+    plan_kernel<<<1, 32, 0, s>>>(copy, plan, fa_base, ra_base, resident_all, resident_few, part_bytes,
+                                 (cudaGraphConditionalHandle)cond_handle, loop);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_correct_dyn(const StorePtrs& st, double* dts, const DynPlan* plan, int64_t n, int64_t ni_max,
+                               double eta, double dt_min, double dt_max, int* err, cudaStream_t s)
+{
+    correct_dyn_kernel<<<(unsigned)((ni_max + 127) / 128), 128, 0, s>>>(st, dts, plan, n, eta, dt_min, dt_max, err);
+    return cudaGetLastError();
 }
 
 }  // namespace nb

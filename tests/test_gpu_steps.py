@@ -126,35 +126,91 @@ def test_steps_flags_eps0_and_t_end(nbmod):
             ctx.sync()
 
 
-def test_steps_host_path_and_mixed(nbmod):
-    """Bound 0: every block goes through nb_step's launches (the seam itself); default bound at
-    N = 3000: a mix.  The oracle is stepped in lock-step with the GPU's own log here, because fp32
-    forces may move a step decision near a threshold (tests/test_gpu_hermite.py)."""
+@pytest.mark.parametrize("queue", [2, 1, 0])
+def test_steps_host_path_and_mixed(nbmod, queue):
+    """Bound 0: every block is handed over (the seam itself); default bound at N = 3000: a mix.
+    queue = 2: handed-over blocks are planned on the device and their kernels run as the body of a
+    WHILE node of one CUDA graph; 1: the same rounds queued on the stream ahead of time; 0: the host
+    takes them through nb_step's launches.  The oracle is
+    stepped in lock-step with the GPU's own log here, because fp32 forces may move a step decision
+    near a threshold (tests/test_gpu_hermite.py)."""
     n, eps2, eta, lo, hi = 3000, 2.0 ** -12, 0.02, 2.0 ** -18, 2.0 ** -5
     m, x, v, a, j, t, dt = _start(n, 970, eps2, eta, lo, hi)
     with nbmod.Context(n) as ctx:
+        ctx.steps_queue(queue)
         for bound, k in ((0, 12), (30000000, 48)):
             ctx.steps_bound(bound)
             _load(ctx, m, x, v, a, j, t, dt)
             l0 = ctx.launch_count()
-            done, gt, gni = ctx.steps(k, eps2, eta, lo, hi)
+            done, gt, gni, us = ctx.steps(k, eps2, eta, lo, hi, times=True)
             launches = ctx.launch_count() - l0
-            rt, rni, _ = _oracle_steps(k, m, x, v, a, j, t, dt, eps2, eta, lo, hi)
+            rt, rni, last = _oracle_steps(k, m, x, v, a, j, t, dt, eps2, eta, lo, hi)
             assert done == k and np.array_equal(gt, rt)
             assert (gni != rni).sum() <= 2 and np.abs(gni - rni).max() <= 2
+            assert (us > 0).all() and us.sum() < 1e6
             g = ctx.state().cpu().numpy()
             assert np.abs(g[1:4] - x).max() < 1e-7 and np.abs(g[4:7] - v).max() < 1e-5
             assert (g[14] != dt).sum() <= max(2, n // 100)
+            if gni[-1] == rni[-1]:
+                # nb_block_forces after a handed-over block: the packed fp32 kernel's tolerances
+                pa, pj, pp = nbmod.binding.nb_block_forces(ctx.h)
+                ni = len(last[0])
+                view = nbmod.context._DeviceView
+                ga = torch.as_tensor(view(pa, 3 * ni, "<f8"), device=ctx.device).cpu().numpy().reshape(3, ni)
+                gp = torch.as_tensor(view(pp, ni, "<f8"), device=ctx.device).cpu().numpy()
+                tol = 1e-5          # the trajectory went through fp32 blocks, whichever kernel took the last one
+                assert (np.linalg.norm(ga - last[1], axis=0) <= tol * np.linalg.norm(last[1], axis=0)).all()
+                assert (np.abs(gp - last[3]) <= tol * np.abs(last[3])).all()
             if bound == 0:
-                assert launches >= 4 * k            # select, predict, pair, reduce, correct per block
+                assert launches >= 4 * k            # every block through launches of its own
             else:
                 small = int(((gni <= 512) & (gni * n <= bound)).sum())
-                print("mixed run: %d of %d blocks in the persistent kernel, %d launches" % (small, k, launches))
-                assert small > 0 and launches < 6 * (k - small) + 2 * (k - small) + 8
+                print("mixed run (queue %d): %d of %d blocks in the persistent kernel, %d launches"
+                      % (queue, small, k, launches))
+                assert small > 0
+                if queue != 1:              # mode 1 may queue rounds beyond the end of the run
+                    assert launches < 6 * (k - small) + 2 * (k - small) + 8
         ctx.sync()
 
 
-def test_steps_slice_overflow_goes_to_host_path(nbmod):
+def test_steps_queued_flags_eps0_t_end_and_overflow(nbmod):
+    """The device-planned path for handed-over blocks (bound 0: every block): unsoftened flagged
+    pairs, eps2 = 0 (the guarded pair kernels), t_end, k larger than what is left, and a block above
+    ni_max (NB_ERR_ARG, nothing advanced past it)."""
+    n, eta, lo, hi = 700, 0.02, 2.0 ** -18, 2.0 ** -6
+    flags = np.zeros(n, np.uint8)
+    flags[[3, 77, 649]] = 1
+    for eps2 in (2.0 ** -8, 0.0):
+        m, x, v, a, j, t, dt = _start(n, 960, eps2, eta, lo, hi, flags)
+        with nbmod.Context(n) as ctx:
+            ctx.steps_bound(0)
+            _load(ctx, m, x, v, a, j, t, dt)
+            ctx.set_flags(np.flatnonzero(flags).astype(np.int32), np.ones(3, np.uint8))
+            rt, rni, _ = _oracle_steps(30, m, x, v, a, j, t, dt, eps2, eta, lo, hi, flags)
+            t_end = rt[17]
+            n_before = int((rt <= t_end).sum())
+            done, gt, gni = ctx.steps(1000, eps2, eta, lo, hi, t_end=t_end)
+            assert done == n_before and np.array_equal(gt, rt[:done])
+            assert (gni != rni[:done]).sum() <= 1
+            done2, gt2, gni2 = ctx.steps(30 - done, eps2, eta, lo, hi)
+            assert done2 == 30 - done and np.array_equal(gt2, rt[done:])
+            g = ctx.state().cpu().numpy()
+            assert np.array_equal(g[13], t)
+            assert np.abs(g[1:4] - x).max() <= 1e-7 and np.abs(g[4:7] - v).max() <= 1e-5
+            ctx.sync()
+    # a block larger than ni_max: every particle due at once, ni_max = 256
+    m, x, v, a, j, t, dt = _start(n, 961, 2.0 ** -8, eta, lo, hi)
+    dt[:] = hi
+    with nbmod.Context(n, ni_max=256) as ctx:
+        _load(ctx, m, x, v, a, j, t, dt)
+        with pytest.raises(nbmod.binding.NBError):
+            ctx.steps(5, 2.0 ** -8, eta, lo, hi)
+        g = ctx.state().cpu().numpy()
+        assert np.array_equal(g[13], t) and np.array_equal(g[1:4], x)
+
+
+@pytest.mark.parametrize("queue", [2, 1, 0])
+def test_steps_slice_overflow_goes_to_host_path(nbmod, queue):
     """More than 128 due particles inside ONE slice of the persistent kernel (N = 30000: 148 slices of
     203): the slice cannot publish them all, the block must be handed to the host path, not truncated.
     And the device time log adds up."""
@@ -167,6 +223,7 @@ def test_steps_slice_overflow_goes_to_host_path(nbmod):
     dt[1000:1150] = lo                      # 150 consecutive particles due first, in one slice
     dt[20000] = 2 * lo
     with nbmod.Context(n) as ctx:
+        ctx.steps_queue(queue)
         _load(ctx, m, x, v, a, j, t, dt)
         done, gt, gni, us = ctx.steps(3, eps2, eta, lo, hi, times=True)
         rt, rni, _ = _oracle_steps(3, m, x, v, a, j, t, dt, eps2, eta, lo, hi)
