@@ -27,12 +27,13 @@ template <int KIND>
 __global__ void __launch_bounds__(128) rate_kernel(float* out, int iters, float a0, double d0)
 {
     constexpr int NCH = 8;
-    float2 f[NCH];
+    float2 f[NCH], g[NCH];
     double d[NCH];
     unsigned u[NCH];
     float s[NCH];
     for (int c = 0; c < NCH; ++c) {
         f[c] = make_float2(a0 + c + threadIdx.x, a0 - c);
+        g[c] = make_float2(a0 * 0.5f + c, a0 + 2 * c);
         d[c] = d0 + c + threadIdx.x;
         u[c] = threadIdx.x * 31 + c;
         s[c] = a0 + c * 0.5f + threadIdx.x;
@@ -60,12 +61,43 @@ __global__ void __launch_bounds__(128) rate_kernel(float* out, int iters, float 
                 // 4/11/17: one F2F.F32.F64 per step fed by a DADD and consumed by an FADD (different pipes)
                 if (KIND == 17) { d[c] = __dadd_rn(d[c], d0); s[c] += __double2float_rn(d[c]); }
                 if (KIND == 11) { f[c] = __ffma2_rn(f[c], m, b); if ((c & 3) == 0) { d[c] = __dadd_rn(d[c], d0); s[c] += __double2float_rn(d[c]); } }
+                // 20/21: the pair body's own mix, 13 FADD2 : 6 FMUL2 : 14 FFMA2, on independent chains
+                // (no MUFU, no loads): 20 = type changes at every instruction, 21 = runs of one type
+                if (KIND == 20) {
+                    f[c] = __ffma2_rn(f[c], m, b); f[c] = __fadd2_rn(f[c], b); f[c] = __ffma2_rn(f[c], m, b); f[c] = __fadd2_rn(f[c], m);
+                    f[c] = __fmul2_rn(f[c], m); f[c] = __ffma2_rn(f[c], m, b); f[c] = __fadd2_rn(f[c], b); f[c] = __ffma2_rn(f[c], b, m);
+                    if (r < 2) { f[c] = __fadd2_rn(f[c], b); f[c] = __fmul2_rn(f[c], m); }
+                    else if (r < 4) { f[c] = __ffma2_rn(f[c], m, b); }
+                    else if (r < 7) { f[c] = __fadd2_rn(f[c], m); }
+                }
+                if (KIND == 21) {
+                    if (r < 3) { f[c] = __fadd2_rn(f[c], b); f[c] = __fadd2_rn(f[c], m); f[c] = __fadd2_rn(f[c], b); f[c] = __fadd2_rn(f[c], m); }
+                    else if (r == 3) { f[c] = __fadd2_rn(f[c], b); f[c] = __fmul2_rn(f[c], m); f[c] = __fmul2_rn(f[c], m); f[c] = __fmul2_rn(f[c], m); }
+                    else if (r == 4) { f[c] = __fmul2_rn(f[c], m); f[c] = __fmul2_rn(f[c], m); f[c] = __fmul2_rn(f[c], m); f[c] = __ffma2_rn(f[c], m, b); f[c] = __ffma2_rn(f[c], b, m); }
+                    else { f[c] = __ffma2_rn(f[c], m, b); f[c] = __ffma2_rn(f[c], b, m); f[c] = __ffma2_rn(f[c], m, b); f[c] = __ffma2_rn(f[c], b, m); }
+                }
+                // 22..25: operands that are all live registers (no constant the reuse cache can hold)
+                if (KIND == 22) f[c] = __ffma2_rn(f[(c + 1) & 7], f[(c + 2) & 7], f[c]);
+                if (KIND == 23) f[c] = __fadd2_rn(f[(c + 1) & 7], f[c]);
+                if (KIND == 24) f[c] = __ffma2_rn(f[(c + 1) & 7], f[(c + 1) & 7], f[c]);
+                if (KIND == 25) f[c] = __ffma2_rn(f[(c + 1) & 7], m, f[c]);
+                // 26: six-word FFMA2 alternating with a two-word FMUL2 (does the operand fetch average out?)
+                if (KIND == 26) { f[c] = __ffma2_rn(f[(c + 1) & 7], f[(c + 2) & 7], f[c]); g[c] = __fmul2_rn(g[c], g[c]); }
+                // 27: six-word FFMA2 x3 sharing the first operand (a reuse chain), then the next chain
+                if (KIND == 27) {
+                    const float2 a = f[(c + 3) & 7];
+                    g[c] = __ffma2_rn(a, f[(c + 1) & 7], g[c]);
+                    g[(c + 1) & 7] = __ffma2_rn(a, f[(c + 2) & 7], g[(c + 1) & 7]);
+                    g[(c + 2) & 7] = __ffma2_rn(a, f[(c + 4) & 7], g[(c + 2) & 7]);
+                }
+                // 28: FFMA2 with one scalar (broadcast) operand: five words
+                if (KIND == 28) f[c] = __ffma2_rn(f[(c + 1) & 7], make_float2(s[c], s[c]), f[c]);
                 if (KIND == 18) { f[c] = __ffma2_rn(f[c], m, b); if ((c & 3) == 0) { d[c] = __dadd_rn(d[c], d0); s[c] += __double2float_rn(d[c]); } if (c == 7 && (r & 3) == 0) s[c] = rsq(s[c]); }
             }
         }
     }
     float acc = 0.f;
-    for (int c = 0; c < NCH; ++c) acc += f[c].x + f[c].y + (float)d[c] + s[c] + (float)u[c];
+    for (int c = 0; c < NCH; ++c) acc += f[c].x + f[c].y + g[c].x + g[c].y + (float)d[c] + s[c] + (float)u[c];
     out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
@@ -199,6 +231,231 @@ __global__ void __launch_bounds__(128, MINB) body_kernel(float* out, int reps, f
         res += A[u].ax.x + A[u].ax.y + A[u].ay.x + A[u].ay.y + A[u].az.x + A[u].az.y + A[u].jx.x + A[u].jx.y +
                A[u].jy.x + A[u].jy.y + A[u].jz.x + A[u].jz.y + A[u].p.x + A[u].p.y;
     out[blockIdx.x * 128 + tid] = res;
+}
+
+// ---------------- the same pair (encoding C) with SCALAR FP32 instructions ----------------
+// Packed f32x2 instructions halve the issue slots but run at 90 % (FFMA2) / 97 % (FADD2, FMUL2) of the
+// lane rate; scalar FFMA sustains 95 %.  A scalar body needs an issue slot per lane-op, so everything
+// else (MUFU, LDS, loop) competes with the FP32 pipe for issue: IPT i-particles per thread share the
+// ten LDS.128 of a j-quad.  33 FFMA-class + 1 MUFU + 10/(4 IPT) LDS per interaction.
+// ---------------- encoding C with the multiply-add CHAINS kept together ----------------
+// Register-file bandwidth (rates 22..25): an FFMA2 whose three operands are three different live
+// register pairs runs at 65 % of the packed rate, one with two different pairs at 96 %: the register
+// file delivers two 32-bit words per lane and clock, an instruction with six operand words takes three
+// clocks of a two-clock pipe slot unless an operand comes from the reuse cache (same register in the
+// same operand slot of the previous instruction).  The pair body has eleven such FFMA2 per j-pair:
+// three t = al*d + w (al shared), six sums += mr3 * (d | t) (mr3 shared), two of the r.w chain.  ptxas
+// treats the sums as leaves and sprinkles them as fillers, which breaks the chains.  SEP != 0 puts the
+// chains of a j-quad into a section of their own, after everything else of that quad.
+__device__ __forceinline__ unsigned long long f2u(float2 v)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(v.x), "f"(v.y));
+    return r;
+}
+__device__ __forceinline__ float2 u2f(unsigned long long r)
+{
+    float2 v;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(v.x), "=f"(v.y) : "l"(r));
+    return v;
+}
+
+template <int SEP>
+__device__ __forceinline__ void section()
+{
+    if (SEP == 1) __syncwarp();
+    if (SEP == 2) asm volatile("bar.warp.sync 0xffffffff;" ::: "memory");
+    if (SEP == 3) asm volatile("" ::: "memory");
+}
+
+template <int MINB, int SEP, int UNR>
+__global__ void __launch_bounds__(128, MINB) body_chain_kernel(float* out, int reps, float eps2f, int opaque)
+{
+    __shared__ __align__(16) float T[10 * TJ];       // xh yh zh xl yl zl vx vy vz m
+    const int tid = threadIdx.x;
+    for (int q = tid; q < TJ; q += 128) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.37 * ((q * 2654435761u + c * 40503u) % 1000) / 1000.0 - 0.18;
+            const float h = (float)x;
+            T[c * TJ + q] = h;
+            T[(3 + c) * TJ + q] = (float)(x - (double)h);
+            T[(6 + c) * TJ + q] = 0.01f * (float)((q * 7 + c * 13) % 17 - 8);
+        }
+        T[9 * TJ + q] = 1.0f / 1048576.0f;
+    }
+    __syncthreads();
+    constexpr int IPT = 2;
+    float2 nxh[IPT][3], nxl[IPT][3], nv[IPT][3];
+    Acc A[IPT];
+    for (int u = 0; u < IPT; ++u) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.001 * (tid + 128 * u) + 0.1 * c + 1e-9 * blockIdx.x;
+            const float h = (float)x;
+            nxh[u][c] = dup(-h);
+            nxl[u][c] = dup(-(float)(x - (double)h));
+            nv[u][c] = dup(0.003f * (tid % 7) - 0.01f * c + 0.002f * u);
+        }
+        A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
+    }
+    const float2 eps2 = dup(eps2f), m3 = dup(-3.0f);
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll UNR
+        for (int p = 0; p < TJ; p += 4) {
+            float4 f[10];
+#pragma unroll
+            for (int c = 0; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+            float2 d[4][3], w[4][3], mr[4], mr3[4], al[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int u = e >> 1, h = e & 1;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const float2 xh = h ? make_float2(f[c].z, f[c].w) : make_float2(f[c].x, f[c].y);
+                    const float2 xl = h ? make_float2(f[3 + c].z, f[3 + c].w) : make_float2(f[3 + c].x, f[3 + c].y);
+                    d[e][c] = __fadd2_rn(__fadd2_rn(xh, nxh[u][c]), __fadd2_rn(xl, nxl[u][c]));
+                    const float2 vv = h ? make_float2(f[6 + c].z, f[6 + c].w) : make_float2(f[6 + c].x, f[6 + c].y);
+                    w[e][c] = __fadd2_rn(vv, nv[u][c]);
+                }
+                const float2 mm = h ? make_float2(f[9].z, f[9].w) : make_float2(f[9].x, f[9].y);
+                float2 r2 = __ffma2_rn(d[e][0], d[e][0], eps2);
+                r2 = __ffma2_rn(d[e][1], d[e][1], r2);
+                r2 = __ffma2_rn(d[e][2], d[e][2], r2);
+                float2 rinv;
+                rinv.x = rsq(r2.x);
+                rinv.y = rsq(r2.y);
+                const float2 rinv2 = __fmul2_rn(rinv, rinv);
+                mr[e] = __fmul2_rn(mm, rinv);
+                mr3[e] = __fmul2_rn(mr[e], rinv2);
+                float2 rv = __fmul2_rn(d[e][0], w[e][0]);
+                rv = __ffma2_rn(d[e][1], w[e][1], rv);
+                rv = __ffma2_rn(d[e][2], w[e][2], rv);
+                al[e] = __fmul2_rn(__fmul2_rn(rinv2, m3), rv);
+            }
+            section<SEP>();
+            if (SEP == 4 && opaque) out[0] = 0.f;
+            if (SEP == 5) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int u = e >> 1;
+                    unsigned long long ax = f2u(A[u].ax), ay = f2u(A[u].ay), az = f2u(A[u].az), jx = f2u(A[u].jx),
+                                       jy = f2u(A[u].jy), jz = f2u(A[u].jz), pp = f2u(A[u].p);
+                    asm volatile(
+                        "{\n\t.reg .b64 tx, ty, tz;\n\t"
+                        "fma.rn.f32x2 tx, %7, %8, %11;\n\t"
+                        "fma.rn.f32x2 ty, %7, %9, %12;\n\t"
+                        "fma.rn.f32x2 tz, %7, %10, %13;\n\t"
+                        "fma.rn.f32x2 %0, %14, %8, %0;\n\t"
+                        "fma.rn.f32x2 %1, %14, %9, %1;\n\t"
+                        "fma.rn.f32x2 %2, %14, %10, %2;\n\t"
+                        "fma.rn.f32x2 %3, %14, tx, %3;\n\t"
+                        "fma.rn.f32x2 %4, %14, ty, %4;\n\t"
+                        "fma.rn.f32x2 %5, %14, tz, %5;\n\t"
+                        "add.rn.f32x2 %6, %6, %15;\n\t}"
+                        : "+l"(ax), "+l"(ay), "+l"(az), "+l"(jx), "+l"(jy), "+l"(jz), "+l"(pp)
+                        : "l"(f2u(al[e])), "l"(f2u(d[e][0])), "l"(f2u(d[e][1])), "l"(f2u(d[e][2])), "l"(f2u(w[e][0])),
+                          "l"(f2u(w[e][1])), "l"(f2u(w[e][2])), "l"(f2u(mr3[e])), "l"(f2u(mr[e])));
+                    A[u].ax = u2f(ax); A[u].ay = u2f(ay); A[u].az = u2f(az); A[u].jx = u2f(jx);
+                    A[u].jy = u2f(jy); A[u].jz = u2f(jz); A[u].p = u2f(pp);
+                }
+            } else
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int u = e >> 1;
+                const float2 tx = __ffma2_rn(al[e], d[e][0], w[e][0]);
+                const float2 ty = __ffma2_rn(al[e], d[e][1], w[e][1]);
+                const float2 tz = __ffma2_rn(al[e], d[e][2], w[e][2]);
+                A[u].ax = __ffma2_rn(mr3[e], d[e][0], A[u].ax);
+                A[u].ay = __ffma2_rn(mr3[e], d[e][1], A[u].ay);
+                A[u].az = __ffma2_rn(mr3[e], d[e][2], A[u].az);
+                A[u].jx = __ffma2_rn(mr3[e], tx, A[u].jx);
+                A[u].jy = __ffma2_rn(mr3[e], ty, A[u].jy);
+                A[u].jz = __ffma2_rn(mr3[e], tz, A[u].jz);
+                A[u].p = __fadd2_rn(A[u].p, mr[e]);
+            }
+            section<SEP>();
+            if (SEP == 4 && opaque) out[1] = 0.f;
+        }
+    }
+    float res = 0.f;
+    for (int u = 0; u < IPT; ++u)
+        res += A[u].ax.x + A[u].ax.y + A[u].ay.x + A[u].ay.y + A[u].az.x + A[u].az.y + A[u].jx.x + A[u].jx.y +
+               A[u].jy.x + A[u].jy.y + A[u].jz.x + A[u].jz.y + A[u].p.x + A[u].p.y;
+    out[blockIdx.x * 128 + tid] = res;
+}
+
+struct Acc1 { float ax, ay, az, jx, jy, jz, p; };
+
+__device__ __forceinline__ void body1(float dx, float dy, float dz, float wx, float wy, float wz, float m,
+                                      float eps2, Acc1& A)
+{
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+    const float rinv = rsq(r2);
+    const float rinv2 = rinv * rinv;
+    const float mr = m * rinv;
+    const float mr3 = mr * rinv2;
+    const float rv = fmaf(dz, wz, fmaf(dy, wy, dx * wx));
+    const float al = (rinv2 * -3.0f) * rv;
+    A.p += mr;
+    A.ax = fmaf(mr3, dx, A.ax);
+    A.ay = fmaf(mr3, dy, A.ay);
+    A.az = fmaf(mr3, dz, A.az);
+    A.jx = fmaf(mr3, fmaf(al, dx, wx), A.jx);
+    A.jy = fmaf(mr3, fmaf(al, dy, wy), A.jy);
+    A.jz = fmaf(mr3, fmaf(al, dz, wz), A.jz);
+}
+
+template <int IPT, int MINB, int UNR, int NT>
+__global__ void __launch_bounds__(NT, MINB) scalar_body_kernel(float* out, int reps, float eps2)
+{
+    __shared__ __align__(16) float T[10 * TJ];       // xh yh zh xl yl zl vx vy vz m
+    const int tid = threadIdx.x;
+    for (int q = tid; q < TJ; q += NT) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.37 * ((q * 2654435761u + c * 40503u) % 1000) / 1000.0 - 0.18;
+            const float h = (float)x;
+            T[c * TJ + q] = h;
+            T[(3 + c) * TJ + q] = (float)(x - (double)h);
+            T[(6 + c) * TJ + q] = 0.01f * (float)((q * 7 + c * 13) % 17 - 8);
+        }
+        T[9 * TJ + q] = 1.0f / 1048576.0f;
+    }
+    __syncthreads();
+    float nxh[IPT][3], nxl[IPT][3], nv[IPT][3];
+    Acc1 A[IPT];
+    for (int u = 0; u < IPT; ++u) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.001 * (tid + NT * u) + 0.1 * c + 1e-9 * blockIdx.x;
+            const float h = (float)x;
+            nxh[u][c] = -h;
+            nxl[u][c] = -(float)(x - (double)h);
+            nv[u][c] = 0.003f * (tid % 7) - 0.01f * c + 0.002f * u;
+        }
+        A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = 0.f;
+    }
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll UNR
+        for (int p = 0; p < TJ; p += 4) {
+            float4 f[10];
+#pragma unroll
+            for (int c = 0; c < 10; ++c) f[c] = *reinterpret_cast<const float4*>(T + c * TJ + p);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                float v[10];
+#pragma unroll
+                for (int c = 0; c < 10; ++c) v[c] = e == 0 ? f[c].x : (e == 1 ? f[c].y : (e == 2 ? f[c].z : f[c].w));
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+                    const float dx = (v[0] + nxh[u][0]) + (v[3] + nxl[u][0]);
+                    const float dy = (v[1] + nxh[u][1]) + (v[4] + nxl[u][1]);
+                    const float dz = (v[2] + nxh[u][2]) + (v[5] + nxl[u][2]);
+                    body1(dx, dy, dz, v[6] + nv[u][0], v[7] + nv[u][1], v[8] + nv[u][2], v[9], eps2, A[u]);
+                }
+            }
+        }
+    }
+    float res = 0.f;
+    for (int u = 0; u < IPT; ++u) res += A[u].ax + A[u].ay + A[u].az + A[u].jx + A[u].jy + A[u].jz + A[u].p;
+    out[blockIdx.x * NT + tid] = res;
 }
 
 struct Acc64 { double ax, ay, az, jx, jy, jz, p; };
@@ -387,6 +644,38 @@ void run_body(const char* name)
            fa.numRegs, occ, ms, r, r / 1.2408e12 * 100);
 }
 
+template <int IPT, int MINB, int UNR, int NT>
+void run_scalar()
+{
+    const int reps = 300;
+    const int grid = nsm * MINB * 5;
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scalar_body_kernel<IPT, MINB, UNR, NT>, NT, 0));
+    cudaFuncAttributes fa;
+    CK(cudaFuncGetAttributes(&fa, scalar_body_kernel<IPT, MINB, UNR, NT>));
+    float ms = time_ms([&] { scalar_body_kernel<IPT, MINB, UNR, NT><<<grid, NT>>>(d_out, reps, 1e-6f); });
+    const double inter = (double)grid * NT * IPT * (double)TJ * reps;
+    const double r = inter / (ms * 1e-3);
+    printf("scalar body C: ipt %d threads %3d unroll %d minb %d regs %3d occ %d : %8.3f ms  %9.3e inter/s = %5.1f%% of 1.2408e12\n",
+           IPT, NT, UNR, MINB, fa.numRegs, occ, ms, r, r / 1.2408e12 * 100);
+}
+
+template <int MINB, int SEP, int UNR>
+void run_chain()
+{
+    const int reps = 300;
+    const int grid = nsm * MINB * 5;
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, body_chain_kernel<MINB, SEP, UNR>, 128, 0));
+    cudaFuncAttributes fa;
+    CK(cudaFuncGetAttributes(&fa, body_chain_kernel<MINB, SEP, UNR>));
+    float ms = time_ms([&] { body_chain_kernel<MINB, SEP, UNR><<<grid, 128>>>(d_out, reps, 1e-6f, 0); });
+    const double inter = (double)grid * 4 * 64 * (double)TJ * reps;
+    const double r = inter / (ms * 1e-3);
+    printf("chain body C: sep %d unroll %d minb %d regs %3d occ %d : %8.3f ms  %9.3e inter/s = %5.1f%% of 1.2408e12\n",
+           SEP, UNR, MINB, fa.numRegs, occ, ms, r, r / 1.2408e12 * 100);
+}
+
 template <int KIND>
 void run_rate(const char* name, double ops_per_iter_thread, int ctas_per_sm)
 {
@@ -425,6 +714,15 @@ int main(int argc, char** argv)
         run_rate<10>("FFMA2 + DADD 4:1 (count FFMA2)", 64, 4);
         run_rate<12>("FFMA2 + MUFU 8:1 (count FFMA2)", 64, 4);
         run_rate<13>("FFMA2 + FFMA 1:1 (count FFMA2)", 64, 4);
+        run_rate<20>("body mix 13A:6M:14F alternating (count all)", 8 * (8 * 8 + 2 * 2 + 2 + 3), 4);
+        run_rate<21>("body mix 13A:6M:14F in runs (count all)", 8 * (12 + 4 + 5 + 12), 4);
+        run_rate<22>("FFMA2 d = a*b+d, a b d all live regs", 64, 4);
+        run_rate<24>("FFMA2 d = a*a+d", 64, 4);
+        run_rate<25>("FFMA2 d = a*const+d", 64, 4);
+        run_rate<23>("FADD2 d = a+d, live regs", 64, 4);
+        run_rate<26>("FFMA2 (6 words) + FMUL2 a*a (2 words) 1:1 (count both)", 128, 4);
+        run_rate<27>("FFMA2 (6 words) in chains of 3 sharing operand a", 192, 4);
+        run_rate<28>("FFMA2 d = a*scalar+d (5 words)", 64, 4);
         run_rate<17>("F2F.F32.F64 (+DADD feed, FADD use)", 64, 4);
         run_rate<11>("FFMA2 + (DADD,F2F) 4:1 (count FFMA2)", 64, 4);
         run_rate<18>("FFMA2:DADD:F2F:MUFU 12:3:3:1 (count FFMA2)", 64, 4);
@@ -442,6 +740,31 @@ int main(int argc, char** argv)
         run_body<3, 1, 4>("D': fp64 x y z + integer-pipe conversion");
         run_body<3, 1, 3>("D': fp64 x y z + integer-pipe conversion");
         run_body<2, 1, 4>("fp64 x y + int conversion, two-float z");
+    }
+    if (all || !strcmp(what, "scalar")) {
+        printf("-- pair body C with scalar FP32 instructions, loop only\n");
+        run_scalar<2, 4, 1, 128>();
+        run_scalar<2, 4, 2, 128>();
+        run_scalar<2, 3, 2, 128>();
+        run_scalar<4, 4, 1, 128>();
+        run_scalar<4, 3, 1, 128>();
+        run_scalar<4, 4, 2, 128>();
+        run_scalar<4, 2, 1, 256>();
+        run_scalar<4, 1, 1, 512>();
+        run_scalar<8, 2, 1, 128>();
+        run_scalar<8, 3, 1, 128>();
+        run_scalar<2, 5, 1, 128>();
+        run_scalar<2, 2, 2, 256>();
+        run_scalar<1, 4, 2, 256>();
+    }
+    if (all || !strcmp(what, "chain")) {
+        printf("-- pair body C, chains of a j-quad in a section of their own (SEP: 0 none, 1 __syncwarp, 2 bar.warp.sync, 3 compiler fence, 4 opaque store)\n");
+        run_chain<3, 0, 1>(); run_chain<3, 0, 2>(); run_chain<4, 0, 1>();
+        run_chain<3, 1, 1>(); run_chain<3, 1, 2>(); run_chain<4, 1, 1>();
+        run_chain<3, 2, 1>(); run_chain<3, 2, 2>();
+        run_chain<3, 3, 1>(); run_chain<3, 3, 2>();
+        run_chain<3, 4, 1>(); run_chain<3, 4, 2>(); run_chain<4, 4, 1>();
+        run_chain<3, 5, 1>(); run_chain<3, 5, 2>(); run_chain<4, 5, 1>();
     }
     if (all || !strcmp(what, "hetero")) {
         printf("-- fp32 two-float (2 i per thread) and fp64 (ipt i per thread) warps in one CTA\n");
