@@ -63,7 +63,7 @@ def parse():
     ap.add_argument("--predict", action="store_true",
                     help="instead of the default line: the Hermite predictor alone against the HBM roofline "
                          "(config 5's N = 2^22 + 11, and N = 2^20 alternating between two contexts)")
-    ap.add_argument("--shard", default="i", choices=["i", "j"],
+    ap.add_argument("--shard", default="i", choices=["i", "j", "jx"],
                     help="multi-GPU decomposition: i = active list sharded, j replicated (default); j = the paper's "
                          "scheme (PAPER.md:55): j sharded, every rank evaluates all active particles by value "
                          "against its slice, one all_reduce of [7][N_i]")
@@ -293,7 +293,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    if args.shard == "j":
+    if args.shard in ("j", "jx"):
         return run_shard_j(args, case, il, t, workload, rank, world, local, dev)
     ctx = nbm.Context(n, max(ni, 1), device=local)
     if args.fp64:
@@ -788,13 +788,56 @@ def run_shard_j(args, case, il, t, workload, rank, world, local, dev):
     mine = torch.from_numpy(il.astype(np.int64)).to(dev)[pos]
     flags_dev = torch.from_numpy(case.flags.astype(np.float64)).to(dev)
 
+    fused = args.shard == "jx"
+    if fused:
+        # the partial forces are exchanged and summed by the kernels over peer memory (nb_xforce)
+        torch.cuda.set_device(dev)
+        sharding.xchg_connect(ctx, ni)
+
     def step():
         nb.nb_predict(h, t)
         px, pv = ctx.predicted()
         loc = mine - lo
         state = torch.cat([px[:, loc], pv[:, loc], flags_dev[None, mine], mine[None].to(torch.float64)], 0)
+        if fused:
+            return sharding.force_j_sharded_xchg(ctx, state, pos, ni, lo, hi, case.eps2)
         return sharding.force_j_sharded(lambda x, v, s_, f_: ctx.force_ext_ids(x, v, s_, f_, case.eps2),
                                         state, pos, ni, lo, hi)
+
+    def small_block(k, reps=200):
+        """One force call of the block-step regime (k active particles, state already on every rank):
+        partial forces + NCCL all_reduce against nb_xforce (one launch)."""
+        sel = torch.from_numpy(il[:k].astype(np.int64)).to(dev)
+        px, pv = ctx.predicted()
+        own = (sel >= lo) & (sel < hi)
+        # the state of particles this rank does not own comes from the case (any value serves the timing)
+        xs = torch.from_numpy(np.ascontiguousarray(case.x[:, il[:k]])).to(dev)
+        vs = torch.from_numpy(np.ascontiguousarray(case.v[:, il[:k]])).to(dev)
+        if bool(own.any()):
+            xs[:, own] = px[:, sel[own] - lo]
+            vs[:, own] = pv[:, sel[own] - lo]
+        sidx = torch.where(own, sel - lo, torch.full_like(sel, -1)).to(torch.int32)
+        ifl = torch.zeros(k, dtype=torch.uint8, device=dev)
+        out = {}
+        for name in ("nccl", "xchg"):
+            def call():
+                if name == "xchg":
+                    return ctx.xforce(xs, vs, sidx, ifl, case.eps2)
+                a, j, p = ctx.force_ext_ids(xs, vs, sidx, ifl, case.eps2)
+                part = torch.cat([a, j, p.reshape(1, -1)], 0)
+                dist.all_reduce(part)
+                return part
+            for _ in range(10):
+                call()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier()
+            f0.record()
+            for _ in range(reps):
+                call()
+            f1.record()
+            barrier()
+            out["us_per_call_" + name] = f0.elapsed_time(f1) * 1e3 / reps
+        return out
 
     def barrier():
         dist.barrier()
@@ -827,6 +870,18 @@ def run_shard_j(args, case, il, t, workload, rank, world, local, dev):
                            "parallelism": "j-sharded x%d (PAPER.md:55), active particles by value" % world},
                 "gpu_launches": int(launches),
                 "bytes_all_reduce_per_step": 56 * ni, "bytes_all_gather_per_step": 72 * ni}
+        if fused:
+            line["config"]["step"] = ("nb_predict(slice) + all_gather(active state) + nb_xforce(slice: pair kernel, "
+                                      "reduction, push to the peers' windows, flags, sum in rank order)")
+            line["bytes_all_reduce_per_step"] = 0
+            line["bytes_pushed_per_step"] = 56 * ni * world
+    sb = None
+    if fused:
+        sb = {"n_i": 4, **small_block(4)}
+        sb16 = {"n_i": 16, **small_block(16)}
+    if rank == 0:
+        if fused:
+            line["small_block"] = [sb, sb16]
         print(json.dumps(line))
     ctx.close()
     dist.destroy_process_group()

@@ -39,7 +39,8 @@ typedef enum {
     NB_ERR_CUDA = -3,    /* a CUDA runtime call or kernel launch failed                             */
     NB_ERR_INDEX = -4,   /* an i_list / idx entry was outside [0, n) (reported by nb_sync)          */
     NB_ERR_STATE = -5,   /* nb_force before any nb_predict, or workspace set too late               */
-    NB_ERR_ARCH = -6     /* device is not compute capability 10.x                                   */
+    NB_ERR_ARCH = -6,    /* device is not compute capability 10.x                                   */
+    NB_ERR_PEER = -7     /* nb_xforce: a peer rank did not push its partial forces in time (nb_sync) */
 } nb_status;
 
 /* ---- lifetime --------------------------------------------------------------------------- */
@@ -185,6 +186,48 @@ int nb_force_ext_ids(nb_ctx* c, int64_t ni, const double* x, const double* v, co
 #define NB_FUSED_MAX 8
 int nb_force_fused(nb_ctx* c, double t, const int32_t* i_list, int64_t ni, double eps2, double* acc,
                    double* jrk, double* pot);
+
+/* ---- j-sharding over GPUs with the exchange done by the kernels -----------------
+ *
+ * PAPER.md:55 (section III.A): "Multi-GPU parallelization is achieved by distributing the j
+ * particles over the various GPUs ... the first kernel computes the partial forces ... and the second
+ * kernel sums these."  Rank r of `world` holds a slice of the j-set in its own context.  Across GPUs the
+ * "second kernel" is an exchange; here it is done by the kernels themselves over peer memory (NVLink /
+ * NVSwitch P2P stores), not by a collective-library call and not through the host (the
+ * host link is "the crucial bottleneck"): every rank owns a WINDOW in device memory
+ * (2 x world x [7][ni_cap] fp64 + flags); a rank stores its partial forces into slot [rank] of every
+ * rank's window, makes them visible system-wide and raises a flag there; it then waits for the flags of
+ * all ranks in its own window and adds the slots in rank order (fixed order: deterministic, identical
+ * on all ranks; R9).  For ni <= 16 all of this happens in the pair kernel's last CTA: pair loop,
+ * reduction, exchange and cross-rank sum are ONE launch; for larger ni two small kernels follow the
+ * reduction.  nb_xforce is a COLLECTIVE: every rank calls it with the same ni and the same i-particles,
+ * in the same order, on a stream of its own device.
+ *
+ * nb_xchg_create: allocate this rank's window (cudaMalloc, not part of the lent workspace).  world in
+ *   [1, 16], rank in [0, world), ni_cap in [1, ni_max] = the largest ni of an nb_xforce call.  Calling
+ *   it again replaces the window (peers must attach anew).
+ * nb_xchg_export: HOST outputs (either may be NULL): `handle` = NB_XCHG_HANDLE_BYTES bytes that
+ *   another PROCESS passes to nb_xchg_attach (a CUDA IPC memory handle); `*dev_ptr` = the window's
+ *   device address, which another context of the SAME process passes instead.
+ * nb_xchg_attach: map rank `peer`'s window: exactly one of `handle` (HOST bytes from the peer's
+ *   nb_xchg_export, another process) and `same_process_ptr` (same process; on another device peer
+ *   access is enabled) is non-NULL.  peer == own rank is accepted and ignored.  All world - 1 peers
+ *   must be attached before nb_xforce (NB_ERR_STATE otherwise).  The caller keeps the peers alive
+ *   until nb_xchg_destroy / nb_destroy of every rank that attached them.
+ * nb_xforce: nb_force_ext_ids on this rank's j-slice (same arguments, DEVICE pointers, mixed precision,
+ *   partial-sum reduction only) followed by the exchange.  phase 0: acc / jrk / pot hold the COMPLETE
+ *   forces when the call's kernels have run; phase 1: compute and push only (acc / jrk / pot then hold
+ *   this rank's partial forces); phase 2: the other half of the last phase-1 call -- wait for the peers
+ *   and sum into acc / jrk / pot (x, v, self_idx, iflags, eps2 are ignored).  The split form lets a
+ *   caller put other work between the halves.  A peer that has not pushed within 20 s latches
+ *   NB_ERR_PEER (returned by nb_sync); the outputs are then meaningless.  ni > ni_cap: NB_ERR_ARG. */
+#define NB_XCHG_HANDLE_BYTES 64
+int nb_xchg_create(nb_ctx* c, int rank, int world, int64_t ni_cap);
+int nb_xchg_export(nb_ctx* c, unsigned char* handle, void** dev_ptr);
+int nb_xchg_attach(nb_ctx* c, int peer, const unsigned char* handle, void* same_process_ptr);
+int nb_xchg_destroy(nb_ctx* c);
+int nb_xforce(nb_ctx* c, int phase, int64_t ni, const double* x, const double* v, const int32_t* self_idx,
+              const uint8_t* iflags, double eps2, double* acc, double* jrk, double* pot);
 
 /* HOST-pointer form: i_list, acc, jrk, pot are host arrays; copies in, runs, copies back and
  * synchronises the stream before returning (so it also returns latched errors). */
@@ -340,7 +383,7 @@ int nb_set_fused(nb_ctx* c, int on);
 /* DEVICE addresses of the last nb_step's acc [3][ni], jrk [3][ni], pot [ni] (any may be NULL). */
 int nb_block_forces(nb_ctx* c, const double** acc, const double** jrk, const double** pot);
 
-int nb_sync(nb_ctx* c);   /* stream sync; returns and clears a latched NB_ERR_INDEX / NB_ERR_STATE */
+int nb_sync(nb_ctx* c);   /* stream sync; returns and clears a latched NB_ERR_INDEX / NB_ERR_PEER / NB_ERR_STATE */
 const char* nb_strerror(int status);
 const char* nb_version(void);
 

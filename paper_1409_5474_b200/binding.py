@@ -11,7 +11,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("NB_LIBRARY") or os.path.join(_HERE, "libnb.so")   # NB_LIBRARY: another build
 
 NB_OK, NB_ERR_ARG, NB_ERR_ALLOC, NB_ERR_CUDA = 0, -1, -2, -3
-NB_ERR_INDEX, NB_ERR_STATE, NB_ERR_ARCH = -4, -5, -6
+NB_ERR_INDEX, NB_ERR_STATE, NB_ERR_ARCH, NB_ERR_PEER = -4, -5, -6, -7
+NB_XCHG_HANDLE_BYTES = 64
 NB_MAX_FLAGGED = 1024
 
 EXPORTS = [
@@ -20,6 +21,7 @@ EXPORTS = [
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_ext_ids", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_order", "nb_force6", "nb_set_precision", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_steps", "nb_set_steps_bound", "nb_set_steps_queue", "nb_block_forces", "nb_strerror", "nb_version",
+    "nb_xchg_create", "nb_xchg_export", "nb_xchg_attach", "nb_xchg_destroy", "nb_xforce",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -75,6 +77,11 @@ lib.nb_set_steps_bound.argtypes = [_vp, _i64]
 lib.nb_set_steps_queue.argtypes = [_vp, _i32]
 lib.nb_block_forces.argtypes = [_vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp), ctypes.POINTER(_vp)]
 lib.nb_version.restype = ctypes.c_char_p
+lib.nb_xchg_create.argtypes = [_vp, _i32, _i32, _i64]
+lib.nb_xchg_export.argtypes = [_vp, _vp, ctypes.POINTER(_vp)]
+lib.nb_xchg_attach.argtypes = [_vp, _i32, _vp, _vp]
+lib.nb_xchg_destroy.argtypes = [_vp]
+lib.nb_xforce.argtypes = [_vp, _i32, _i64, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]
 
 
 class NBError(RuntimeError):
@@ -237,6 +244,36 @@ def nb_force_ext_ids(c, ni, x, v, self_idx, iflags, eps2, acc, jrk, pot):
     """DEVICE x, v (3, ni) fp64, self_idx int32 (ni,), iflags uint8 (ni,) or None."""
     _check(lib.nb_force_ext_ids(c, ni, _ptr(x), _ptr(v), _ptr(self_idx), _ptr(iflags), eps2, _ptr(acc), _ptr(jrk),
                                 _ptr(pot)), "nb_force_ext_ids")
+
+
+def nb_xchg_create(c, rank, world, ni_cap):
+    _check(lib.nb_xchg_create(c, int(rank), int(world), int(ni_cap)), "nb_xchg_create")
+
+
+def nb_xchg_export(c):
+    """-> (handle: NB_XCHG_HANDLE_BYTES bytes for another process, dev_ptr: int for this process)."""
+    buf = ctypes.create_string_buffer(NB_XCHG_HANDLE_BYTES)
+    ptr = ctypes.c_void_p()
+    _check(lib.nb_xchg_export(c, ctypes.cast(buf, ctypes.c_void_p), ctypes.byref(ptr)), "nb_xchg_export")
+    return bytes(buf.raw), int(ptr.value)
+
+
+def nb_xchg_attach(c, peer, handle=None, same_process_ptr=None):
+    """handle: bytes from the peer's nb_xchg_export (another process); same_process_ptr: int."""
+    buf = ctypes.create_string_buffer(bytes(handle), NB_XCHG_HANDLE_BYTES) if handle is not None else None
+    _check(lib.nb_xchg_attach(c, int(peer), ctypes.cast(buf, ctypes.c_void_p) if buf is not None else None,
+                              ctypes.c_void_p(same_process_ptr) if same_process_ptr is not None else None),
+           "nb_xchg_attach")
+
+
+def nb_xchg_destroy(c):
+    _check(lib.nb_xchg_destroy(c), "nb_xchg_destroy")
+
+
+def nb_xforce(c, phase, ni, x, v, self_idx, iflags, eps2, acc, jrk, pot):
+    """As nb_force_ext_ids (DEVICE pointers) plus the exchange over peer memory; phase 0, 1 or 2."""
+    _check(lib.nb_xforce(c, int(phase), ni, _ptr(x), _ptr(v), _ptr(self_idx), _ptr(iflags), eps2, _ptr(acc), _ptr(jrk),
+                         _ptr(pot)), "nb_xforce")
 
 
 def nb_set_order(c, order):

@@ -167,6 +167,39 @@ class Context:
         self._keep = [dx, dv, ds, df]
         return acc, jrk, pot
 
+    # -- j-sharding with the exchange done by the kernels over peer memory (nb.h: nb_xforce) -----
+    def xchg_create(self, rank, world, ni_cap):
+        nb.nb_xchg_create(self.h, rank, world, ni_cap)
+
+    def xchg_export(self):
+        """(IPC handle bytes for another process, device address for another context of this one)."""
+        return nb.nb_xchg_export(self.h)
+
+    def xchg_attach(self, peer, handle=None, same_process_ptr=None):
+        nb.nb_xchg_attach(self.h, peer, handle, same_process_ptr)
+
+    def xchg_destroy(self):
+        nb.nb_xchg_destroy(self.h)
+
+    def xforce(self, x, v, self_idx, iflags, eps2, phase=0, out=None):
+        """force_ext_ids on this rank's j-slice + the exchange: phase 0 = complete forces; 1 = compute
+        and push (returns this rank's partial forces); 2 = wait and sum into `out` (the tensors phase
+        1 returned)."""
+        if phase == 2:
+            acc, jrk, pot = out
+            nb.nb_xforce(self.h, 2, pot.shape[0], None, None, None, None, eps2, acc, jrk, pot)
+            return acc, jrk, pot
+        dx, dv = self._dev(x), self._dev(v)
+        ds = self._dev(self_idx, torch.int32)
+        df = self._dev(iflags, torch.uint8) if iflags is not None else None
+        ni = dx.shape[1]
+        acc = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        jrk = torch.empty((3, ni), dtype=torch.float64, device=self.device)
+        pot = torch.empty((ni,), dtype=torch.float64, device=self.device)
+        nb.nb_xforce(self.h, phase, ni, dx, dv, ds, df, eps2, acc, jrk, pot)
+        self._keep = [dx, dv, ds, df]
+        return acc, jrk, pot
+
     # -- block-step layer (marshalling only) --------------------------------------------------
     def init_steps(self, i_list, acc, jrk, eta_s, dt_min, dt_max):
         il = self._dev(i_list, torch.int32)

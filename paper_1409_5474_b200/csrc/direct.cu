@@ -1,5 +1,5 @@
-// direct.cu -- nb_force for a HANDFUL of active particles (N_i <= DIRECT_NI_MAX): one launch that
-// streams the packed predicted j-set once at HBM speed.
+// direct.cu -- nb_force (and the by-value calls with jerk) for a HANDFUL of active particles
+// (N_i <= DIRECT_NI_MAX): one launch that streams the packed predicted j-set once at HBM speed.
 //
 // with few active i "the thread-per-i mapping cannot hide latencies".  With a handful of
 // them the call is not arithmetic at all: it is one pass over N x 44 B.  The tile-ring kernel of
@@ -19,6 +19,7 @@
 // guarded packed pair (R6).
 #include "nb_internal.h"
 #include "pair32.h"
+#include "xchg.h"
 
 namespace nb {
 
@@ -57,7 +58,31 @@ direct_kernel(ForceArgs P, ReduceArgs R)
     // a2: the active particles, from the pack (two-float position, fp32 velocity; R8, R17)
     if (tid == 0) sflagged = 0u;
     __syncthreads();
-    if (tid < NI) {
+    if (tid < NI && P.ext_x) {
+        // by value (nb_force_ext / nb_force_ext_ids / nb_xforce): fp64 position split in two floats here
+        // (PAPER.md:53), velocity rounded; the member of the j-set it is, if any, is excluded by index
+        const int e = tid < P.ni ? tid : 0;
+        float h[3], l[3], w[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double xc = P.ext_x[(int64_t)c * P.ni + e];
+            h[c] = __double2float_rn(xc);
+            l[c] = __double2float_rn(xc - (double)h[c]);
+            w[c] = __double2float_rn(P.ext_v[(int64_t)c * P.ni + e]);
+        }
+        IPart I;
+        I.nxh = dup(-h[0]); I.nyh = dup(-h[1]); I.nzh = dup(-h[2]);
+        I.nxl = dup(-l[0]); I.nyl = dup(-l[1]); I.nzl = dup(-l[2]);
+        I.nvx = dup(-w[0]); I.nvy = dup(-w[1]); I.nvz = dup(-w[2]);
+        sI[tid] = I;
+        int q = -1;
+        if (tid < P.ni && P.ext_self) {
+            const int s = P.ext_self[e];
+            if (s >= 0 && s < P.n) q = s;
+            if (P.any_flagged && P.ext_flags && (P.ext_flags[e] & 1)) atomicOr(&sflagged, 1u << tid);
+        }
+        sself[tid] = q;
+    } else if (tid < NI) {
         int q = tid < P.ni ? P.i_list[tid] : -1;
         if (tid < P.ni && (q < 0 || q >= P.n)) {
             atomicOr(P.err, 1);
@@ -168,6 +193,8 @@ direct_kernel(ForceArgs P, ReduceArgs R)
         __threadfence();
         for (int k = warp; k < R.ni; k += DIRECT_THREADS / 32) reduce_row<true>(R, k, lane);
         if (tid == 0) *R.counter = 0u;
+        // j-sharded call (nb_xforce): the same CTA exchanges with the peers (xchg.h)
+        if (R.xchg) xchg_in_cta<DIRECT_THREADS>(R, P.err, tid);
     }
 }
 

@@ -15,6 +15,7 @@
 #include "nb_internal.h"
 #include "pair32.h"
 #include "tma.h"
+#include "xchg.h"
 
 namespace nb {
 
@@ -298,6 +299,8 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
             __threadfence();                  // acquire: the other CTAs' partials
             for (int k = tid >> 5; k < R.ni; k += NWARPS) reduce_row<true>(R, k, tid & 31);
             if (tid == 0) *R.counter = 0u;    // ready for the next call on this stream
+            // j-sharded call (nb_xforce): the same CTA exchanges with the peers (xchg.h)
+            if (MODE == 1 && R.xchg) xchg_in_cta<FORCE_THREADS>(R, P.err, tid);
         }
     }
     if (DYN) {

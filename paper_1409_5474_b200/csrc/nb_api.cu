@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "nb_internal.h"
+#include "xchg.h"
 
 using namespace nb;
 
@@ -13,6 +14,15 @@ struct nb_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     int64_t n_max = 0, ni_max = 0, n_cap = 0, n = 0;
+
+    // j-sharded calls (nb_xforce): this rank's exchange window and the peers' as mapped here (xchg.h)
+    Xchg xchg_host{};                   // host copy of the descriptor; world == 0: no window
+    Xchg* xchg_dev = nullptr;
+    unsigned char* xchg_win = nullptr;
+    unsigned* xchg_ticket = nullptr;
+    bool xchg_ipc[XCHG_MAX_WORLD] = {}; // win[r] was opened from an IPC handle (closed by nb_xchg_destroy)
+    unsigned xchg_epoch = 0;            // epoch of the last push
+    int xchg_call = -1;                 // phase of the nb_xforce call in progress (-1: an ordinary force call)
     int sm_count = 148;
     int blocks_per_sm[8] = {1, 1, 1, 1, 1, 1, 1, 1};   // all-i kernel, its guarded form, few-i kernel, its guarded form; [4..7] the same for nb_steps' device-planned kernels
 
@@ -382,14 +392,26 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // a handful of i: the few-i kernel's last CTA also reduces, the call is one launch
     const bool reduce_here = jsh > 0 && !mode && !f64 && a.ntiles > 0 && tiles_a == 0 && ni <= 16;
     a.reduce_here = reduce_here ? 1 : 0;
+    // nb_xforce: the reducing CTA also exchanges with the peers (force.cu); otherwise two small kernels
+    // after the reduction do (below)
+    const bool xchg = c->xchg_call >= 0;
+    const bool direct = (kmode == 0 || kmode == 1) && !f64 && !mode && c->tune_splits == 0 && ni <= DIRECT_NI_MAX &&
+                        a.ntiles > 0 &&
+                        direct_terms_per_lane(a.ntiles, direct_grid(a.ntiles, c->sm_count)) <= 64;
+    if (xchg && (reduce_here || direct)) {
+        r.xchg = c->xchg_dev;
+        r.xchg_epoch = c->xchg_epoch;
+        r.xchg_phase = c->xchg_call;
+    }
 
     int launched = 0;
     nb_ctx::Rec* rec = nullptr;
-    // a handful of members of the j-set: the direct kernel (direct.cu) streams the pack once, one
-    // launch; it keeps whole per-thread sums in fp32, so only while they stay within R17's 64 terms
-    if (kmode == 0 && !f64 && !mode && c->tune_splits == 0 && ni <= DIRECT_NI_MAX && a.ntiles > 0) {
+    // a handful of active particles (members of the j-set, or by value with jerk): the direct kernel
+    // (direct.cu) streams the pack once, one launch; it keeps whole per-thread sums in fp32, so only
+    // while they stay within R17's 64 terms
+    if (direct) {
         const int grid = direct_grid(a.ntiles, c->sm_count);
-        if (direct_terms_per_lane(a.ntiles, grid) <= 64) {
+        {
             const int nip = ni <= 1 ? 1 : (ni <= 2 ? 2 : (ni <= 4 ? 4 : 8));
             a.jsh = 0;
             a.k0 = 0;
@@ -453,6 +475,16 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     if (!reduce_here) {
         if (launch_reduce(r, c->stream) != cudaSuccess) return NB_ERR_CUDA;
         ++launched;
+        if (xchg) {
+            if (launch_xchg_push(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->xchg_ticket, c->stream) != cudaSuccess)
+                return NB_ERR_CUDA;
+            ++launched;
+            if (c->xchg_call == 0) {
+                if (launch_xchg_sum(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->err, c->stream) != cudaSuccess)
+                    return NB_ERR_CUDA;
+                ++launched;
+            }
+        }
     }
     if (rec) {
         cudaEventRecord(rec->e[2], c->stream);
@@ -465,6 +497,23 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     c->last[3] = mode;
     c->launches += launched;
     return NB_OK;
+}
+
+void xchg_release(nb_ctx* c)
+{
+    for (int r = 0; r < XCHG_MAX_WORLD; ++r) {
+        if (c->xchg_ipc[r] && c->xchg_host.win[r]) cudaIpcCloseMemHandle(c->xchg_host.win[r]);
+        c->xchg_ipc[r] = false;
+    }
+    if (c->xchg_win) cudaFree(c->xchg_win);
+    if (c->xchg_dev) cudaFree(c->xchg_dev);
+    if (c->xchg_ticket) cudaFree(c->xchg_ticket);
+    c->xchg_win = nullptr;
+    c->xchg_dev = nullptr;
+    c->xchg_ticket = nullptr;
+    c->xchg_host = Xchg{};
+    c->xchg_epoch = 0;
+    cudaGetLastError();
 }
 
 }  // namespace
@@ -483,6 +532,7 @@ const char* nb_strerror(int status)
         case NB_ERR_INDEX: return "particle index out of range";
         case NB_ERR_STATE: return "call out of order (predict before force; workspace before data)";
         case NB_ERR_ARCH: return "device is not compute capability 10.x";
+        case NB_ERR_PEER: return "a peer rank did not answer the exchange in time";
         default: return "unknown status";
     }
 }
@@ -545,6 +595,7 @@ int nb_destroy(nb_ctx* c)
     if (c->steps_exec) cudaGraphExecDestroy(c->steps_exec);
     if (c->steps_graph) cudaGraphDestroy(c->steps_graph);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    xchg_release(c);
     if (c->err_pinned) cudaFreeHost(c->err_pinned);
     for (nb_ctx::Rec& R : c->ring)
         for (cudaEvent_t e : R.e)
@@ -791,6 +842,130 @@ int nb_force_ext_ids(nb_ctx* c, int64_t ni, const double* x, const double* v, co
     if (ni > 0 && (!x || !v || !self_idx || !acc || !jrk || !pot)) return NB_ERR_ARG;
     DeviceGuard g(c->device);
     return force_impl(c, nullptr, ni, eps2, acc, jrk, pot, x, v, self_idx, iflags);
+}
+
+int nb_xchg_create(nb_ctx* c, int rank, int world, int64_t ni_cap)
+{
+    if (!c || world < 1 || world > XCHG_MAX_WORLD || rank < 0 || rank >= world || ni_cap < 1 || ni_cap > c->ni_max)
+        return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    xchg_release(c);
+    const size_t bytes = (size_t)XCHG_HDR + (size_t)2 * world * NOUT * (size_t)ni_cap * sizeof(double);
+    if (cudaMalloc(&c->xchg_win, bytes) != cudaSuccess || cudaMalloc(&c->xchg_dev, sizeof(Xchg)) != cudaSuccess ||
+        cudaMalloc(&c->xchg_ticket, sizeof(unsigned)) != cudaSuccess) {
+        xchg_release(c);
+        return NB_ERR_ALLOC;
+    }
+    c->xchg_host.rank = rank;
+    c->xchg_host.world = world;
+    c->xchg_host.ni_cap = ni_cap;
+    c->xchg_host.win[rank] = c->xchg_win;
+    if (cudaMemset(c->xchg_win, 0, bytes) != cudaSuccess || cudaMemset(c->xchg_ticket, 0, sizeof(unsigned)) != cudaSuccess ||
+        cudaMemcpy(c->xchg_dev, &c->xchg_host, sizeof(Xchg), cudaMemcpyHostToDevice) != cudaSuccess) {
+        xchg_release(c);
+        return NB_ERR_CUDA;
+    }
+    return NB_OK;
+}
+
+int nb_xchg_export(nb_ctx* c, unsigned char* handle, void** dev_ptr)
+{
+    if (!c || (!handle && !dev_ptr)) return NB_ERR_ARG;
+    if (!c->xchg_win) return NB_ERR_STATE;
+    DeviceGuard g(c->device);
+    if (handle) {
+        static_assert(sizeof(cudaIpcMemHandle_t) == NB_XCHG_HANDLE_BYTES, "IPC handle size");
+        cudaIpcMemHandle_t h;
+        if (cudaIpcGetMemHandle(&h, c->xchg_win) != cudaSuccess) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        memcpy(handle, &h, sizeof(h));
+    }
+    if (dev_ptr) *dev_ptr = c->xchg_win;
+    return NB_OK;
+}
+
+int nb_xchg_attach(nb_ctx* c, int peer, const unsigned char* handle, void* same_process_ptr)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->xchg_win) return NB_ERR_STATE;
+    if (peer < 0 || peer >= c->xchg_host.world || (!handle == !same_process_ptr)) return NB_ERR_ARG;
+    if (peer == c->xchg_host.rank) return NB_OK;           // my own window is attached by nb_xchg_create
+    DeviceGuard g(c->device);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
+    if (c->xchg_ipc[peer] && c->xchg_host.win[peer]) cudaIpcCloseMemHandle(c->xchg_host.win[peer]);
+    c->xchg_ipc[peer] = false;
+    c->xchg_host.win[peer] = nullptr;
+    if (handle) {
+        cudaIpcMemHandle_t h;
+        memcpy(&h, handle, sizeof(h));
+        void* p = nullptr;
+        if (cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+            cudaGetLastError();
+            return NB_ERR_CUDA;
+        }
+        c->xchg_host.win[peer] = static_cast<unsigned char*>(p);
+        c->xchg_ipc[peer] = true;
+    } else {
+        // a window of another context of THIS process; on another device peer access is switched on
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, same_process_ptr) != cudaSuccess || at.type != cudaMemoryTypeDevice) {
+            cudaGetLastError();
+            return NB_ERR_ARG;
+        }
+        if (at.device != c->device) {
+            const cudaError_t e = cudaDeviceEnablePeerAccess(at.device, 0);
+            if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) {
+                cudaGetLastError();
+                return NB_ERR_CUDA;
+            }
+            cudaGetLastError();
+        }
+        c->xchg_host.win[peer] = static_cast<unsigned char*>(same_process_ptr);
+    }
+    if (cudaMemcpy(c->xchg_dev, &c->xchg_host, sizeof(Xchg), cudaMemcpyHostToDevice) != cudaSuccess) return NB_ERR_CUDA;
+    return NB_OK;
+}
+
+int nb_xchg_destroy(nb_ctx* c)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard g(c->device);
+    cudaStreamSynchronize(c->stream);
+    xchg_release(c);
+    return NB_OK;
+}
+
+int nb_xforce(nb_ctx* c, int phase, int64_t ni, const double* x, const double* v, const int32_t* self_idx,
+              const uint8_t* iflags, double eps2, double* acc, double* jrk, double* pot)
+{
+    if (!c || phase < 0 || phase > 2 || ni < 0 || !isfinite(eps2) || eps2 < 0.0) return NB_ERR_ARG;
+    if (!c->xchg_win) return NB_ERR_STATE;
+    for (int r = 0; r < c->xchg_host.world; ++r)
+        if (!c->xchg_host.win[r]) return NB_ERR_STATE;   // a peer's window is not attached yet
+    if (ni > c->xchg_host.ni_cap) return NB_ERR_ARG;
+    if (ni > 0 && (!acc || !jrk || !pot || (phase != 2 && (!x || !v)))) return NB_ERR_ARG;
+    if (c->precision != 0 || c->tune_reduce != 0) return NB_ERR_STATE;   // mixed precision, partial-sum reduction
+    if (ni == 0) return NB_OK;
+    DeviceGuard g(c->device);
+    if (phase == 2) {
+        // the other half of a phase-1 call: wait for the peers' pushes of that epoch, add in rank order
+        if (c->xchg_epoch == 0) return NB_ERR_STATE;
+        if (launch_xchg_sum(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->err, c->stream) != cudaSuccess)
+            return NB_ERR_CUDA;
+        c->launches += 1;
+        return NB_OK;
+    }
+    int rc = ensure_alloc(c);
+    if (rc != NB_OK) return rc;
+    if (!c->predicted) return NB_ERR_STATE;
+    c->xchg_epoch += 1;
+    c->xchg_call = phase;
+    rc = force_impl(c, nullptr, ni, eps2, acc, jrk, pot, x, v, self_idx, iflags);
+    c->xchg_call = -1;
+    return rc;
 }
 
 int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double* acc,
@@ -1568,11 +1743,12 @@ int nb_sync(nb_ctx* c)
     }
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NB_ERR_CUDA;
     if (*c->err_pinned) {
-        // device latch: bit 0 = an index was out of range, bit 1 = a due particle had a zero step
+        // device latch: bit 0 = an index was out of range, bit 1 = a due particle had a zero step,
+        // bit 2 = a peer did not answer an exchange (nb_xforce)
         const int bits = *c->err_pinned;
         *c->err_pinned = 0;
         if (cudaMemsetAsync(c->err, 0, sizeof(int), c->stream) != cudaSuccess) return NB_ERR_CUDA;
-        return (bits & 1) ? NB_ERR_INDEX : NB_ERR_STATE;
+        return (bits & 1) ? NB_ERR_INDEX : ((bits & 4) ? NB_ERR_PEER : NB_ERR_STATE);
     }
     return NB_OK;
 }

@@ -109,6 +109,9 @@ struct ReduceArgs {
     const int32_t* ext_self;
     const uint8_t* ext_flags;
     unsigned* counter;        // ticket counter of the few-i kernel's own reduction (zero between calls)
+    const struct Xchg* xchg;  // j-sharded call (nb_xforce, xchg.h): the rank's exchange descriptor, else NULL
+    unsigned xchg_epoch;      // ... the call's epoch
+    int xchg_phase;           // ... 0: push, wait and sum inside the reducing CTA; 1: push only
 };
 
 // kernel launchers (each returns the cudaError of the launch)

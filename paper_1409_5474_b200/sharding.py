@@ -117,3 +117,40 @@ def force_j_sharded(force_by_value_ids, state_local, pos_local, ni, lo, hi, grou
     part = torch.cat([acc, jrk, pot.reshape(1, -1)], dim=0).contiguous()
     dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
     return part[0:3], part[3:6], part[6]
+
+
+# ---- (3) j-sharding with the exchange done by the kernels (nb.h: nb_xchg_*, nb_xforce) -----------
+#
+# Step 4 above -- the paper's "second kernel", across GPUs -- without a collective call: every rank
+# owns a window in device memory, the pair kernel's reducing CTA stores the rank's partial forces into
+# every rank's window over NVLink peer memory, raises a flag, waits for the peers' flags and adds the
+# slots in rank order (csrc/xchg.h).  What is host logic is the one-time wiring: exchanging the
+# windows' IPC handles.
+
+
+def xchg_connect(ctx, ni_cap, group=None):
+    """Create this rank's window (ctx.xchg_create), exchange the IPC handles with all ranks of the
+    group (one all_gather_object), attach every peer's window, barrier.  ctx: a Context (or anything
+    with xchg_create / xchg_export / xchg_attach).  Returns (rank, world)."""
+    rank, world = dist.get_rank(group), dist.get_world_size(group)
+    ctx.xchg_create(rank, world, ni_cap)
+    handle, _ = ctx.xchg_export()
+    handles = [None] * world
+    dist.all_gather_object(handles, handle, group=group)
+    for r in range(world):
+        if r != rank:
+            ctx.xchg_attach(r, handle=handles[r])
+    dist.barrier(group=group)                 # nobody pushes before everybody has attached
+    return rank, world
+
+
+def force_j_sharded_xchg(ctx, state_local, pos_local, ni, lo, hi, eps2, group=None):
+    """force_j_sharded with step 4 inside the kernels: gathers the active particles' state (step 2,
+    still one all_gather -- an integrator that keeps the active state replicated, as the paper's host
+    does, needs none), then ONE ctx.xforce call returns the complete forces on every rank."""
+    st = gather_active_state(state_local, pos_local, ni, group)
+    gidx = st[7].to(torch.int64)
+    mine = (gidx >= lo) & (gidx < hi)
+    self_idx = torch.where(mine, gidx - lo, torch.full_like(gidx, -1)).to(torch.int32)
+    iflags = st[6].to(torch.uint8)
+    return ctx.xforce(st[0:3].contiguous(), st[3:6].contiguous(), self_idx, iflags, eps2)

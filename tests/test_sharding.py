@@ -144,3 +144,131 @@ def test_force_j_sharded_world2_gloo(ni, eps2):
     assert sorted(r[0] for r in res) == [0, 1]
     assert all(r[1] < 1e-12 for r in res), res
     assert all(r[2] for r in res), res
+
+
+def _worker_x(rank, world, port, ni, eps2, out_q):
+    """Host logic of the peer-memory exchange (sharding.xchg_connect / force_j_sharded_xchg).  The
+    stand-in context does on the CPU what csrc/xchg.h does on the device -- every rank has a window of
+    `world` slots, a push writes a rank's partial forces into slot [rank] of EVERY window, the sum adds
+    the slots of one's own window in rank order -- with files under a shared directory as the
+    "peer memory" and the oracle as each rank's pair kernel."""
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import tempfile
+    import time
+    import torch.distributed as dist
+    import nbgen
+    import oracle
+    from paper_1409_5474_b200 import sharding
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        c = nbgen.config1(777)
+        c.m = c.m * (0.5 + nbgen.Streams(9, c.n).uniform())
+        c.flags[[5, 300, 390, 776]] = 1
+        c.x[:, 390] = c.x[:, 5] + 1e-3
+        lo, hi = sharding.shard_bounds(c.n, rank, world)
+        shared = [tempfile.mkdtemp(prefix="nbx%d_" % rank)]
+
+        class Window:
+            def __init__(self):
+                self.rank = self.world = None
+                self.cap = 0
+                self.peers = {}
+                self.epoch = 0
+                self.log = []
+
+            def xchg_create(self, r, w, ni_cap):
+                self.rank, self.world, self.cap = r, w, ni_cap
+                self.peers = {r: shared[0]}
+                self.log.append(("create", r, w))
+
+            def xchg_export(self):
+                return ("%-64s" % shared[0]).encode()[:64], 0
+
+            def xchg_attach(self, peer, handle=None, same_process_ptr=None):
+                assert handle is not None and len(handle) == 64 and peer != self.rank
+                self.peers[peer] = handle.decode().strip()
+                self.log.append(("attach", peer))
+
+            def xforce(self, x, v, self_idx, iflags, eps2_):
+                assert sorted(self.peers) == list(range(self.world)) and x.shape[1] <= self.cap
+                self.epoch += 1
+                xi, vi, sidx, ifl = x.numpy(), v.numpy(), self_idx.numpy(), iflags.numpy()
+                k = xi.shape[1]
+                mm = np.concatenate([c.m[lo:hi], np.zeros(k)])
+                xx = np.concatenate([c.x[:, lo:hi], xi], 1)
+                vv = np.concatenate([c.v[:, lo:hi], vi], 1)
+                ff = np.concatenate([c.flags[lo:hi], ifl]).astype(np.uint8)
+                who = np.where(sidx >= 0, sidx, hi - lo + np.arange(k)).astype(np.int32)
+                a, j, p = oracle.force(mm, xx, vv, who, eps2_, ff)
+                part = np.concatenate([a, j, p[None]], 0)
+                buf = self.epoch & 1
+                for peer, d in self.peers.items():                      # push: data, then the flag
+                    np.save(os.path.join(d, "slot%d_%d.npy" % (buf, self.rank)), part)
+                    with open(os.path.join(d, "flag%d_%d.tmp" % (buf, self.rank)), "w") as f:
+                        f.write(str(self.epoch))
+                    os.replace(os.path.join(d, "flag%d_%d.tmp" % (buf, self.rank)),
+                               os.path.join(d, "flag%d_%d" % (buf, self.rank)))
+                total = None
+                for r in range(self.world):                             # wait and sum, rank 0 first
+                    fn = os.path.join(shared[0], "flag%d_%d" % (buf, r))
+                    t0 = time.time()
+                    while True:
+                        try:
+                            if int(open(fn).read() or -1) == self.epoch:
+                                break
+                        except (OSError, ValueError):
+                            pass
+                        assert time.time() - t0 < 60
+                        time.sleep(0.001)
+                    s = np.load(os.path.join(shared[0], "slot%d_%d.npy" % (buf, r)))
+                    total = s if total is None else total + s
+                t = torch.from_numpy(total)
+                return t[0:3], t[3:6], t[6]
+
+        w = Window()
+        assert sharding.xchg_connect(w, 512) == (rank, world)
+        assert w.log == [("create", rank, world)] + [("attach", r) for r in range(world) if r != rank]
+        worst, same = 0.0, True
+        for call in range(3):                                           # walks through both buffers
+            il = nbgen.permutation(6 + call, c.n)[:ni].copy()
+            il[:min(ni, 4)] = [5, 390, 300, 776][:min(ni, 4)]
+            pos = sharding.owned(il, lo, hi)
+            mine = il[pos.numpy()]
+            state = torch.from_numpy(np.concatenate([c.x[:, mine], c.v[:, mine],
+                                                     c.flags[None, mine].astype(np.float64),
+                                                     mine[None].astype(np.float64)], 0))
+            acc, jrk, pot = sharding.force_j_sharded_xchg(w, state, pos, len(il), lo, hi, eps2)
+            ra, rj, rp = oracle.force(c.m, c.x, c.v, il, eps2, c.flags)
+            worst = max(worst, np.abs(acc.numpy() - ra).max() / np.abs(ra).max(),
+                        np.abs(jrk.numpy() - rj).max() / np.abs(rj).max(),
+                        np.abs(pot.numpy() - rp).max() / np.abs(rp).max())
+            both = [None] * world
+            dist.all_gather_object(both, (acc.numpy().tobytes(), jrk.numpy().tobytes(), pot.numpy().tobytes()))
+            same = same and all(b == both[0] for b in both)             # identical bits on every rank
+        out_q.put((rank, float(worst), bool(same)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("ni,eps2", [(301, 1e-4), (5, 1e-12)])
+def test_xchg_host_logic_world2_gloo(ni, eps2):
+    """sharding.xchg_connect wires every rank to every peer's window (handles travel by
+    all_gather_object, own rank skipped, barrier before the first push) and force_j_sharded_xchg returns
+    the unsharded force on every rank, bit-identical across ranks (rank-order sum)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker_x, args=(r, 2, port, ni, eps2, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=180) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [0, 1]
+    assert all(r[1] < 1e-12 for r in res), res
+    assert all(r[2] for r in res), res
