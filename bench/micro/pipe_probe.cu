@@ -383,6 +383,69 @@ __global__ void __launch_bounds__(128, MINB) body_chain_kernel(float* out, int r
     out[blockIdx.x * 128 + tid] = res;
 }
 
+// ---------------- encoding C, thread-level instead of instruction-level parallelism ----------------
+// One evaluation (one i against one j-pair) per loop trip and IPT i per thread: with a single
+// evaluation in flight ptxas emits its instructions in dependency order, which keeps the chains
+// t = al*d + w (x3, al shared) and sum += mr3*(d|t) (x6, mr3 shared) together, so that the reuse
+// cache serves the shared operand; latency is hidden by the other warps (NT/32 x MINB per SM).
+template <int IPT, int PAIRS, int MINB, int NT>
+__global__ void __launch_bounds__(NT, MINB) body_tlp_kernel(float* out, int reps, float eps2f)
+{
+    __shared__ __align__(16) float T[10 * TJ];       // xh yh zh xl yl zl vx vy vz m
+    const int tid = threadIdx.x;
+    for (int q = tid; q < TJ; q += NT) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.37 * ((q * 2654435761u + c * 40503u) % 1000) / 1000.0 - 0.18;
+            const float h = (float)x;
+            T[c * TJ + q] = h;
+            T[(3 + c) * TJ + q] = (float)(x - (double)h);
+            T[(6 + c) * TJ + q] = 0.01f * (float)((q * 7 + c * 13) % 17 - 8);
+        }
+        T[9 * TJ + q] = 1.0f / 1048576.0f;
+    }
+    __syncthreads();
+    float2 nxh[IPT][3], nxl[IPT][3], nv[IPT][3];
+    Acc A[IPT];
+    for (int u = 0; u < IPT; ++u) {
+        for (int c = 0; c < 3; ++c) {
+            const double x = 0.001 * (tid + NT * u) + 0.1 * c + 1e-9 * blockIdx.x;
+            const float h = (float)x;
+            nxh[u][c] = dup(-h);
+            nxl[u][c] = dup(-(float)(x - (double)h));
+            nv[u][c] = dup(0.003f * (tid % 7) - 0.01f * c + 0.002f * u);
+        }
+        A[u].ax = A[u].ay = A[u].az = A[u].jx = A[u].jy = A[u].jz = A[u].p = make_float2(0.f, 0.f);
+    }
+    const float2 eps2 = dup(eps2f), m3 = dup(-3.0f);
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll 1
+        for (int p = 0; p < TJ; p += 2 * PAIRS) {
+            float2 f[PAIRS][10];
+#pragma unroll
+            for (int h = 0; h < PAIRS; ++h)
+#pragma unroll
+                for (int c = 0; c < 10; ++c) f[h][c] = *reinterpret_cast<const float2*>(T + c * TJ + p + 2 * h);
+#pragma unroll
+            for (int h = 0; h < PAIRS; ++h)
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+                    float2 d[3], w[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        d[c] = __fadd2_rn(__fadd2_rn(f[h][c], nxh[u][c]), __fadd2_rn(f[h][3 + c], nxl[u][c]));
+                        w[c] = __fadd2_rn(f[h][6 + c], nv[u][c]);
+                    }
+                    body32(d[0], d[1], d[2], w[0], w[1], w[2], f[h][9], eps2, m3, A[u]);
+                }
+        }
+    }
+    float res = 0.f;
+    for (int u = 0; u < IPT; ++u)
+        res += A[u].ax.x + A[u].ax.y + A[u].ay.x + A[u].ay.y + A[u].az.x + A[u].az.y + A[u].jx.x + A[u].jx.y +
+               A[u].jy.x + A[u].jy.y + A[u].jz.x + A[u].jz.y + A[u].p.x + A[u].p.y;
+    out[blockIdx.x * NT + tid] = res;
+}
+
 struct Acc1 { float ax, ay, az, jx, jy, jz, p; };
 
 __device__ __forceinline__ void body1(float dx, float dy, float dz, float wx, float wy, float wz, float m,
@@ -676,6 +739,22 @@ void run_chain()
            SEP, UNR, MINB, fa.numRegs, occ, ms, r, r / 1.2408e12 * 100);
 }
 
+template <int IPT, int PAIRS, int MINB, int NT>
+void run_tlp()
+{
+    const int reps = 300;
+    const int grid = nsm * MINB * 5;
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, body_tlp_kernel<IPT, PAIRS, MINB, NT>, NT, 0));
+    cudaFuncAttributes fa;
+    CK(cudaFuncGetAttributes(&fa, body_tlp_kernel<IPT, PAIRS, MINB, NT>));
+    float ms = time_ms([&] { body_tlp_kernel<IPT, PAIRS, MINB, NT><<<grid, NT>>>(d_out, reps, 1e-6f); });
+    const double inter = (double)grid * NT * IPT * (double)TJ * reps;
+    const double r = inter / (ms * 1e-3);
+    printf("tlp body C: ipt %d pairs/trip %d threads %3d minb %d regs %3d occ %2d (%2d warps/SM): %8.3f ms  %9.3e inter/s = %5.1f%% of 1.2408e12\n",
+           IPT, PAIRS, NT, MINB, fa.numRegs, occ, occ * NT / 32, ms, r, r / 1.2408e12 * 100);
+}
+
 template <int KIND>
 void run_rate(const char* name, double ops_per_iter_thread, int ctas_per_sm)
 {
@@ -765,6 +844,14 @@ int main(int argc, char** argv)
         run_chain<3, 3, 1>(); run_chain<3, 3, 2>();
         run_chain<3, 4, 1>(); run_chain<3, 4, 2>(); run_chain<4, 4, 1>();
         run_chain<3, 5, 1>(); run_chain<3, 5, 2>(); run_chain<4, 5, 1>();
+    }
+    if (all || !strcmp(what, "tlp")) {
+        printf("-- pair body C, one evaluation in flight per thread, latency hidden by warps\n");
+        run_tlp<1, 1, 8, 128>(); run_tlp<1, 1, 6, 128>(); run_tlp<1, 1, 4, 128>(); run_tlp<1, 1, 4, 256>();
+        run_tlp<1, 2, 8, 128>(); run_tlp<1, 2, 6, 128>(); run_tlp<1, 2, 4, 256>();
+        run_tlp<2, 1, 6, 128>(); run_tlp<2, 1, 4, 128>(); run_tlp<2, 1, 3, 128>(); run_tlp<2, 1, 3, 256>();
+        run_tlp<2, 2, 4, 128>(); run_tlp<2, 2, 3, 128>();
+        run_tlp<4, 1, 3, 128>(); run_tlp<4, 1, 4, 128>();
     }
     if (all || !strcmp(what, "hetero")) {
         printf("-- fp32 two-float (2 i per thread) and fp64 (ipt i per thread) warps in one CTA\n");
