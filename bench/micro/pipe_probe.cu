@@ -852,6 +852,7 @@ int main(int argc, char** argv)
         run_tlp<2, 1, 6, 128>(); run_tlp<2, 1, 4, 128>(); run_tlp<2, 1, 3, 128>(); run_tlp<2, 1, 3, 256>();
         run_tlp<2, 2, 4, 128>(); run_tlp<2, 2, 3, 128>();
         run_tlp<4, 1, 3, 128>(); run_tlp<4, 1, 4, 128>();
+        run_tlp<4, 2, 2, 128>(); run_tlp<3, 2, 3, 128>(); run_tlp<3, 2, 2, 128>(); run_tlp<3, 1, 3, 128>(); run_tlp<3, 1, 4, 128>();
     }
     if (all || !strcmp(what, "hetero")) {
         printf("-- fp32 two-float (2 i per thread) and fp64 (ipt i per thread) warps in one CTA\n");
