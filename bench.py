@@ -635,58 +635,78 @@ def run_fewi(args):
     n = case.n
     dev = torch.device("cuda", 0)
     rows = []
-    with nbm.Context(n, 1 << 10) as ctx:
+    n_small = 1024            # the same call on the case's first 1024 particles: what a call costs before any streaming
+    with nbm.Context(n, 1 << 10) as ctx, nbm.Context(n_small, 1 << 10) as small:
         ctx.load_case(case)
-        h = ctx.h
+        sl = slice(0, n_small)
+        small.set_j(case.m[sl], case.x[:, sl], case.v[:, sl], case.a[:, sl], case.j[:, sl], case.t[sl])
         flush = torch.zeros(256 << 20, dtype=torch.uint8, device=dev)      # > L2: reading it evicts the pack / store
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def timed(c, call):
+            """(a) back to back, the j data resident in L2 as far as it fits; (b) every call after an L2
+            flush, timed alone with events around the call (median of 20)."""
+            for _ in range(5):
+                call()
+            c.sync()
+            reps = 200
+            e0.record()
+            for _ in range(reps):
+                call()
+            e1.record()
+            c.sync()
+            warm = e0.elapsed_time(e1) / reps * 1e3
+            cold = []
+            for _ in range(20):
+                flush.sum()                 # a READ pass: the L2 then holds clean lines of this buffer only
+                e0.record()
+                call()
+                e1.record()
+                c.sync()
+                cold.append(e0.elapsed_time(e1) * 1e3)
+            return warm, float(np.median(cold))
+
         for ni in (1, 2, 4, 8, 16, 64):
-            d_il = torch.from_numpy(np.ascontiguousarray(il_all[:ni])).to(dev)
+            il_big = torch.from_numpy(np.ascontiguousarray(il_all[:ni])).to(dev)
+            il_small = torch.arange(ni, dtype=torch.int32, device=dev)
             o = [torch.empty((3, ni), dtype=torch.float64, device=dev),
                  torch.empty((3, ni), dtype=torch.float64, device=dev),
                  torch.empty((ni,), dtype=torch.float64, device=dev)]
             for name in ("nb_force", "nb_force_fused"):
                 if name == "nb_force_fused" and ni > nb.NB_FUSED_MAX:
                     continue
-                if name == "nb_force":
-                    nb.nb_predict(h, t)
-                    call = lambda: nb.nb_force(h, d_il, ni, case.eps2, *o)
-                    nbytes = 44.0 * n
-                else:
-                    call = lambda: nb.nb_force_fused(h, t, d_il, ni, case.eps2, *o)
-                    nbytes = 112.0 * n
-                for _ in range(5):
-                    call()
-                ctx.sync()
-                # (a) back to back, the j data resident in L2 as far as it fits; (b) every call after an
-                # L2 flush, timed alone with events around the call
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                reps = 200
-                e0.record()
-                for _ in range(reps):
-                    call()
-                e1.record()
-                ctx.sync()
-                warm = e0.elapsed_time(e1) / reps * 1e3
-                cold = []
-                for _ in range(20):
-                    flush.sum()                 # a READ pass: the L2 then holds clean lines of this buffer only
-                    e0.record()
-                    call()
-                    e1.record()
-                    ctx.sync()
-                    cold.append(e0.elapsed_time(e1) * 1e3)
-                cold_us = float(np.median(cold))
+                res = {}
+                for c, d_il, nn in ((ctx, il_big, n), (small, il_small, n_small)):
+                    h = c.h
+                    if name == "nb_force":
+                        nb.nb_predict(h, t)
+                        call = lambda: nb.nb_force(h, d_il, ni, case.eps2, *o)
+                        per = 44.0
+                    else:
+                        call = lambda: nb.nb_force_fused(h, t, d_il, ni, case.eps2, *o)
+                        per = 112.0
+                    res[nn] = timed(c, call)
+                warm, cold_us = res[n]
+                warm_s, cold_s = res[n_small]
+                nbytes = per * n
                 info = ctx.last_launch()
                 rows.append({"call": name, "n_i": ni, "us_per_call_back_to_back": warm, "us_per_call_after_l2_flush": cold_us,
                              "bytes_per_call": nbytes, "gbs_after_flush": nbytes / cold_us / 1e3,
                              "hbm_frac": nbytes / cold_us / 1e3 / peaks["hbm_gbs"],
                              "gbs_back_to_back": nbytes / warm / 1e3,
+                             "us_same_call_n1024_back_to_back": warm_s, "us_same_call_n1024_after_l2_flush": cold_s,
+                             "gbs_incremental_after_flush": per * (n - n_small) / max(cold_us - cold_s, 1e-3) / 1e3,
+                             "hbm_frac_incremental": per * (n - n_small) / max(cold_us - cold_s, 1e-3) / 1e3 / peaks["hbm_gbs"],
                              "kernels": int(info["kernels"]), "ctas": int(info["ctas"])})
     best = max(r["hbm_frac"] for r in rows if r["n_i"] == 1)
     line = {"metric": "GB/s of the j data streamed by one few-i force call", "value": best * peaks["hbm_gbs"],
             "unit": "GB/s", "n_gpus": 1, "steps": 200, "warmup": 5, "higher_is_better": True, "dtype": "f32/f64",
             "data": "synthetic", "config": {"workload": workload + "_few_i", "n_j": n,
-                                            "l2": "hbm_frac rows: the L2 is flushed (a 256 MB buffer is read) before every timed call"},
+                                            "l2": "hbm_frac rows: the L2 is flushed (a 256 MB buffer is read) before every timed call",
+                                            "incremental": "the same call on the first 1024 particles is timed the same way: "
+                                                           "hbm_frac_incremental = bytes of the other N - 1024 particles over "
+                                                           "the time difference, i.e. the streaming rate without the call's "
+                                                           "fixed latency (launch, gather, ticket, reduction, event overhead)"},
             "roofline": {"bound": "hbm", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "unit": "GB/s",
                          "achieved": best * peaks["hbm_gbs"], "frac": best, "traffic": None},
             "rows": rows}
