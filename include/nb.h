@@ -219,13 +219,15 @@ int nb_force_fused(nb_ctx* c, double t, const int32_t* i_list, int64_t ni, doubl
  *   forces when the call's kernels have run; phase 1: compute and push only (acc / jrk / pot then hold
  *   this rank's partial forces); phase 2: the other half of the last phase-1 call -- wait for the peers
  *   and sum into acc / jrk / pot (x, v, self_idx, iflags, eps2 are ignored).  The split form lets a
- *   caller put other work between the halves.  A peer that has not pushed within 20 s latches
- *   NB_ERR_PEER (returned by nb_sync); the outputs are then meaningless.  ni > ni_cap: NB_ERR_ARG. */
+ *   caller put other work between the halves.  A peer that has not pushed within the time limit
+ *   (20 s; nb_xchg_set_timeout: seconds in (0, 3600]) latches NB_ERR_PEER (returned by nb_sync); the
+ *   outputs are then meaningless.  ni > ni_cap: NB_ERR_ARG. */
 #define NB_XCHG_HANDLE_BYTES 64
 int nb_xchg_create(nb_ctx* c, int rank, int world, int64_t ni_cap);
 int nb_xchg_export(nb_ctx* c, unsigned char* handle, void** dev_ptr);
 int nb_xchg_attach(nb_ctx* c, int peer, const unsigned char* handle, void* same_process_ptr);
 int nb_xchg_destroy(nb_ctx* c);
+int nb_xchg_set_timeout(nb_ctx* c, double seconds);
 int nb_xforce(nb_ctx* c, int phase, int64_t ni, const double* x, const double* v, const int32_t* self_idx,
               const uint8_t* iflags, double eps2, double* acc, double* jrk, double* pot);
 

@@ -21,7 +21,7 @@ EXPORTS = [
     "nb_predict", "nb_get_predicted", "nb_force", "nb_force_ext", "nb_force_ext_ids", "nb_force_fused", "nb_set_fused", "nb_force_host", "nb_set_order", "nb_force6", "nb_set_precision", "nb_set_tuning",
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_steps", "nb_set_steps_bound", "nb_set_steps_queue", "nb_block_forces", "nb_strerror", "nb_version",
-    "nb_xchg_create", "nb_xchg_export", "nb_xchg_attach", "nb_xchg_destroy", "nb_xforce",
+    "nb_xchg_create", "nb_xchg_export", "nb_xchg_attach", "nb_xchg_destroy", "nb_xchg_set_timeout", "nb_xforce",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -81,6 +81,7 @@ lib.nb_xchg_create.argtypes = [_vp, _i32, _i32, _i64]
 lib.nb_xchg_export.argtypes = [_vp, _vp, ctypes.POINTER(_vp)]
 lib.nb_xchg_attach.argtypes = [_vp, _i32, _vp, _vp]
 lib.nb_xchg_destroy.argtypes = [_vp]
+lib.nb_xchg_set_timeout.argtypes = [_vp, _dbl]
 lib.nb_xforce.argtypes = [_vp, _i32, _i64, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]
 
 
@@ -264,6 +265,10 @@ def nb_xchg_attach(c, peer, handle=None, same_process_ptr=None):
     _check(lib.nb_xchg_attach(c, int(peer), ctypes.cast(buf, ctypes.c_void_p) if buf is not None else None,
                               ctypes.c_void_p(same_process_ptr) if same_process_ptr is not None else None),
            "nb_xchg_attach")
+
+
+def nb_xchg_set_timeout(c, seconds):
+    _check(lib.nb_xchg_set_timeout(c, float(seconds)), "nb_xchg_set_timeout")
 
 
 def nb_xchg_destroy(c):

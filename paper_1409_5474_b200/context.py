@@ -178,6 +178,9 @@ class Context:
     def xchg_attach(self, peer, handle=None, same_process_ptr=None):
         nb.nb_xchg_attach(self.h, peer, handle, same_process_ptr)
 
+    def xchg_timeout(self, seconds):
+        nb.nb_xchg_set_timeout(self.h, seconds)
+
     def xchg_destroy(self):
         nb.nb_xchg_destroy(self.h)
 

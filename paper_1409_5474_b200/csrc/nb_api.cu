@@ -23,6 +23,7 @@ struct nb_ctx {
     bool xchg_ipc[XCHG_MAX_WORLD] = {}; // win[r] was opened from an IPC handle (closed by nb_xchg_destroy)
     unsigned xchg_epoch = 0;            // epoch of the last push
     int xchg_call = -1;                 // phase of the nb_xforce call in progress (-1: an ordinary force call)
+    unsigned long long xchg_limit_ns = XCHG_LIMIT_NS;
     int sm_count = 148;
     int blocks_per_sm[8] = {1, 1, 1, 1, 1, 1, 1, 1};   // all-i kernel, its guarded form, few-i kernel, its guarded form; [4..7] the same for nb_steps' device-planned kernels
 
@@ -402,6 +403,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
         r.xchg = c->xchg_dev;
         r.xchg_epoch = c->xchg_epoch;
         r.xchg_phase = c->xchg_call;
+        r.xchg_limit_ns = c->xchg_limit_ns;
     }
 
     int launched = 0;
@@ -480,7 +482,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
                 return NB_ERR_CUDA;
             ++launched;
             if (c->xchg_call == 0) {
-                if (launch_xchg_sum(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->err, c->stream) != cudaSuccess)
+                if (launch_xchg_sum(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->err, c->xchg_limit_ns, c->stream) != cudaSuccess)
                     return NB_ERR_CUDA;
                 ++launched;
             }
@@ -929,6 +931,13 @@ int nb_xchg_attach(nb_ctx* c, int peer, const unsigned char* handle, void* same_
     return NB_OK;
 }
 
+int nb_xchg_set_timeout(nb_ctx* c, double seconds)
+{
+    if (!c || !(seconds > 0.0) || seconds > 3600.0) return NB_ERR_ARG;
+    c->xchg_limit_ns = (unsigned long long)(seconds * 1e9);
+    return NB_OK;
+}
+
 int nb_xchg_destroy(nb_ctx* c)
 {
     if (!c) return NB_ERR_ARG;
@@ -953,7 +962,7 @@ int nb_xforce(nb_ctx* c, int phase, int64_t ni, const double* x, const double* v
     if (phase == 2) {
         // the other half of a phase-1 call: wait for the peers' pushes of that epoch, add in rank order
         if (c->xchg_epoch == 0) return NB_ERR_STATE;
-        if (launch_xchg_sum(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->err, c->stream) != cudaSuccess)
+        if (launch_xchg_sum(c->xchg_dev, c->xchg_epoch, acc, jrk, pot, ni, c->err, c->xchg_limit_ns, c->stream) != cudaSuccess)
             return NB_ERR_CUDA;
         c->launches += 1;
         return NB_OK;

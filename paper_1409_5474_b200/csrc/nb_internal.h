@@ -112,6 +112,7 @@ struct ReduceArgs {
     const struct Xchg* xchg;  // j-sharded call (nb_xforce, xchg.h): the rank's exchange descriptor, else NULL
     unsigned xchg_epoch;      // ... the call's epoch
     int xchg_phase;           // ... 0: push, wait and sum inside the reducing CTA; 1: push only
+    unsigned long long xchg_limit_ns;   // ... how long to wait for a peer
 };
 
 // kernel launchers (each returns the cudaError of the launch)

@@ -39,9 +39,9 @@ __global__ void __launch_bounds__(XT) xchg_push_kernel(const Xchg* __restrict__ 
 // every CTA waits for the flags by itself (it depends on the peers only, never on another CTA of this
 // grid), then sums its share of the slots in rank order
 __global__ void __launch_bounds__(XT) xchg_sum_kernel(const Xchg* __restrict__ X, unsigned epoch, double* acc, double* jrk,
-                                                       double* pot, long long ni, int* err)
+                                                       double* pot, long long ni, int* err, unsigned long long limit_ns)
 {
-    xchg_wait(X, epoch, threadIdx.x, err, XCHG_LIMIT_NS);
+    xchg_wait(X, epoch, threadIdx.x, err, limit_ns);
     const long long total = (long long)NOUT * ni;
     for (long long q = (long long)blockIdx.x * XT + threadIdx.x; q < total; q += (long long)gridDim.x * XT) {
         const int c = (int)(q / ni);
@@ -67,9 +67,9 @@ cudaError_t launch_xchg_push(const Xchg* X, unsigned epoch, double* acc, double*
 }
 
 cudaError_t launch_xchg_sum(const Xchg* X, unsigned epoch, double* acc, double* jrk, double* pot, long long ni, int* err,
-                            cudaStream_t s)
+                            unsigned long long limit_ns, cudaStream_t s)
 {
-    xchg_sum_kernel<<<grid_for(ni), XT, 0, s>>>(X, epoch, acc, jrk, pot, ni, err);
+    xchg_sum_kernel<<<grid_for(ni), XT, 0, s>>>(X, epoch, acc, jrk, pot, ni, err, limit_ns);
     return cudaGetLastError();
 }
 

@@ -102,7 +102,7 @@ __device__ __forceinline__ double xchg_sum(const Xchg* X, unsigned epoch, int c,
     return s;
 }
 
-constexpr unsigned long long XCHG_LIMIT_NS = 20ull * 1000ull * 1000ull * 1000ull;   // 20 s
+constexpr unsigned long long XCHG_LIMIT_NS = 20ull * 1000ull * 1000ull * 1000ull;   // default: 20 s (nb_xchg_set_timeout)
 
 // The exchange inside the CTA that has just reduced a j-sharded call (force.cu few-i kernel, direct.cu):
 // what R.acc / R.jrk / R.pot hold is this rank's PARTIAL force.  The CTA (NT threads, all of them call
@@ -123,7 +123,7 @@ __device__ __forceinline__ void xchg_in_cta(const ReduceArgs& R, int* err, int t
     }
     xchg_raise(X, R.xchg_epoch, tid);
     if (R.xchg_phase == 0) {
-        xchg_wait(X, R.xchg_epoch, tid, err, XCHG_LIMIT_NS);
+        xchg_wait(X, R.xchg_epoch, tid, err, R.xchg_limit_ns);
         for (int q = tid; q < total; q += NT) {
             const int c = q / R.ni, k = q % R.ni;
             *out_ptr(R.acc, R.jrk, R.pot, c, k, R.ni) = xchg_sum(X, R.xchg_epoch, c, k);
@@ -136,6 +136,6 @@ __device__ __forceinline__ void xchg_in_cta(const ReduceArgs& R, int* err, int t
 cudaError_t launch_xchg_push(const Xchg* X, unsigned epoch, double* acc, double* jrk, double* pot, long long ni,
                              unsigned* ticket, cudaStream_t s);
 cudaError_t launch_xchg_sum(const Xchg* X, unsigned epoch, double* acc, double* jrk, double* pot, long long ni, int* err,
-                            cudaStream_t s);
+                            unsigned long long limit_ns, cudaStream_t s);
 
 }  // namespace nb

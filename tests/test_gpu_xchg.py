@@ -218,3 +218,30 @@ def test_two_processes_share_windows_by_ipc_handle(nbmod):
     assert sorted(r[0] for r in res) == [0, 1]
     assert all(r[1] <= 1.0 for r in res), res          # within the north_star tolerances of the oracle
     assert all(r[2] for r in res), res                 # identical bits in both processes
+
+
+def test_a_silent_peer_is_reported_not_waited_for_forever(nbmod):
+    """Rank 0 of 2 whose peer never pushes: the wait gives up after the time limit, latches NB_ERR_PEER
+    (nb_sync) and the context stays usable."""
+    n, t = 2048, 0.1
+    m, x, v, a, j, tj = _j_set(n, 940)
+    flags = np.zeros(n, np.uint8)
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    with nbmod.Context(n, 64) as c0, nbmod.Context(n, 64) as c1:
+        for r, c in enumerate((c0, c1)):
+            _load_slice(c, 0, n, m, x, v, a, j, tj, flags, t)
+            c.xchg_create(r, 2, 64)
+        c0.xchg_attach(1, same_process_ptr=c1.xchg_export()[1])
+        c0.xchg_timeout(0.05)
+        il = np.arange(5, dtype=np.int32)
+        for ni in (5, 40):                                     # in the pair kernel's last CTA; in xchg_sum_kernel
+            c0.xforce(xp[:, :ni], vp[:, :ni], np.arange(ni, dtype=np.int32), None, 1e-4)
+            with pytest.raises(nbmod.binding.NBError) as e:
+                c0.sync()
+            assert e.value.status == nbmod.binding.NB_ERR_PEER
+        c0.sync()                                              # the latch is cleared
+        got = [q.cpu().numpy() for q in c0.force(il, 1e-4)]
+        c0.sync()
+        check_parity(got, oracle.force(m, xp, vp, il, 1e-4))
+        with pytest.raises(nbmod.binding.NBError):
+            c0.xchg_timeout(0.0)
