@@ -53,7 +53,7 @@ constexpr int ST_SMEM = STEPS_NI_MAX * 6 * 8 + NOUT * ST_TILE * 8 + ST_KEYS * 8;
 // NB_STEPS_TRACE (development builds only): CTA 0 stamps %globaltimer at the phase boundaries of every
 // step into the partial buffer's tail, 8 words per step
 #ifdef NB_STEPS_TRACE
-#define TRACE(k) do { if (b == 0 && tid == 0) P.trace[s * 8 + (k)] = gtime(); } while (0)
+#define TRACE(k) do { if (P.trace && b == 0 && tid == 0) P.trace[s * 8 + (k)] = gtime(); } while (0)
 #else
 #define TRACE(k) do { } while (0)
 #endif
