@@ -127,6 +127,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
     __shared__ unsigned long long swmin[ST_WARPS];
     __shared__ int swsum[ST_WARPS];
     __shared__ int goff[ST_GMAX + 1];
+    __shared__ __align__(16) int sfirst[ST_GMAX][4];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = (int)gridDim.x, b = (int)blockIdx.x;
@@ -189,8 +190,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
         unsigned long long kg = ~0ull;
         int cg_ = 0;
         if (tid < G) {
-            kg = __ldcg(&slots[tid].key);
-            cg_ = __ldcg(&slots[tid].count);
+            // key, count and -- in the same round trip -- the first four published indices of the slice:
+            // most blocks are a handful of particles, whose indices then need no second trip
+            const int4 head = __ldcg(reinterpret_cast<const int4*>(&slots[tid].key));
+            kg = ((unsigned long long)(unsigned)head.y << 32) | (unsigned)head.x;
+            cg_ = head.z;
+            *reinterpret_cast<int4*>(&sfirst[tid][0]) = __ldcg(reinterpret_cast<const int4*>(&slots[tid].idx[0]));
         }
         const unsigned long long kall = block_min(kg, swmin, lane, warp);
         const int mine = (tid < G && kg == kall && kall != ~0ull) ? cg_ : 0;
@@ -271,7 +276,8 @@ __global__ void __launch_bounds__(ST_THREADS, 1) steps_kernel(StepsArgs P)
                 if (goff[gm] <= tid) g0 = gm;
                 else g1 = gm;
             }
-            const int64_t i = __ldcg(&slots[g0].idx[tid - goff[g0]]);
+            const int pos = tid - goff[g0];
+            const int64_t i = pos < 4 ? sfirst[g0][pos] : __ldcg(&slots[g0].idx[pos]);
             sl[tid] = (int)i;
             // ---- C: predicted i-particles ...
             const double dti = t1 - ldcg(T + i);
