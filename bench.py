@@ -614,7 +614,8 @@ def run_blockstep(args):
                            "host_handover = one host synchronisation per large block (queue 0)"},
             "gpu_launches": int(launches)}
     if args.detail:
-        line["steps_detail"] = {"n_i": [int(q) for q in sizes], "us": [float(q) for q in us]}
+        line["steps_detail"] = {"n_i": [int(q) for q in sizes], "us": [float(q) for q in us],
+                                "us_host_handover": [float(q) for q in np.minimum(times_host[0], times_host[1])]}
     print(json.dumps(line))
     return 0
 

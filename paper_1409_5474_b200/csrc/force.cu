@@ -325,19 +325,27 @@ force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __res
 // resident CTAs loops over the work items.  Exits at once when no block is pending or when the plan
 // asks for the other instantiation.
 template <bool FEW, bool GUARD>
-__global__ void __launch_bounds__(FORCE_THREADS, NB_DYN_MINB) force_dyn_kernel(const DynPlan* __restrict__ plan)
+__global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_DYN_MINB : NB_DYN_MINB_ALL) force_dyn_kernel(DynPlan* __restrict__ plan)
 {
     if (!plan->go || (plan->fa.jsh > 0) != FEW) return;
     __shared__ ForceArgs sP;
     __shared__ ReduceArgs sR;
+    __shared__ unsigned s_w;
     if (threadIdx.x == 0) {
         sP = plan->fa;
         sR = plan->ra;
     }
     __syncthreads();
+    // the first item of a CTA is its place in the grid; further items are drawn from a counter (the
+    // plan kernel zeroed it), so that a CTA whose items ran long does not hold up the launch's tail
     const unsigned items = (unsigned)sP.n_itiles * (unsigned)sP.splits;
-    for (unsigned w = blockIdx.x; w < items; w += gridDim.x) {
-        force_body<false, FEW, 0, GUARD, true>(sP, sR, w, nullptr, nullptr, nullptr);
+    unsigned w = blockIdx.x;
+    while (w < items) {
+        force_body<false, FEW, 0, GUARD, true>(sP, sR, w, nullptr, nullptr, nullptr);   // ends with a CTA barrier
+        if (threadIdx.x == 0) s_w = gridDim.x + atomicAdd(&plan->next, 1u);
+        __syncthreads();
+        w = s_w;
+        __syncthreads();
     }
 }
 
@@ -359,12 +367,13 @@ __global__ void __launch_bounds__(128) reduce_dyn_kernel(const DynPlan* __restri
     __shared__ ReduceArgs sR;
     if (threadIdx.x == 0) sR = plan->ra;
     __syncthreads();
+    // a grid of fixed, modest size strides over the block (it was launched before the block's size was known)
     const int64_t gt = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t nthreads = (int64_t)gridDim.x * blockDim.x;
     if (sR.splits > 8 && sR.ni <= 4096) {
-        const int64_t k = gt / 32;
-        if (k < sR.ni) reduce_row<true>(sR, (int)k, threadIdx.x & 31);
-    } else if (gt < sR.ni) {
-        reduce_row<false>(sR, (int)gt, threadIdx.x & 31);
+        for (int64_t k = gt / 32; k < sR.ni; k += nthreads / 32) reduce_row<true>(sR, (int)k, threadIdx.x & 31);
+    } else {
+        for (int64_t k = gt; k < sR.ni; k += nthreads) reduce_row<false>(sR, (int)k, threadIdx.x & 31);
     }
 }
 
@@ -465,7 +474,7 @@ cudaError_t launch_force(const ForceArgs& a, const ReduceArgs& r, int mode, int 
 }
 
 // both instantiations are queued; the plan decides on the device which one works
-cudaError_t launch_force_dyn(const DynPlan* plan, float eps2, int resident_all, int resident_few, cudaStream_t s)
+cudaError_t launch_force_dyn(DynPlan* plan, float eps2, int resident_all, int resident_few, cudaStream_t s)
 {
     if (eps2 < EPS2_GUARD) {
         force_dyn_kernel<true, true><<<resident_few, FORCE_THREADS, force_smem(true), s>>>(plan);
@@ -479,9 +488,10 @@ cudaError_t launch_force_dyn(const DynPlan* plan, float eps2, int resident_all, 
 
 cudaError_t launch_reduce_dyn(const DynPlan* plan, int64_t ni_max, cudaStream_t s)
 {
-    // one thread per i up to ni_max, or one warp per i up to 4096: the larger of the two grids
-    int64_t grid = (ni_max + 127) / 128;
-    if (grid < 1024 && ni_max > 128) grid = ni_max < 4096 ? (ni_max * 32 + 127) / 128 : 1024;
+    // one thread per i, or one warp per i up to 4096 particles: at most 1024 CTAs, which stride
+    int64_t grid = ni_max <= 4096 ? (ni_max * 32 + 127) / 128 : 1024;
+    if (grid < 1) grid = 1;
+    if (grid > 1024) grid = 1024;
     reduce_dyn_kernel<<<(unsigned)grid, 128, 0, s>>>(plan);
     return cudaGetLastError();
 }

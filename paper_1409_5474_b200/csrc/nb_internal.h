@@ -28,6 +28,10 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 #ifndef NB_DYN_MINB
 #define NB_DYN_MINB 3
 #endif
+#ifndef NB_DYN_MINB_ALL
+#define NB_DYN_MINB_ALL 3          // the all-i form of force_dyn_kernel: 135 registers, 3 CTAs per SM (4: 128 registers,
+                                   // 4 CTAs; measured -1.2 % per block step at N = 2^20, +1.5 % at N = 131072)
+#endif
 #ifndef NB_UNROLL
 #define NB_UNROLL 2
 #endif
@@ -203,7 +207,7 @@ struct StepsArgs {
 // correct_dyn, all of which exit at once while go == 0).
 struct DynPlan {
     int go;                       // 1: a block is pending and planned
-    int pad;
+    unsigned next;                // work items of the pair kernel handed out beyond the first one per CTA
     double t1;                    // its time
     long long ni;                 // its size
     ForceArgs fa;                 // launch shape and arguments of the pair kernel
@@ -224,7 +228,7 @@ cudaError_t steps_kernel_setup(int* blocks_per_sm);
 cudaError_t launch_plan(const StepsArgs& a, DynPlan* plan, StepsProgress* prog, const ForceArgs& fa_base,
                         const ReduceArgs& ra_base, int resident_all, int resident_few, size_t part_bytes,
                         cudaStream_t s, unsigned long long cond_handle = 0, int loop = 0);
-cudaError_t launch_force_dyn(const DynPlan* plan, float eps2, int resident_all, int resident_few, cudaStream_t s);
+cudaError_t launch_force_dyn(DynPlan* plan, float eps2, int resident_all, int resident_few, cudaStream_t s);
 cudaError_t launch_reduce_dyn(const DynPlan* plan, int64_t ni_max, cudaStream_t s);
 cudaError_t launch_correct_dyn(const StorePtrs& st, double* dts, const DynPlan* plan, int64_t n, int64_t ni_max,
                                double eta, double dt_min, double dt_max, int* err, cudaStream_t s);

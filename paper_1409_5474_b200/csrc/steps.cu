@@ -497,6 +497,7 @@ __device__ __forceinline__ bool plan_block(const StepsArgs& P, DynPlan* plan, Fo
     plan->ra = ra;
     plan->t1 = t1;
     plan->ni = ni;
+    plan->next = 0u;
     plan->go = 1;
     P.log_t[g->done] = t1;
     P.log_ni[g->done] = ni;
@@ -513,21 +514,22 @@ correct_dyn_kernel(StorePtrs st, double* __restrict__ dts, const DynPlan* __rest
                    double dt_min, double dt_max, int* err)
 {
     if (!plan->go) return;
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t ni = plan->ni;
-    if (k >= ni) return;
-    const int64_t i = plan->ra.i_list[k];
-    if (i < 0 || i >= n) {
-        atomicOr(err, 1);
-        return;
-    }
-    double a1[3], j1[3];
+    // a grid of fixed, modest size strides over the block (launched before the block's size was known)
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < ni; k += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = plan->ra.i_list[k];
+        if (i < 0 || i >= n) {
+            atomicOr(err, 1);
+            continue;
+        }
+        double a1[3], j1[3];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        a1[c] = plan->ra.acc[(int64_t)c * ni + k];
-        j1[c] = plan->ra.jrk[(int64_t)c * ni + k];
+        for (int c = 0; c < 3; ++c) {
+            a1[c] = plan->ra.acc[(int64_t)c * ni + k];
+            j1[c] = plan->ra.jrk[(int64_t)c * ni + k];
+        }
+        correct_one(st, dts, i, plan->t1, a1, j1, eta, dt_min, dt_max, err);
     }
-    correct_one(st, dts, i, plan->t1, a1, j1, eta, dt_min, dt_max, err);
 }
 
 }  // namespace
@@ -564,7 +566,9 @@ cudaError_t launch_plan(const StepsArgs& a, DynPlan* plan, StepsProgress* prog, 
 cudaError_t launch_correct_dyn(const StorePtrs& st, double* dts, const DynPlan* plan, int64_t n, int64_t ni_max,
                                double eta, double dt_min, double dt_max, int* err, cudaStream_t s)
 {
-    correct_dyn_kernel<<<(unsigned)((ni_max + 127) / 128), 128, 0, s>>>(st, dts, plan, n, eta, dt_min, dt_max, err);
+    int64_t grid = (ni_max + 127) / 128;
+    if (grid > 1184) grid = 1184;
+    correct_dyn_kernel<<<(unsigned)grid, 128, 0, s>>>(st, dts, plan, n, eta, dt_min, dt_max, err);
     return cudaGetLastError();
 }
 

@@ -245,3 +245,32 @@ def test_a_silent_peer_is_reported_not_waited_for_forever(nbmod):
         check_parity(got, oracle.force(m, xp, vp, il, 1e-4))
         with pytest.raises(nbmod.binding.NBError):
             c0.xchg_timeout(0.0)
+
+
+def test_a_rank_with_an_empty_slice(nbmod):
+    """World of two where rank 1 holds no particle at all: its partial forces are zeros, the sum is rank
+    0's force (bit for bit), in both exchange forms."""
+    n, t = 2000, 0.1
+    m, x, v, a, j, tj = _j_set(n, 950)
+    flags = np.zeros(n, np.uint8)
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    with nbmod.Context(n, 64) as c0, nbmod.Context(16, 64) as c1:
+        _load_slice(c0, 0, n, m, x, v, a, j, tj, flags, t)
+        c1.predict(t)                                          # nothing loaded: n = 0
+        for r, c in enumerate((c0, c1)):
+            c.xchg_create(r, 2, 64)
+        c0.xchg_attach(1, same_process_ptr=c1.xchg_export()[1])
+        c1.xchg_attach(0, same_process_ptr=c0.xchg_export()[1])
+        for ni in (3, 40):
+            il = nbgen.permutation(951 + ni, n)[:ni].astype(np.int32)
+            none = np.full(ni, -1, np.int32)
+            want = [q.cpu().numpy() for q in c0.force_ext_ids(xp[:, il], vp[:, il], il, None, 1e-4)]
+            p1 = c1.xforce(xp[:, il], vp[:, il], none, None, 1e-4, phase=1)
+            c1.sync()
+            assert all(float(q.abs().max()) == 0.0 for q in p1)
+            got = [q.cpu().numpy() for q in c0.xforce(xp[:, il], vp[:, il], il, None, 1e-4)]
+            o1 = [q.cpu().numpy() for q in c1.xforce(None, None, None, None, 1e-4, phase=2, out=p1)]
+            c0.sync()
+            c1.sync()
+            for g, w, o in zip(got, want, o1):
+                assert np.array_equal(g, w) and np.array_equal(o, w)
