@@ -154,3 +154,63 @@ def force_j_sharded_xchg(ctx, state_local, pos_local, ni, lo, hi, eps2, group=No
     self_idx = torch.where(mine, gidx - lo, torch.full_like(gidx, -1)).to(torch.int32)
     iflags = st[6].to(torch.uint8)
     return ctx.xforce(st[0:3].contiguous(), st[3:6].contiguous(), self_idx, iflags, eps2)
+
+
+# ---- (4) one block step of the j-sharded integrator (host logic around the C-ABI calls) -----------
+#
+# PAPER.md:41/:49 (block time steps: "only the particles are updated that require a force update at a
+# certain time") on the j-sharded layout of PAPER.md:55: every rank schedules, predicts and corrects
+# ITS slice; what crosses ranks per block step is one double (the block time), the state of the due
+# particles (72 B each) and their partial forces (56 B each).
+
+
+def step_j_sharded(ctx, lo, hi, flags_local, eps2, eta, dt_min, dt_max, group=None, exchange="xchg"):
+    """One block step.  ctx: this rank's Context holding particles [lo, hi) with steps initialised
+    (init_steps / set_dt); flags_local: device uint8 tensor (hi - lo,) of their flag bits.
+    exchange: "xchg" = nb_xforce (partial forces exchanged and summed by the kernels over peer memory:
+    xchg_connect first), "xchg_split" = the same with the two halves of the call separated by a host
+    barrier (for ranks that share one GPU: no kernel then waits for another process's kernel), "nccl" =
+    nb_force_ext_ids + all_reduce.  Returns (t, ni): the block time and the number of particles
+    advanced over all ranks.  Every rank must call it."""
+    dev = flags_local.device
+    # 1. my slice's earliest time and who is due then (R21); the block time is the minimum over ranks
+    t_loc, ni_loc, il_loc = ctx.next_block()
+    tt = torch.tensor([t_loc if ni_loc > 0 else float("inf")], dtype=torch.float64, device=dev)
+    dist.all_reduce(tt, op=dist.ReduceOp.MIN, group=group)
+    t = float(tt.item())
+    due = il_loc.to(torch.int64) if (ni_loc > 0 and t_loc == t) else torch.empty(0, dtype=torch.int64, device=dev)
+    # 2. my slice predicted to t (R1, R8); the predicted state of my due particles travels to all ranks,
+    #    in rank order = ascending global index (R21)
+    ctx.predict(t)
+    px, pv = ctx.predicted()
+    k = due.shape[0]
+    counts = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(dist.get_world_size(group))]
+    dist.all_gather(counts, torch.tensor([k], dtype=torch.int64, device=dev), group=group)
+    counts = [int(c.item()) for c in counts]
+    ni, first = sum(counts), sum(counts[:dist.get_rank(group)])
+    pos = first + torch.arange(k, dtype=torch.int64, device=dev)
+    state = torch.cat([px[:, due], pv[:, due], flags_local[due].to(torch.float64)[None],
+                       (due + lo).to(torch.float64)[None]], 0)
+    st = gather_active_state(state, pos, ni, group)
+    gidx = st[7].to(torch.int64)
+    mine = (gidx >= lo) & (gidx < hi)
+    self_idx = torch.where(mine, gidx - lo, torch.full_like(gidx, -1)).to(torch.int32)
+    iflags = st[6].to(torch.uint8)
+    x, v = st[0:3].contiguous(), st[3:6].contiguous()
+    # 3. forces of ALL ranks' particles on the due ones (PAPER.md:55)
+    if exchange == "xchg":
+        acc, jrk, _ = ctx.xforce(x, v, self_idx, iflags, eps2)
+    elif exchange == "xchg_split":
+        part = ctx.xforce(x, v, self_idx, iflags, eps2, phase=1)
+        ctx.sync()
+        dist.barrier(group=group)
+        acc, jrk, _ = ctx.xforce(None, None, None, None, eps2, phase=2, out=part)
+    else:
+        acc, jrk, pot = ctx.force_ext_ids(x, v, self_idx, iflags, eps2)
+        part = torch.cat([acc, jrk, pot.reshape(1, -1)], 0).contiguous()
+        dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
+        acc, jrk = part[0:3], part[3:6]
+    # 4. corrector, new steps (R12, R18..R20): the owners, on their own particles
+    if k:
+        ctx.correct(due.to(torch.int32), t, acc[:, pos].contiguous(), jrk[:, pos].contiguous(), eta, dt_min, dt_max)
+    return t, ni

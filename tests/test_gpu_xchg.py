@@ -274,3 +274,85 @@ def test_a_rank_with_an_empty_slice(nbmod):
             c1.sync()
             for g, w, o in zip(got, want, o1):
                 assert np.array_equal(g, w) and np.array_equal(o, w)
+
+
+def _step_worker(rank, world, port, out_q):
+    import os
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    sys.path.insert(0, os.path.join(root, "tests"))
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch.distributed as dist
+    from oracle import hermite as H
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import sharding
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n, eps2, eta, dmin, dmax, steps = 1024, 2.0 ** -12, 0.02, 2.0 ** -14, 2.0 ** -6, 14
+        m, x, v = nbgen.plummer(n, 960)
+        m = m * (0.5 + nbgen.Streams(961, n).uniform())
+        flags = np.zeros(n, np.uint8)
+        flags[[10, 900]] = 1
+        il = np.arange(n, dtype=np.int32)
+        a, j, _ = oracle.force(m, x, v, il, eps2, flags)
+        t = np.zeros(n)
+        dt = H.quantise_dt(H.initial_dt(a, j, eta), dmin, dmax)
+        lo, hi = sharding.shard_bounds(n, rank, world)
+        sl = slice(lo, hi)
+        dev = torch.device("cuda", 0)
+        with nbm.Context(hi - lo, n) as ctx:
+            ctx.set_j(m[sl], x[:, sl], v[:, sl], a[:, sl], j[:, sl], t[sl])
+            fl = np.flatnonzero(flags[sl]).astype(np.int32)
+            if len(fl):
+                ctx.set_flags(fl, np.ones(len(fl), np.uint8))
+            ctx.set_dt(dt[sl])
+            sharding.xchg_connect(ctx, n)
+            fdev = torch.from_numpy(flags[sl].copy()).to(dev)
+            log = [sharding.step_j_sharded(ctx, lo, hi, fdev, eps2, eta, dmin, dmax, exchange="xchg_split")
+                   for _ in range(steps)]
+            ctx.sync()
+            mine = ctx.state().cpu().numpy()
+            dist.barrier()
+        # the same steps by ONE context holding all particles (nb_step), on this rank's own
+        with nbm.Context(n) as full:
+            full.set_j(m, x, v, a, j, t)
+            full.set_flags(np.array([10, 900], np.int32), np.ones(2, np.uint8))
+            full.set_dt(dt)
+            ref = [full.step(eps2, eta, dmin, dmax) for _ in range(steps)]
+            full.sync()
+            want = full.state().cpu().numpy()[:, sl]
+        same_log = [(float(q[0]), int(q[1])) for q in log] == [(float(q[0]), int(q[1])) for q in ref]
+        err_x = float(np.abs(mine[1:4] - want[1:4]).max())
+        err_v = float(np.abs(mine[4:7] - want[4:7]).max())
+        same_dt = bool(np.array_equal(mine[13], want[13]) and np.array_equal(mine[14], want[14]))
+        out_q.put((rank, same_log, err_x, err_v, same_dt, int(max(q[1] for q in ref))))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_block_steps_of_two_ranks_equal_one_context(nbmod):
+    """sharding.step_j_sharded with real contexts: two processes on the one GPU, each scheduling,
+    predicting and correcting half of 1024 particles, forces through nb_xforce (split halves: no kernel
+    waits for another process's kernel).  14 block steps give the block times, block sizes, particle
+    times and power-of-two steps of ONE context running nb_step on all particles, and its positions to
+    fp32-summation order."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_step_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=300) for _ in procs]
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [0, 1]
+    assert all(r[1] for r in res), res
+    assert all(r[2] < 1e-9 and r[3] < 1e-7 for r in res), res
+    assert all(r[4] for r in res), res

@@ -272,3 +272,104 @@ def test_xchg_host_logic_world2_gloo(ni, eps2):
     assert sorted(r[0] for r in res) == [0, 1]
     assert all(r[1] < 1e-12 for r in res), res
     assert all(r[2] for r in res), res
+
+
+def _worker_step(rank, world, port, steps, out_q):
+    """sharding.step_j_sharded over gloo: every rank's context is a stand-in that keeps a slice of the
+    particles and answers next_block / predict / predicted / force_ext_ids / correct with the oracle
+    (oracle/hermite.py, oracle.predict, oracle.force).  The sharded run must reproduce the oracle's
+    unsharded block-step integration: same block times and sizes, same state."""
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch.distributed as dist
+    import nbgen
+    import oracle
+    from oracle import hermite as H
+    from paper_1409_5474_b200 import sharding
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n, eps2, eta, dmin, dmax = 200, 2.0 ** -10, 0.02, 2.0 ** -12, 2.0 ** -6
+        m, x, v = nbgen.plummer(n, 977)
+        m = m * (0.5 + nbgen.Streams(978, n).uniform())
+        flags = np.zeros(n, np.uint8)
+        flags[[3, 150]] = 1
+        il = np.arange(n, dtype=np.int32)
+        a, j, _ = oracle.force(m, x, v, il, eps2, flags)
+        t = np.zeros(n)
+        dt = H.quantise_dt(H.initial_dt(a, j, eta), dmin, dmax)
+        lo, hi = sharding.shard_bounds(n, rank, world)
+
+        class Slice:
+            """particles [lo, hi) of the set, with the oracle as every kernel"""
+            def __init__(self):
+                sl = slice(lo, hi)
+                self.m, self.x, self.v = m[sl].copy(), x[:, sl].copy(), v[:, sl].copy()
+                self.a, self.j, self.t, self.dt = a[:, sl].copy(), j[:, sl].copy(), t[sl].copy(), dt[sl].copy()
+                self.f = flags[sl].copy()
+
+            def next_block(self):
+                t1, idx = H.next_block(self.t, self.dt)
+                return t1, len(idx), torch.from_numpy(idx)
+
+            def predict(self, tp):
+                self.xp, self.vp = oracle.predict(tp, self.x, self.v, self.a, self.j, self.t)
+
+            def predicted(self):
+                return torch.from_numpy(self.xp), torch.from_numpy(self.vp)
+
+            def force_ext_ids(self, xi, vi, sidx, ifl, e2):
+                xi, vi, sidx, ifl = xi.numpy(), vi.numpy(), sidx.numpy(), ifl.numpy()
+                k = xi.shape[1]
+                mm = np.concatenate([self.m, np.zeros(k)])
+                xx = np.concatenate([self.xp, xi], 1)
+                vv = np.concatenate([self.vp, vi], 1)
+                ff = np.concatenate([self.f, ifl]).astype(np.uint8)
+                who = np.where(sidx >= 0, sidx, hi - lo + np.arange(k)).astype(np.int32)
+                fa, fj, fp = oracle.force(mm, xx, vv, who, e2, ff)
+                return torch.from_numpy(fa), torch.from_numpy(fj), torch.from_numpy(fp)
+
+            def correct(self, idx, t1, a1, j1, eta_, dmin_, dmax_):
+                H.corrector_step(self.x, self.v, self.a, self.j, self.t, self.dt, idx.numpy().astype(np.int64), t1,
+                                 a1.numpy(), j1.numpy(), eta_, dmin_, dmax_)
+
+        me = Slice()
+        fl = torch.from_numpy(me.f)
+        log = [sharding.step_j_sharded(me, lo, hi, fl, eps2, eta, dmin, dmax, exchange="nccl") for _ in range(steps)]
+        # the unsharded oracle run from the same start
+        ref = []
+        for _ in range(steps):
+            t1, idx = H.next_block(t, dt)
+            xp, vp = oracle.predict(t1, x, v, a, j, t)
+            a1, j1, _ = oracle.force(m, xp, vp, idx, eps2, flags)
+            H.corrector_step(x, v, a, j, t, dt, idx, t1, a1, j1, eta, dmin, dmax)
+            ref.append((t1, len(idx)))
+        sl = slice(lo, hi)
+        same_log = [(float(q[0]), int(q[1])) for q in log] == [(float(q[0]), int(q[1])) for q in ref]
+        err = max(np.abs(me.x - x[:, sl]).max(), np.abs(me.v - v[:, sl]).max(), np.abs(me.a - a[:, sl]).max() * 1e-3)
+        same_dt = bool(np.array_equal(me.dt, dt[sl]) and np.array_equal(me.t, t[sl]))
+        out_q.put((rank, same_log, float(err), same_dt, max(q[1] for q in ref)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_step_j_sharded_world2_gloo():
+    """PAPER.md:41/:49 on the j-sharded layout of PAPER.md:55: 40 block steps (past t = 2^-6, where
+    every particle is due at once) with two ranks equal the unsharded oracle integration."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker_step, args=(r, 2, port, 40, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=180) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [0, 1]
+    assert all(r[1] for r in res), res                 # block times and sizes identical to the unsharded run
+    assert all(r[2] < 1e-11 for r in res), res         # state equal up to the order of the fp64 additions
+    assert all(r[3] for r in res), res                 # every particle's time and power-of-two step identical
+    assert res[0][4] == 200                            # the run contains the all-particles block
