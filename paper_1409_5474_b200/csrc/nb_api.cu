@@ -971,6 +971,7 @@ int nb_xforce(nb_ctx* c, int phase, int64_t ni, const double* x, const double* v
     if (rc != NB_OK) return rc;
     if (!c->predicted) return NB_ERR_STATE;
     c->xchg_epoch += 1;
+    if (c->xchg_epoch == 0) c->xchg_epoch = 2;     // 0 is the windows' initial flag value; parity keeps alternating
     c->xchg_call = phase;
     rc = force_impl(c, nullptr, ni, eps2, acc, jrk, pot, x, v, self_idx, iflags);
     c->xchg_call = -1;
