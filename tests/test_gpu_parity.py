@@ -354,3 +354,28 @@ def test_bitwise_repeatability_of_every_kernel_path(nbmod):
                     assert all(np.array_equal(p, q) for p, q in zip(first, got)), (ni, rep)
             ctx.sync()
         side.synchronize()
+
+
+def test_sixteen_million_particles(nbmod):
+    """Largest size exercised: N = 2^24 + 5 (1.9 GB of j-store, 131073 tiles with a ragged last one),
+    four times config 5.  Active subsets of 3, 40 and 600 particles (the first and the last particle
+    among them) against ALL j: the handful falls back from the direct kernel to the tile kernel here
+    (its per-thread fp32 sums would exceed R17's 64 terms), the others take the threads-per-i and the
+    all-i mapping.  Oracle: every checked particle against all 16.8 M."""
+    n, eps2 = (1 << 24) + 5, 1e-6
+    m, x, v = nbgen.plummer(n, 4242)
+    a, j = nbgen.mean_field(x, v)
+    tj = 0.01 * nbgen.Streams(4243, n).uniform()
+    t = 0.01
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    with nbmod.Context(n, 1024) as ctx:
+        ctx.set_j(m, x, v, a, j, tj)
+        ctx.predict(t)
+        for ni in (3, 40, 600):
+            il = nbgen.permutation(7 + ni, n)[:ni].astype(np.int32)
+            il[0], il[1] = n - 1, 0
+            got = [q.cpu().numpy() for q in ctx.force(il, eps2)]
+            ctx.sync()
+            print("N=2^24+5 ni=%d" % ni, check_parity(got, oracle.force(m, xp, vp, il, eps2)), ctx.last_launch())
+        px, _ = ctx.predicted(n - 4099, 4099)
+        assert rel_err_vec(px.cpu().numpy(), xp[:, n - 4099:]).max() <= 1e-14
