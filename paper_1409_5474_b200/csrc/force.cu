@@ -28,7 +28,10 @@ namespace {
 // g + 2 jl, .. of every tile (neighbouring lanes read neighbouring 16-byte pieces: no bank
 // conflicts), and the jl partial sums meet in a shuffle butterfly before the CTA's partial is
 // written.  Ring depth: the few-i kernel does little arithmetic per tile and lives on bytes in flight.
-__host__ __device__ constexpr int stages_for(bool few) { return few ? 2 * STAGES : STAGES; }
+// few-i kernel: a ring stage holds KT consecutive tiles (one bulk copy, one wait, one release per KT
+// tiles: with 8 j per thread and tile the per-tile ring work was as many instructions as the pairs)
+__host__ __device__ constexpr int tiles_per_stage(bool few) { return few ? 4 : 1; }
+__host__ __device__ constexpr int stages_for(bool few) { return few ? 2 : STAGES; }
 
 // MODE 0: i-particles are members of the j-set, given by index (nb_force).  MODE 1: i-particles
 // given by value, "a completely different set", acc + jerk + pot -- optionally with the
@@ -48,16 +51,18 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
                                            double* __restrict__ opot)
 {
     constexpr int STG = stages_for(FEW);
+    constexpr int KT = tiles_per_stage(FEW);
+    constexpr int STAGE_BYTES = KT * TILE_BYTES;
     constexpr bool JERK = (MODE != 2);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG * TILE_BYTES);
-    int* rel = reinterpret_cast<int*>(smem_raw + STG * TILE_BYTES + STG * 8);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG * STAGE_BYTES);
+    int* rel = reinterpret_cast<int*>(smem_raw + STG * STAGE_BYTES + STG * 8);
     // all-i kernel: the fp64 sums live in shared memory ([u][c][thread], touched once per tile)
     constexpr bool DSM = !FEW;
-    double* sd = reinterpret_cast<double*>(smem_raw + STG * (TILE_BYTES + 16)) + threadIdx.x;
+    double* sd = reinterpret_cast<double*>(smem_raw + STG * (STAGE_BYTES + 16)) + threadIdx.x;
     // index of each i (or -1), only needed in the masked path and in the tail: kept out of registers
-    int* sidx = reinterpret_cast<int*>(smem_raw + STG * (TILE_BYTES + 16) +
+    int* sidx = reinterpret_cast<int*>(smem_raw + STG * (STAGE_BYTES + 16) +
                                        (DSM ? IPT * NOUT * FORCE_THREADS * 8 : 0)) + threadIdx.x;
 
     const int tid = threadIdx.x;
@@ -76,10 +81,11 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
             rel[s] = 0;
         }
         mbar_fence_init();
-        for (int s = 0; s < STG && t0 + s < t1; ++s) {
-            mbar_expect_tx(smem_u32(&bars[s]), TILE_BYTES);
-            bulk_g2s(smem_u32(tiles + s * TILE_FLOATS), P.pack + (int64_t)(t0 + s) * TILE_FLOATS,
-                     TILE_BYTES, smem_u32(&bars[s]));
+        for (int s = 0; s < STG && t0 + s * KT < t1; ++s) {
+            const int nt = t1 - (t0 + s * KT) < KT ? t1 - (t0 + s * KT) : KT;      // tiles are contiguous: one copy
+            mbar_expect_tx(smem_u32(&bars[s]), nt * TILE_BYTES);
+            bulk_g2s(smem_u32(tiles + s * KT * TILE_FLOATS), P.pack + (int64_t)(t0 + s * KT) * TILE_FLOATS,
+                     nt * TILE_BYTES, smem_u32(&bars[s]));
         }
     }
 
@@ -145,10 +151,21 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
     // a3: pair loop over the tiles of the subset.  No CTA-wide barrier inside: a warp that is done
     // with a stage bumps the stage's release counter, and the warp that brings it to a multiple of
     // NWARPS (the last one out) refills the stage, so warps drift up to STG-1 tiles apart.
-    for (int t = t0; t < t1; ++t) {
-        const int st = (t - t0) % STG;
-        mbar_wait(smem_u32(&bars[st]), ((t - t0) / STG) & 1);
-        const float* T = tiles + st * TILE_FLOATS;
+    for (int tg = t0; tg < t1; tg += KT) {
+        const int st = ((tg - t0) / KT) % STG;
+        mbar_wait(smem_u32(&bars[st]), (((tg - t0) / KT) / STG) & 1);
+        const int tend = tg + KT < t1 ? tg + KT : t1;
+        // does the stage hold the own index of one of my i-particles (R5)?  Once per stage, so that
+        // the common tile pays nothing for it
+        bool own = false;
+        if (KT > 1 && (MODE == 1 || (MODE == 0 && !GUARD))) {
+#pragma unroll
+            for (int u = 0; u < IPT; ++u)
+                own = own || (unsigned)(sidx[u * FORCE_THREADS] - tg * TJ) < (unsigned)((tend - tg) * TJ);
+        }
+#pragma unroll 1
+        for (int t = tg; t < tend; ++t) {
+        const float* T = tiles + (st * KT + (t - tg)) * TILE_FLOATS;
 
         // Flagged-flagged pairs (R7): the whole tile goes through the masked scalar pair, warp-uniform;
         // that path also excludes the self pair by index.  Every other tile is packed.
@@ -171,7 +188,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
             // R5 (see pot_lane): when this tile holds the own index of one of my i-particles, in my
             // share of the tile, that particle's fp32 sums are moved to fp64 first, so that the pot
             // lane starts empty (the all-i kernel flushes after every tile anyway)
-            if (FEW && (MODE == 1 || (MODE == 0 && !GUARD))) {
+            if (FEW && own && (MODE == 1 || (MODE == 0 && !GUARD))) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u) {
                     const int q = sidx[u * FORCE_THREADS] - t * TJ;
@@ -195,7 +212,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
                     for (int u = 0; u < IPT; ++u) quad<JERK, GUARD>(I[u], A[u], f, eps2, m3);
                 }
             }
-            if (MODE == 1 || (MODE == 0 && !GUARD)) {
+            if ((KT == 1 || own) && (MODE == 1 || (MODE == 0 && !GUARD))) {
 #pragma unroll
                 for (int u = 0; u < IPT; ++u) {
                     const int q = sidx[u * FORCE_THREADS] - t * TJ;
@@ -230,15 +247,19 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
             }
         }
 
-        // release the stage; the last warp out refills it with tile t + STG
+        }   // tiles of the stage
+
+        // release the stage; the last warp out refills it with the tiles STG stages further on
         __syncwarp();
         if ((tid & 31) == 0) {
             __threadfence_block();     // this warp's reads of the stage are ordered before its release
             const int old = atomicAdd(&rel[st], 1);
-            if ((old & (NWARPS - 1)) == NWARPS - 1 && t + STG < t1) {
-                mbar_expect_tx(smem_u32(&bars[st]), TILE_BYTES);
-                bulk_g2s(smem_u32(tiles + st * TILE_FLOATS),
-                         P.pack + (int64_t)(t + STG) * TILE_FLOATS, TILE_BYTES, smem_u32(&bars[st]));
+            const int tn = tg + STG * KT;
+            if ((old & (NWARPS - 1)) == NWARPS - 1 && tn < t1) {
+                const int nt = t1 - tn < KT ? t1 - tn : KT;
+                mbar_expect_tx(smem_u32(&bars[st]), nt * TILE_BYTES);
+                bulk_g2s(smem_u32(tiles + st * KT * TILE_FLOATS), P.pack + (int64_t)tn * TILE_FLOATS, nt * TILE_BYTES,
+                         smem_u32(&bars[st]));
             }
         }
     }
@@ -392,7 +413,7 @@ constexpr int NWARPS_CHECK = FORCE_THREADS / 32;
 static_assert((NWARPS_CHECK & (NWARPS_CHECK - 1)) == 0, "warps per CTA must be a power of two");
 __host__ __device__ constexpr int force_smem(bool few)
 {
-    return stages_for(few) * (TILE_BYTES + 16) + (few ? 0 : IPT * NOUT * FORCE_THREADS * 8) +
+    return stages_for(few) * (tiles_per_stage(few) * TILE_BYTES + 16) + (few ? 0 : IPT * NOUT * FORCE_THREADS * 8) +
            IPT * FORCE_THREADS * 4;
 }
 
