@@ -301,7 +301,8 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
             } else {
 #pragma unroll
                 for (int c = 0; c < NOUT; ++c)
-                    P.part[((int64_t)c * P.ni_pad + ku) * P.splits + sp2] = o[c];   // [c][i][subset]
+                    P.part[P.part_i_fastest ? ((int64_t)c * P.splits + sp2) * P.ni_pad + ku      // [c][subset][i]
+                                            : ((int64_t)c * P.ni_pad + ku) * P.splits + sp2] = o[c];    // [c][i][subset]
             }
         }
     }

@@ -395,6 +395,13 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     a.reduce_here = reduce_here ? 1 : 0;
     // nb_xforce: the reducing CTA also exchanges with the peers (force.cu); otherwise two small kernels
     // after the reduction do (below)
+    // the thread-per-i reduction (launch_reduce: few subsets or many particles) reads [c][subset][i],
+    // which the pair kernel stores coalesced; the warp-per-i reduction strides over [c][i][subset]
+    {
+        const int most = splits_a > splits_b ? splits_a : splits_b;
+        const bool warp_reduce = !r.atomic_mode && most > 8 && ni <= 4096;
+        a.part_i_fastest = r.part_i_fastest = (!f64 && !reduce_here && !warp_reduce) ? 1 : 0;
+    }
     const bool xchg = c->xchg_call >= 0;
     const bool direct = (kmode == 0 || kmode == 1) && !f64 && !mode && c->tune_splits == 0 && ni <= DIRECT_NI_MAX &&
                         a.ntiles > 0 &&

@@ -94,6 +94,7 @@ struct ForceArgs {
     int any_flagged;
     const double* pack64;     // fp64 tiles (precision mode 1), else unused
     double eps2d;
+    int part_i_fastest;       // partial sums as [c][subset][i] (coalesced stores; the thread-per-i reduction) instead of [c][i][subset]
 };
 
 struct ReduceArgs {
@@ -117,6 +118,7 @@ struct ReduceArgs {
     unsigned xchg_epoch;      // ... the call's epoch
     int xchg_phase;           // ... 0: push, wait and sum inside the reducing CTA; 1: push only
     unsigned long long xchg_limit_ns;   // ... how long to wait for a peer
+    int part_i_fastest;       // layout of part / part_b, as in ForceArgs
 };
 
 // kernel launchers (each returns the cudaError of the launch)

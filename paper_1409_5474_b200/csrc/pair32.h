@@ -248,7 +248,9 @@ __device__ __forceinline__ void reduce_row(const ReduceArgs& R, int k, int lane)
         } else {
             for (int s = 0; s < ns; ++s) {
 #pragma unroll
-                for (int c = 0; c < NOUT; ++c) o[c] += __ldcg(part + ((int64_t)c * stride + kl) * ns + s);
+                for (int c = 0; c < NOUT; ++c)
+                    o[c] += __ldcg(part + (R.part_i_fastest ? ((int64_t)c * ns + s) * stride + kl
+                                                            : ((int64_t)c * stride + kl) * ns + s));
             }
         }
     }
