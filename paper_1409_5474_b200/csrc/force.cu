@@ -335,7 +335,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
 }
 
 template <bool ATOMIC, bool FEW, int MODE, bool GUARD>
-__global__ void __launch_bounds__(FORCE_THREADS, NB_MINB)
+__global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_MINB_FEW : NB_MINB)
 force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __restrict__ ojrk,
              double* __restrict__ opot)
 {

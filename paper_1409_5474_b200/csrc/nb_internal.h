@@ -25,6 +25,9 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 #ifndef NB_MINB
 #define NB_MINB 3
 #endif
+#ifndef NB_MINB_FEW
+#define NB_MINB_FEW 3
+#endif
 #ifndef NB_DYN_MINB
 #define NB_DYN_MINB 3
 #endif
