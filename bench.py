@@ -576,7 +576,7 @@ def run_blockstep(args):
     ms_host, _, launches_host, _, _ = min((r for md, r in runs if md == "steps_host"), key=lambda r: r[0])
     ms, wall, launches, sizes, t = min((r for md, r in runs if md == "steps"), key=lambda r: r[0])
     sizes = np.array(sizes, dtype=np.float64)
-    small = (sizes <= 512) & (sizes * n <= (args.steps_bound if args.steps_bound >= 0 else 3.0e7))
+    small = (sizes <= 512) & (sizes * n <= (args.steps_bound if args.steps_bound >= 0 else 1.5e7))
     in_kernel = int(small.sum())
     us = np.minimum(times[0], times[1])                    # per-step device time (%globaltimer), best of 2
     floor_us = sizes * n / 1.2408e12 * 1e6                  # pair work at 100 % of the FP32 peak
@@ -587,7 +587,7 @@ def run_blockstep(args):
             "data": "synthetic",
             "config": {"workload": "blockstep_plummer_N%d" % n, "eta": eta, "eps2": eps2,
                        "step": "nb_steps: scheduler + predictor-in-pair-loop + reduce + corrector per block in "
-                               "one persistent kernel; blocks above 512 particles or 3e7 pairs: launch shape planned "
+                               "one persistent kernel; blocks above 512 particles or 1.5e7 pairs: launch shape planned "
                                "on the device, predictor + packed fp32 pair kernel + reduction + corrector queued "
                                "ahead of time (no host round trip)"},
             "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),

@@ -343,13 +343,13 @@ int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, do
  * crucial bottleneck"; with individual steps most blocks hold a handful of
  * particles).  One persistent cooperative kernel runs scheduler -> predictor inside an IEEE-double
  * pair loop over the j-store -> reduction -> corrector -> step criterion for step after step
- * (three grid-wide barriers per step, no launch, no synchronisation; same readings R1..R9, R12,
- * R18..R21 and the same decisions as nb_step).  It hands a block back to the host only when the block
+ * (two grid-wide barriers per step, no launch, no synchronisation; same readings R1..R9, R12,
+ * R18..R21 and the same decisions as nb_step).  It leaves a block to other kernels only when the block
  * is large -- more than 512 particles, or N_i x n above the bound of nb_set_steps_bound (default
- * 3e7 pairs) -- because nb_step's packed fp32 pair kernel is then the faster way; after that one
- * nb_step (queued without a second synchronisation: time and size of the block are known) the kernel
- * is started again.  So the host synchronises once per LARGE block and once at the end, never per
- * small block.
+ * 1.5e7 pairs: beyond it the packed fp32 pair kernel plus its launches beats the fp64 loop) -- and
+ * how those kernels are issued is nb_set_steps_queue's choice: by default their launch shape is
+ * planned on the device and they run as the body of a WHILE node of one CUDA graph, so that the host
+ * synchronises once per nb_steps call; in mode 0 once per large block.
  * Stops after k steps, or before the first block whose time exceeds t_end (+inf: no limit; NaN is
  * NB_ERR_ARG).  HOST outputs: *done = steps taken; t_log[0..done), ni_log[0..done) and us_log[0..done)
  * = block time, block size and device time in microseconds (%globaltimer) of every step (each may be

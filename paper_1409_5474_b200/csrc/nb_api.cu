@@ -58,7 +58,7 @@ struct nb_ctx {
     long long* steps_log_ni = nullptr;
     unsigned long long* steps_log_ns = nullptr;
     int64_t steps_log_cap = 0;
-    int64_t steps_max_pairs = 30000000; // blocks with ni x n above this go through nb_step's launches
+    int64_t steps_max_pairs = 15000000; // blocks with ni x n above this go through the packed fp32 pair kernel
     int steps_ok = -1;                  // -1 unknown, 0 the cooperative kernel cannot be resident, 1 fine
     DynPlan* steps_plan = nullptr;      // the device-planned launch shape of a handed-over block
     StepsProgress* steps_prog = nullptr;   // where a queued batch of nb_steps stands
