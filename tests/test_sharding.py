@@ -253,23 +253,23 @@ def _worker_x(rank, world, port, ni, eps2, out_q):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("ni,eps2", [(301, 1e-4), (5, 1e-12)])
-def test_xchg_host_logic_world2_gloo(ni, eps2):
+@pytest.mark.parametrize("ni,eps2,world", [(301, 1e-4, 2), (5, 1e-12, 2), (64, 1e-4, 3)])
+def test_xchg_host_logic_world2_gloo(ni, eps2, world):
     """sharding.xchg_connect wires every rank to every peer's window (handles travel by
     all_gather_object, own rank skipped, barrier before the first push) and force_j_sharded_xchg returns
-    the unsharded force on every rank, bit-identical across ranks (rank-order sum)."""
+    the unsharded force on every rank, bit-identical across ranks (rank-order sum); two and three ranks."""
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker_x, args=(r, 2, port, ni, eps2, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker_x, args=(r, world, port, ni, eps2, q)) for r in range(world)]
     for p in procs:
         p.start()
     res = [q.get(timeout=180) for _ in procs]
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    assert sorted(r[0] for r in res) == [0, 1]
+    assert sorted(r[0] for r in res) == list(range(world))
     assert all(r[1] < 1e-12 for r in res), res
     assert all(r[2] for r in res), res
 
@@ -354,21 +354,22 @@ def _worker_step(rank, world, port, steps, out_q):
         dist.destroy_process_group()
 
 
-def test_step_j_sharded_world2_gloo():
+@pytest.mark.parametrize("world", [2, 3])
+def test_step_j_sharded_world2_gloo(world):
     """PAPER.md:41/:49 on the j-sharded layout of PAPER.md:55: 40 block steps (past t = 2^-6, where
     every particle is due at once) with two ranks equal the unsharded oracle integration."""
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker_step, args=(r, 2, port, 40, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker_step, args=(r, world, port, 40, q)) for r in range(world)]
     for p in procs:
         p.start()
     res = [q.get(timeout=180) for _ in procs]
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    assert sorted(r[0] for r in res) == [0, 1]
+    assert sorted(r[0] for r in res) == list(range(world))
     assert all(r[1] for r in res), res                 # block times and sizes identical to the unsharded run
     assert all(r[2] < 1e-11 for r in res), res         # state equal up to the order of the fp64 additions
     assert all(r[3] for r in res), res                 # every particle's time and power-of-two step identical
