@@ -73,6 +73,9 @@ def parse():
     ap.add_argument("--steps-bound", type=float, default=-1.0,
                     help="with --blockstep: largest N_i x N the persistent kernel of nb_steps takes itself")
     ap.add_argument("--detail", action="store_true", help="with --blockstep: add the per-step sizes and device times")
+    ap.add_argument("--scaling", type=int, default=0, metavar="LOG2MAX",
+                    help="the direct-code curve of the paper's Fig. 2: one all-active force evaluation for "
+                         "N = 2^10 ... 2^LOG2MAX (23: ~2 minutes)")
     ap.add_argument("--fewi", action="store_true",
                     help="instead of the default line: the force call for a handful of active particles "
                          "(N_i = 1..64 of config 3, N = 2^20), nb_force and nb_force_fused, against the HBM roofline")
@@ -962,10 +965,65 @@ def run_kick(args):
     return 0
 
 
+def run_scaling(args):
+    """The direct-code curve of the paper's Fig. 2 (wall-clock time as a function of the
+    number of particles, 10^3 to 10^7, one GPU) on one B200: one all-active force evaluation -- predictor
+    + pair kernel + reduction -- of a Plummer sphere of N = 2^10 ... 2^log2max particles."""
+    import numpy as np
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    import nbgen
+    import paper_1409_5474_b200 as nbm
+    from paper_1409_5474_b200 import binding as nb
+    dev = torch.device("cuda", 0)
+    rows = []
+    for lg in range(10, args.scaling + 1):
+        n = 1 << lg
+        m, x, v = nbgen.plummer(n, nbgen.SEED0 + 40 + lg)
+        eps2 = (4.0 / n) ** 2
+        with nbm.Context(n) as ctx:
+            ctx.set_j(m, x, v)
+            il = torch.arange(n, dtype=torch.int32, device=dev)
+            acc = torch.empty((3, n), dtype=torch.float64, device=dev)
+            jrk = torch.empty((3, n), dtype=torch.float64, device=dev)
+            pot = torch.empty((n,), dtype=torch.float64, device=dev)
+
+            def call():
+                nb.nb_predict(ctx.h, 0.0)
+                nb.nb_force(ctx.h, il, n, eps2, acc, jrk, pot)
+            pairs = float(n) * n
+            reps = 1 if pairs > 2e13 else (3 if pairs > 1e12 else (20 if pairs > 1e10 else 200))
+            for _ in range(1 if pairs > 2e13 else 3):
+                call()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ctx.sync()
+            e0.record()
+            for _ in range(reps):
+                call()
+            e1.record()
+            ctx.sync()
+            ms = e0.elapsed_time(e1) / reps
+            assert bool(torch.isfinite(pot).all())
+            rows.append({"n": n, "ms_per_evaluation": ms, "interactions_per_s": pairs / (ms * 1e-3),
+                         "frac_fp32_peak": pairs / (ms * 1e-3) / 1.2408e12, "evaluations_timed": reps})
+    top = rows[-1]
+    line = {"metric": "interactions/s", "value": top["interactions_per_s"], "unit": "interactions/s", "n_gpus": 1,
+            "steps": top["evaluations_timed"], "warmup": 3, "ms_per_step": top["ms_per_evaluation"],
+            "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "fig2_direct_code_all_active_N_2^10_to_2^%d" % args.scaling,
+                       "step": "nb_predict + nb_force on all N particles (one full force evaluation)"},
+            "rows": rows}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.scaling > 0:
+        return run_scaling(args)
     if args.kick:
         return run_kick(args)
     if args.fewi:

@@ -143,9 +143,15 @@ Layout layout(int64_t n_max, int64_t ni_max)
     L.tileflag = off; off += up((size_t)(ntiles + 31) / 32 * 4);
     L.flag_list = off; off += up((size_t)NB_MAX_FLAGGED * 4);
     L.flag_stage = off; off += up((size_t)4 * NB_MAX_FLAGGED * 4);    // (index, value) pairs of one nb_set_flags
-    // partial sums: S * 7 * ni_pad doubles.  S = 1 needs 56 B per i; small i-sets want many splits.
-    // 4x leaves the remainder segment of an all-active call room for ~16 j-subsets (a full last wave)
-    L.part_bytes = (size_t)NOUT * sizeof(double) * (size_t)ni_pad * 4;
+    // partial sums: S * 7 * ni_pad doubles.  S = 1 needs 56 B per i; what is split is at most one wave
+    // of i-tiles (the remainder segment, or a call that does not fill the chip once): room for 16
+    // j-subsets of up to 640 i-tiles (160 SMs x 4 CTAs), so that such a call can fill whole waves
+    // (with 4 x ni_pad an all-active call of 131072 particles was held to 4 subsets: 0.66 of the peak)
+    {
+        const size_t wave = (size_t)640 * ITILE;
+        const size_t split_part = (size_t)ni_pad < wave ? (size_t)ni_pad : wave;
+        L.part_bytes = (size_t)NOUT * sizeof(double) * ((size_t)ni_pad + 15 * split_part);
+    }
     if (L.part_bytes < ((size_t)32 << 20)) L.part_bytes = (size_t)32 << 20;
     L.part = off; off += up(L.part_bytes);
     L.err = off; off += up(2 * sizeof(int));           // error latch, reduction ticket
