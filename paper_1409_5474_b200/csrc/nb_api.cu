@@ -290,8 +290,12 @@ int choose_splits_scan(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad
         const int64_t ctas = (int64_t)n_itiles * s;
         const int64_t waves = (ctas + resident - 1) / resident;
         const int64_t per = (ntiles + s - 1) / s;
-        // each CTA also pays a fixed cost of about two tiles (gather, pipeline fill, partial store)
-        const double eff = (double)n_itiles * ntiles / ((double)waves * resident * (per + 2));
+        // each CTA also pays a fixed cost of about two tiles (gather, pipeline fill, partial store); and
+        // the SMs do not all run at one speed, so a call of few waves ends with its slowest SM while many
+        // short CTAs balance (measured at N = 2^20, N_i = 151552: 1 / 2 / 4 / 6 / 12 / 23 waves of equal
+        // CTAs: 0.759 / 0.770 / 0.776 / 0.778 / 0.780 / 0.781 of the peak)
+        const double eff = (double)n_itiles * ntiles / ((double)waves * resident * (per + 2)) *
+                           (1.0 - 0.028 / pow((double)waves, 1.25));
         if (eff > best_eff * 1.004) {   // prefer fewer splits unless better by more than noise
             best_eff = eff;
             best = (int)s;
@@ -359,7 +363,8 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // the i-tiles are cut in two segments.  A = the largest multiple of the resident CTA
     // count, one j-subset each (whole waves of equal CTAs); B = the rest, whose j is split in S
     // subsets so that its CTAs fill the chip once more instead of leaving a ragged last wave.
-    int tiles_a = (c->tune_splits > 0) ? 0 : (n_itiles / resident) * resident;
+    // (fewer than four whole waves are better cut finer as well: see choose_splits)
+    int tiles_a = (c->tune_splits > 0 || n_itiles / resident < 4) ? 0 : (n_itiles / resident) * resident;
     int tiles_b = n_itiles - tiles_a;
     int splits_a = tiles_a > 0 ? 1 : 0, splits_b = 0;
     const int64_t pad_a = (int64_t)tiles_a * itile, pad_b = (int64_t)tiles_b * itile;

@@ -191,11 +191,12 @@ def test_few_active_i_share_threads(nbmod, ni):
 
 
 def test_whole_wave_segment_plus_remainder(nbmod):
-    """More i-tiles than resident CTAs: the dispatcher runs whole waves with one j-subset and the
-    remainder with a split j (two pair-kernel launches, one reduction).  Duplicates keep N small."""
+    """Four waves of i-tiles and more: the dispatcher runs whole waves with one j-subset and the
+    remainder with a split j (two pair-kernel launches, one reduction); below four waves the whole call
+    is split.  Duplicates keep N small."""
     c = _random_case(3000, 92, eps2=2.0 ** -18)
     c.flags[[7, 2999]] = 1
-    ni = 148 * 4 * 256 + 1234                                     # > 592 full i-tiles + a ragged one
+    ni = 4 * 148 * 4 * 256 + 1234                                 # > 4 x 592 full i-tiles + a ragged one
     il = (nbgen.permutation(93, ni) % c.n).astype(np.int32)
     got, info = _gpu_force(nbmod, c, 0.1, il)
     # whether 3 or 4 CTAs are resident per SM, a whole-wave segment and a split remainder exist
