@@ -1092,7 +1092,8 @@ int nb_force6(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double*
     // j split in subsets while the i-tiles alone do not fill the chip; 10 sums per i
     const int resident = c->sm_count * c->blocks_per_sm6;
     a.splits = 1;
-    if (a.ntiles > 0 && a.n_itiles < resident)
+    // (also for a few waves of i-tiles, whose ragged last wave and slowest SM would set the time: choose_splits)
+    if (a.ntiles > 0 && a.n_itiles < 4 * resident)
         a.splits = choose_splits(c, a.n_itiles, a.ntiles, a.ni_pad, c->part_bytes * NOUT / 10, resident);
     nb_ctx::Rec* rec = prof_next(c);
     if (rec) cudaEventRecord(rec->e[0], c->stream);
