@@ -290,11 +290,12 @@ int choose_splits_scan(const nb_ctx* c, int n_itiles, int ntiles, int64_t ni_pad
         const int64_t ctas = (int64_t)n_itiles * s;
         const int64_t waves = (ctas + resident - 1) / resident;
         const int64_t per = (ntiles + s - 1) / s;
-        // each CTA also pays a fixed cost of about two tiles (gather, pipeline fill, partial store); and
+        // each CTA also pays a fixed cost of about half a tile (gather, pipeline fill, partial store; fitted:
+        // with 2 tiles config 2 ran at 0.755, with 0.5 at 0.769, mean over a 114-point (N, N_i) sweep +0.5 %); and
         // the SMs do not all run at one speed, so a call of few waves ends with its slowest SM while many
         // short CTAs balance (measured at N = 2^20, N_i = 151552: 1 / 2 / 4 / 6 / 12 / 23 waves of equal
         // CTAs: 0.759 / 0.770 / 0.776 / 0.778 / 0.780 / 0.781 of the peak)
-        const double eff = (double)n_itiles * ntiles / ((double)waves * resident * (per + 2)) *
+        const double eff = (double)n_itiles * ntiles / ((double)waves * resident * (per + 0.5)) *
                            (1.0 - 0.028 / pow((double)waves, 1.25));
         if (eff > best_eff * 1.004) {   // prefer fewer splits unless better by more than noise
             best_eff = eff;
