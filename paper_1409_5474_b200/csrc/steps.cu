@@ -472,7 +472,7 @@ __device__ __forceinline__ bool plan_block(const StepsArgs& P, DynPlan* plan, Fo
         const long long items = (long long)n_itiles * sw;
         const long long waves = (items + resident - 1) / resident;
         const long long per = (fa.ntiles + sw - 1) / sw;
-        const double eff = (double)n_itiles * fa.ntiles / ((double)waves * resident * (double)(per + 2));
+        const double eff = (double)n_itiles * fa.ntiles / ((double)waves * resident * ((double)per + 0.5));
         // (no term for the number of waves here, unlike choose_splits: the resident CTAs of force_dyn_kernel
         // draw their items from a counter, which balances the SMs by itself)
         if (eff > best * 1.004) {
