@@ -136,7 +136,7 @@ int nb_get_predicted(nb_ctx* c, int64_t first, int64_t count, double* out);
  *     jrk_i = sum m_j ( w s^-3/2 - 3 (r.w) r s^-5/2 )             (s == 0 contributes nothing, R6)
  * Outputs, DEVICE fp64, in i_list order: acc[0..ni) = ax, acc[ni..2ni) = ay, acc[2ni..3ni) = az;
  * jrk likewise; pot[0..ni).  Precision: position differences carry >= 48 bits, pair terms are
- * fp32, sums of at most 64 terms are fp32 and everything above them fp64 (DESIGN.md
+ * fp32, sums of at most 128 terms are fp32 and everything above them fp64 (DESIGN.md
  * section 7.2); results agree with exact summation to <= 1e-5 (acc, pot) and <= 1e-4 (jerk) relative
  * per particle, for ANY eps2 >= 0: the self pair is excluded by index before any fp32 sum, so small
  * softenings (m_i/eps far above |pot_i|) cost no accuracy.  Input limits (R14): every pair

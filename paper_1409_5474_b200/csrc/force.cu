@@ -195,6 +195,13 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
                     if ((unsigned)q < (unsigned)TJ && ((q >> 2) & (jl - 1)) == jlane) flush<1, JERK>(A[u], D[DSM ? 0 : u]);
                 }
             }
+            if (!FEW && NB_FLUSH_TILES > 1 && (MODE == 1 || (MODE == 0 && !GUARD))) {
+                // sums run over NB_FLUSH_TILES tiles: the tile with the own index must start empty
+#pragma unroll
+                for (int u = 0; u < IPT; ++u)
+                    if ((unsigned)(sidx[u * FORCE_THREADS] - t * TJ) < (unsigned)TJ)
+                        flush<FORCE_THREADS, JERK>(A[u], sd + u * NOUT * FORCE_THREADS);
+            }
             if (FEW) {
 #pragma unroll 2
                 for (int k = 0; k < nq; ++k) {
@@ -237,9 +244,9 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
                 }
             }
         }
-        // fp32 sums stay short (R17: 64 terms per lane) before they move to fp64: a thread
-        // adds 64 / jl terms per lane and tile
-        if (!FEW || ((t - t0) & (jl - 1)) == jl - 1 || t == t1 - 1) {
+        // fp32 sums stay short before they move to fp64: a thread adds 64 / jl terms per lane and tile; the
+        // all-i kernel flushes every NB_FLUSH_TILES tiles (128 terms), the few-i kernel every jl tiles (64)
+        if ((!FEW && ((t - t0) & (NB_FLUSH_TILES - 1)) == NB_FLUSH_TILES - 1) || (FEW && ((t - t0) & (jl - 1)) == jl - 1) || t == t1 - 1) {
 #pragma unroll
             for (int u = 0; u < IPT; ++u) {
                 if (DSM) flush<FORCE_THREADS, JERK>(A[u], sd + u * NOUT * FORCE_THREADS);

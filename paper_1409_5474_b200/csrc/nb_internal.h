@@ -25,6 +25,13 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 #ifndef NB_MINB
 #define NB_MINB 3
 #endif
+#ifndef NB_FLUSH_TILES
+#define NB_FLUSH_TILES 2           // all-i kernel: tiles per fp32 run before the sums move to fp64 (power of two):
+                                   // 128 terms per lane sum.  Measured at config 3's headline call, 1 / 2 / 4 tiles: 0.778 /
+                                   // 0.787 / 0.789 of the FP32 peak; worst errors over the five configs (tolerances 1e-5,
+                                   // 1e-4, 1e-5): acc 9.8e-7 / 1.5e-6 / 3.0e-6, jerk 7.2e-6 / 8.4e-6 / 1.3e-5, pot
+                                   // 7.7e-7 / 1.9e-6 / 4.0e-6
+#endif
 #ifndef NB_MINB_FEW
 #define NB_MINB_FEW 3
 #endif
