@@ -5,6 +5,7 @@
 #include <string.h>
 #include <vector>
 
+#include <cstdlib>
 #include "nb_internal.h"
 #include "xchg.h"
 
@@ -150,7 +151,7 @@ Layout layout(int64_t n_max, int64_t ni_max)
     {
         const size_t wave = (size_t)640 * ITILE;
         const size_t split_part = (size_t)ni_pad < wave ? (size_t)ni_pad : wave;
-        L.part_bytes = (size_t)NOUT * sizeof(double) * ((size_t)ni_pad + 15 * split_part);
+        L.part_bytes = (size_t)NOUT * sizeof(double) * ((size_t)2 * ni_pad + 15 * split_part);   // 2: the whole waves, two subsets
     }
     if (L.part_bytes < ((size_t)32 << 20)) L.part_bytes = (size_t)32 << 20;
     L.part = off; off += up(L.part_bytes);
@@ -367,11 +368,17 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // (fewer than four whole waves are better cut finer as well: see choose_splits)
     int tiles_a = (c->tune_splits > 0 || n_itiles / resident < 4) ? 0 : (n_itiles / resident) * resident;
     int tiles_b = n_itiles - tiles_a;
-    int splits_a = tiles_a > 0 ? 1 : 0, splits_b = 0;
     const int64_t pad_a = (int64_t)tiles_a * itile, pad_b = (int64_t)tiles_b * itile;
-    double* part_b = c->part + (size_t)NOUT * pad_a;
+    // A's whole waves run with two j-subsets when the partial-sum buffer has the room (it has, as nb_create
+    // sizes it): twice as many, half as long CTAs balance the SMs better (measured on the headline call:
+    // 1 / 2 / 4 subsets: 0.7880 / 0.7897 / 0.7904 of the peak)
+    int splits_a = tiles_a > 0 ? 1 : 0, splits_b = 0;
+    if (tiles_a > 0 && a.ntiles >= 64 && !f64 &&
+        (size_t)NOUT * sizeof(double) * ((size_t)2 * pad_a + (size_t)16 * pad_b) <= c->part_bytes)
+        splits_a = 2;
+    double* part_b = c->part + (size_t)NOUT * pad_a * splits_a;
     if (a.ntiles > 0 && tiles_b > 0) {
-        const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a;
+        const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a * splits_a;
         splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left, resident);
     }
     if (a.ntiles == 0) splits_a = splits_b = 0;   // n == 0: the reduction of zero partials writes zeros
@@ -473,7 +480,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             a.k0 = 0;
             a.n_itiles = tiles_a;
             a.ni_pad = (int)pad_a;
-            a.splits = 1;
+            a.splits = splits_a;
             a.part = c->part;
             if ((f64 ? launch_force64(a, kmode, c->stream)
                      : launch_force(a, r, kmode, mode, acc, jrk, pot, c->stream)) != cudaSuccess)
