@@ -169,7 +169,8 @@ __global__ void __launch_bounds__(FORCE_THREADS, 2) force6_kernel(Force6Args P)
                 pair6(I[u], A[u], hi, eps2, self[u], p + 2, ifl[u]);
             }
         }
-        // fp32 sums over one tile (64 terms per lane), then fp64
+        // fp32 sums over NB_FLUSH_TILES tiles (128 terms per lane), then fp64 (as force.cu's all-i kernel)
+        if (((t - t0) & (NB_FLUSH_TILES - 1)) == NB_FLUSH_TILES - 1 || t == t1 - 1)
 #pragma unroll
         for (int u = 0; u < IPT; ++u) {
             double* d = sd + u * NOUT6 * FORCE_THREADS;
