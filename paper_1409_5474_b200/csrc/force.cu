@@ -54,6 +54,7 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
     constexpr int KT = tiles_per_stage(FEW);
     constexpr int STAGE_BYTES = KT * TILE_BYTES;
     constexpr bool JERK = (MODE != 2);
+    constexpr int FT = (MODE == 2) ? 1 : NB_FLUSH_TILES;     // tiles per fp32 run of the all-i kernel (nb_internal.h)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG * STAGE_BYTES);
@@ -195,8 +196,8 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
                     if ((unsigned)q < (unsigned)TJ && ((q >> 2) & (jl - 1)) == jlane) flush<1, JERK>(A[u], D[DSM ? 0 : u]);
                 }
             }
-            if (!FEW && NB_FLUSH_TILES > 1 && (MODE == 1 || (MODE == 0 && !GUARD))) {
-                // sums run over NB_FLUSH_TILES tiles: the tile with the own index must start empty
+            if (!FEW && FT > 1 && (MODE == 1 || (MODE == 0 && !GUARD))) {
+                // sums run over FT tiles: the tile with the own index must start empty
 #pragma unroll
                 for (int u = 0; u < IPT; ++u)
                     if ((unsigned)(sidx[u * FORCE_THREADS] - t * TJ) < (unsigned)TJ)
@@ -245,8 +246,8 @@ __device__ __forceinline__ void force_body(const ForceArgs& P, const ReduceArgs&
             }
         }
         // fp32 sums stay short before they move to fp64: a thread adds 64 / jl terms per lane and tile; the
-        // all-i kernel flushes every NB_FLUSH_TILES tiles (128 terms), the few-i kernel every jl tiles (64)
-        if ((!FEW && ((t - t0) & (NB_FLUSH_TILES - 1)) == NB_FLUSH_TILES - 1) || (FEW && ((t - t0) & (jl - 1)) == jl - 1) || t == t1 - 1) {
+        // all-i kernel flushes every FT tiles (128 terms), the few-i kernel every jl tiles (64)
+        if ((!FEW && ((t - t0) & (FT - 1)) == FT - 1) || (FEW && ((t - t0) & (jl - 1)) == jl - 1) || t == t1 - 1) {
 #pragma unroll
             for (int u = 0; u < IPT; ++u) {
                 if (DSM) flush<FORCE_THREADS, JERK>(A[u], sd + u * NOUT * FORCE_THREADS);
