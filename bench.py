@@ -255,11 +255,11 @@ def measured_peaks():
 # DRAM bytes per launch cannot be measured inside a timed run (they need ncu's counters), so `traffic`
 # is quoted from the committed `ncu --set full` captures of this same command, per launch:
 # force_kernel, default workload: a call is two launches (whole waves, then the remainder with j split).
-# profiles/r2c_cfg3_first.md: the whole-wave launch (3552 CTAs, 87 % of the call's time) moved 57.63 MB
-# read + 36.84 MB written = 94.5 MB -- the 46 MB pack once plus the 51 MB of partial sums it writes.
-# profiles/r2b_cfg3_second.md: the remainder launch (7072 CTAs), captured alone: 56.73 MB read + 74.69 MB
-# written = 131.4 MB (the pack once more, and most of its 101 MB of partial sums).  Sum over the call:
-FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": 94.48e6 + 131.42e6}
+# profiles/r2c_cfg3_first.md: the whole-wave launch (7104 CTAs, 87 % of the call's time) moved 68.28 MB
+# read + 81.39 MB written = 149.7 MB -- the 46 MB pack plus the 102 MB of partial sums it writes (two
+# j-subsets).  profiles/r2b_cfg3_second.md: the remainder launch (7072 CTAs), captured alone: 56.73 MB
+# read + 74.69 MB written = 131.4 MB (the pack once more, and most of its 101 MB of partial sums).  Sum:
+FORCE_KERNEL_DRAM_TRAFFIC = {"cfg3": 149.67e6 + 131.42e6}
 # predict_kernel (profiles/r2_predict_full.md, profiles/r2_cfg3_full.md), by particle count:
 # N = 2^22 + 11: 474.04 MB read (= 113 B x N exactly) + 150.20 MB written of the 184.5 MB the kernel
 # stores (the rest was still in the L2 when the kernel ended) = 624.2 MB; N = 2^20: 118.5 + 18.3 MB.
