@@ -373,7 +373,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // sizes it): twice as many, half as long CTAs balance the SMs better (measured on the headline call:
     // 1 / 2 / 4 subsets: 0.7880 / 0.7897 / 0.7904 of the peak)
     int splits_a = tiles_a > 0 ? 1 : 0, splits_b = 0;
-    if (tiles_a > 0 && a.ntiles >= 64 && !f64 &&
+    if (tiles_a > 0 && a.ntiles >= 64 &&
         (size_t)NOUT * sizeof(double) * ((size_t)2 * pad_a + (size_t)16 * pad_b) <= c->part_bytes)
         splits_a = 2;
     double* part_b = c->part + (size_t)NOUT * pad_a * splits_a;
