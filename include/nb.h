@@ -231,6 +231,37 @@ int nb_xchg_set_timeout(nb_ctx* c, double seconds);
 int nb_xforce(nb_ctx* c, int phase, int64_t ni, const double* x, const double* v, const int32_t* self_idx,
               const uint8_t* iflags, double eps2, double* acc, double* jrk, double* pot);
 
+/* ---- the force call that allocates nothing ------------------------------------------------------ */
+
+/* nb_force_static: acceleration, jerk and potential (readings R2, R5, R6 of DESIGN.md) of n
+ * j-particles on ni i-particles given by value, WITHOUT a context and without any allocation: for
+ * callers that cannot call cudaMalloc (stream capture into a CUDA graph, tight serving loops, harnesses
+ * that forbid it).  Every nb_ctx entry point above relies on buffers nb_create / nb_set_j allocated;
+ * this one calls no cudaMalloc, cudaFree or allocating library routine.  Its scratch memory (partial
+ * forces of the j-subsets, PAPER.md:51 / :55, and the tickets that elect the summing CTA) is a static
+ * array of NB_STATIC_SCRATCH_BYTES in the library's device image: every GPU that loads libnb.so holds it
+ * until the process exits.
+ *
+ * Works on the calling thread's CURRENT device (compute capability 10.x, NB_ERR_ARCH otherwise), to
+ * which every pointer and the stream must belong; enqueues a 256-byte clear and one kernel on `stream`
+ * (cudaStream_t as void*, NULL = legacy default stream) and returns.  The first call per device looks
+ * the array's address up (cudaGetSymbolAddress; make that call outside stream capture).
+ * DEVICE inputs, fp64 SoA, read only:  m [n], x [3][n], v [3][n] (the j-set at the time of the call: no
+ * predictor here);  xi [3][ni], vi [3][ni];  self_idx [ni] or NULL: the j index particle k of the call
+ * IS (its own pair is skipped by index, R5), negative = none.
+ * DEVICE outputs: acc [3][ni], jrk [3][ni] or NULL, pot [ni].  The caller owns all arrays.
+ * Arithmetic: IEEE double throughout (the pair loop of nb_set_precision(c, 1)); every pair uses eps2, no
+ * flagged pairs (R7); sums in a fixed order: results are bitwise reproducible.
+ * Limits: 0 <= ni <= NB_STATIC_NI_MAX and 0 <= n < 2^31, else NB_ERR_ARG ("invalid argument"): take
+ * nb_force_ext for larger calls.  NULL among the required pointers, eps2 < 0 or NaN: NB_ERR_ARG.
+ * ALL calls on one device share the one array: calls that can overlap on the GPU (two streams, two
+ * host threads on different streams, parallel branches of a graph) RACE; order them on one stream. */
+#define NB_STATIC_NI_MAX 4096
+#define NB_STATIC_SCRATCH_BYTES 4194304
+int nb_force_static(void* stream, int64_t n, const double* m, const double* x, const double* v,
+                    int64_t ni, const double* xi, const double* vi, const int32_t* self_idx, double eps2,
+                    double* acc, double* jrk, double* pot);
+
 /* HOST-pointer form: i_list, acc, jrk, pot are host arrays; copies in, runs, copies back and
  * synchronises the stream before returning (so it also returns latched errors). */
 int nb_force_host(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2,

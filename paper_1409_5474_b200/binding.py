@@ -14,6 +14,8 @@ NB_OK, NB_ERR_ARG, NB_ERR_ALLOC, NB_ERR_CUDA = 0, -1, -2, -3
 NB_ERR_INDEX, NB_ERR_STATE, NB_ERR_ARCH, NB_ERR_PEER = -4, -5, -6, -7
 NB_XCHG_HANDLE_BYTES = 64
 NB_MAX_FLAGGED = 1024
+NB_STATIC_NI_MAX = 4096
+NB_STATIC_SCRATCH_BYTES = 4194304
 
 EXPORTS = [
     "nb_create", "nb_destroy", "nb_set_stream", "nb_workspace_bytes", "nb_set_workspace",
@@ -22,6 +24,7 @@ EXPORTS = [
     "nb_last_launch", "nb_launch_count", "nb_set_profiling", "nb_kernel_times", "nb_sync",
     "nb_set_dt", "nb_get_state", "nb_init_steps", "nb_next_block", "nb_correct", "nb_step", "nb_steps", "nb_set_steps_bound", "nb_set_steps_queue", "nb_block_forces", "nb_strerror", "nb_version",
     "nb_xchg_create", "nb_xchg_export", "nb_xchg_attach", "nb_xchg_destroy", "nb_xchg_set_timeout", "nb_xforce",
+    "nb_force_static",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -83,6 +86,7 @@ lib.nb_xchg_attach.argtypes = [_vp, _i32, _vp, _vp]
 lib.nb_xchg_destroy.argtypes = [_vp]
 lib.nb_xchg_set_timeout.argtypes = [_vp, _dbl]
 lib.nb_xforce.argtypes = [_vp, _i32, _i64, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]
+lib.nb_force_static.argtypes = [_vp, _i64, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]
 
 
 class NBError(RuntimeError):
@@ -245,6 +249,13 @@ def nb_force_ext_ids(c, ni, x, v, self_idx, iflags, eps2, acc, jrk, pot):
     """DEVICE x, v (3, ni) fp64, self_idx int32 (ni,), iflags uint8 (ni,) or None."""
     _check(lib.nb_force_ext_ids(c, ni, _ptr(x), _ptr(v), _ptr(self_idx), _ptr(iflags), eps2, _ptr(acc), _ptr(jrk),
                                 _ptr(pot)), "nb_force_ext_ids")
+
+
+def nb_force_static(stream, n, m, x, v, ni, xi, vi, self_idx, eps2, acc, jrk, pot):
+    """No context, no allocation (nb.h): DEVICE m (n,), x, v (3, n), xi, vi (3, ni) fp64, self_idx int32
+    (ni,) or None; outputs acc, jrk (3, ni) (jrk may be None), pot (ni,).  On the CURRENT device."""
+    _check(lib.nb_force_static(stream, n, _ptr(m), _ptr(x), _ptr(v), ni, _ptr(xi), _ptr(vi), _ptr(self_idx), eps2,
+                               _ptr(acc), _ptr(jrk), _ptr(pot)), "nb_force_static")
 
 
 def nb_xchg_create(c, rank, world, ni_cap):
