@@ -79,6 +79,9 @@ def parse():
     ap.add_argument("--fewi", action="store_true",
                     help="instead of the default line: the force call for a handful of active particles "
                          "(N_i = 1..64 of config 3, N = 2^20), nb_force and nb_force_fused, against the HBM roofline")
+    ap.add_argument("--midsize", action="store_true",
+                    help="instead of the default line: nb_force for N_i = 256 ... 4128 active particles (full i-tiles, "
+                         "and i-tiles plus a few) at N = 2^16, 2^17, 2^20, against the FP32 roofline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target duration of the cpu_baseline sample")
     return ap.parse_args()
@@ -719,6 +722,60 @@ def run_fewi(args):
     return 0
 
 
+def run_midsize(args):
+    """PAPER.md:51 between the two regimes it names: some hundreds to thousands of active particles (the
+    blocks of a block-time-step code at N ~ 1e5 ... 1e6).  One nb_force call, by index, on a Plummer set:
+    N_i at multiples of the 256-slot i-tile and a few particles above them, where the last tile would be
+    mostly padding and goes to the few-i kernel as a segment of its own."""
+    import numpy as np
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    import nbgen
+    import paper_1409_5474_b200 as nbm
+    dev = torch.device("cuda", 0)
+    peaks = measured_peaks()
+    props = torch.cuda.get_device_properties(dev)
+    peak = props.multi_processor_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / FLOP_PER_INTERACTION
+    rows = []
+    for n in (1 << 16, 1 << 17, 1 << 20):
+        m, x, v = nbgen.plummer(n, 7)
+        zero = np.zeros((3, n))
+        with nbm.Context(n, 8192) as ctx:
+            ctx.set_j(m, x, v, zero, zero, np.zeros(n))
+            ctx.predict(0.0)
+            perm = torch.from_numpy(nbgen.permutation(8, n).astype(np.int32)).to(dev)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for ni in (256, 257, 288, 320, 384, 512, 520, 640, 768, 800, 1024, 1056, 2048, 2080, 3100, 4096, 4128):
+                il = perm[:ni].contiguous()
+                reps = max(5, min(300, int(1e11 / (ni * n))))
+                for _ in range(max(args.warmup, 3)):
+                    ctx.force(il, 2.0 ** -20)
+                ctx.sync()
+                e0.record()
+                for _ in range(reps):
+                    ctx.force(il, 2.0 ** -20)
+                e1.record()
+                ctx.sync()
+                us = e0.elapsed_time(e1) / reps * 1e3
+                info = ctx.last_launch()
+                rows.append({"n_j": n, "n_i": ni, "us_per_call": us, "interactions_per_s": ni * n / us * 1e6,
+                             "frac_fp32_peak": ni * n / us * 1e6 / peak, "kernels": int(info["kernels"]),
+                             "ctas": int(info["ctas"])})
+    best = max(rows, key=lambda r: r["frac_fp32_peak"])
+    line = {"metric": "interactions/s", "value": best["interactions_per_s"], "unit": "interactions/s", "n_gpus": 1,
+            "steps": "5..300 calls per row", "warmup": max(args.warmup, 3), "higher_is_better": True, "dtype": "f32",
+            "data": "synthetic", "config": {"workload": "plummer_midsize_calls", "value_is": "the best row",
+                                            "l2": "no flush: back-to-back calls, the packed j-set (44 B per particle) stays in the L2"},
+            "roofline": {"bound": "alu", "unit": "interactions/s", "peak": peak, "achieved": best["interactions_per_s"],
+                         "frac": best["frac_fp32_peak"], "traffic": None,
+                         "peak_source": "derived: %d SMs x 128 FP32 lanes x 2 x %.0f MHz / 60 flop" % (
+                             props.multi_processor_count, peaks["sm_max_mhz"])},
+            "rows": rows}
+    print(json.dumps(line))
+    return 0
+
+
 def run_predict(args):
     """The Hermite predictor (a1) against the HBM roofline, where its working set cannot sit in the L2:
     (a) config 5's N = 2^22 + 11 (470 MB of j-store, 185 MB of packed records), (b) config 3's
@@ -1028,6 +1085,8 @@ def main():
         return run_kick(args)
     if args.fewi:
         return run_fewi(args)
+    if args.midsize:
+        return run_midsize(args)
     if args.predict:
         return run_predict(args)
     if args.blockstep > 0:

@@ -368,7 +368,35 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // (fewer than four whole waves are better cut finer as well: see choose_splits)
     int tiles_a = (c->tune_splits > 0 || n_itiles / resident < 4) ? 0 : (n_itiles / resident) * resident;
     int tiles_b = n_itiles - tiles_a;
-    const int64_t pad_a = (int64_t)tiles_a * itile, pad_b = (int64_t)tiles_b * itile;
+    // Mid-size calls whose last i-tile is at most half full (N_i = 256 q + rem, rem <= 128): that tile would
+    // cost a full pass over j for 256 slots.  It is taken out as a segment of its own for the few-i kernel
+    // (2^jsh threads per i: 128 .. 8 slots per CTA), A = the q full tiles with j split by choose_splits --
+    // when a 256-slot pass over j costs clearly more than the smaller one plus a launch (measured at
+    // N = 131072: N_i = 288 / 320 went from 100 us to 74 / 82 us, at N = 2^20: N_i = 257 from 591 us to 325 us;
+    // at N = 32768 a launch costs what the pass costs, so small j-sets keep one segment).  Only up to 4096
+    // particles, where a warp per i sums the partials: the thread-per-i reduction of larger calls would add
+    // the tail's hundreds of j-subsets one dependent load at a time (measured: +130 us at N_i = 4128).
+    int jsh_b = jsh, itile_b = itile, resident_b = resident;
+    bool tail = false;
+    if (!f64 && !mode && jsh == 0 && tiles_a == 0 && c->tune_splits == 0 && NB_TAIL_SEGMENT && ni > ITILE && ni <= 4096 &&
+        a.ntiles > 0) {
+        const int rem = (int)(ni % ITILE);
+        if (rem >= 1 && rem <= ITILE / 2) {
+            int jb = 0;
+            while (jb < JSH_MAX && (ITILE >> (jb + 1)) >= rem) ++jb;
+            const int ib = ITILE >> jb;
+            const double saved_s = (double)n_launch * ((double)ITILE - 1.3 * ib) / 0.9e12;
+            if (saved_s >= 15e-6) {
+                tail = true;
+                jsh_b = jb;
+                itile_b = ib;
+                tiles_a = n_itiles - 1;
+                tiles_b = 1;
+                resident_b = c->sm_count * c->blocks_per_sm[2 + (guard ? 1 : 0)];
+            }
+        }
+    }
+    const int64_t pad_a = (int64_t)tiles_a * itile, pad_b = (int64_t)tiles_b * itile_b;
     // A's whole waves run with two j-subsets when the partial-sum buffer has the room (it has, as nb_create
     // sizes it): twice as many, half as long CTAs balance the SMs better (measured on the headline call:
     // 1 / 2 / 4 subsets: 0.7880 / 0.7897 / 0.7904 of the peak)
@@ -376,10 +404,16 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     if (tiles_a > 0 && a.ntiles >= 64 &&
         (size_t)NOUT * sizeof(double) * ((size_t)2 * pad_a + (size_t)16 * pad_b) <= c->part_bytes)
         splits_a = 2;
+    if (tail) {
+        // room for the tail's partials first: at most two waves of its CTAs
+        const int64_t sb_max = a.ntiles < 2 * resident_b ? a.ntiles : 2 * resident_b;
+        const size_t keep = (size_t)NOUT * sizeof(double) * (size_t)pad_b * (size_t)sb_max;
+        splits_a = choose_splits(c, tiles_a, a.ntiles, pad_a, c->part_bytes - keep, resident);
+    }
     double* part_b = c->part + (size_t)NOUT * pad_a * splits_a;
     if (a.ntiles > 0 && tiles_b > 0) {
         const size_t left = c->part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a * splits_a;
-        splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left, resident);
+        splits_b = choose_splits(c, tiles_b, a.ntiles, pad_b, left, resident_b);
     }
     if (a.ntiles == 0) splits_a = splits_b = 0;   // n == 0: the reduction of zero partials writes zeros
 
@@ -478,6 +512,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
         if (rec) cudaEventRecord(rec->e[0], c->stream);
         if (tiles_a > 0) {
             a.k0 = 0;
+            a.jsh = jsh;
             a.n_itiles = tiles_a;
             a.ni_pad = (int)pad_a;
             a.splits = splits_a;
@@ -489,6 +524,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
         }
         if (tiles_b > 0) {
             a.k0 = (int)pad_a;
+            a.jsh = jsh_b;
             a.n_itiles = tiles_b;
             a.ni_pad = (int)pad_b;
             a.splits = splits_b;

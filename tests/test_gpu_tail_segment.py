@@ -1,0 +1,131 @@
+"""-m gpu: mid-size calls whose last i-tile is at most half full (N_i = 256 q + rem, 1 <= rem <= 128): the
+dispatcher hands that tile to the few-i kernel as a segment of its own (nb_api.cu force_impl, DESIGN.md
+7.3) when the j-set is large enough for a 256-slot pass to cost more than a launch.  Two pair-kernel
+launches of DIFFERENT variants (thread per i; 2 .. 32 threads per i) write two partial buffers that one
+reduction reads.  Checked element by element against the oracle: by index (own pair, flagged pairs, a bad
+index in either segment), by value with ids, acc + pot only, eps2 = 0; and that calls just outside the
+rule (rem = 0, rem > 128, small N) keep one segment."""
+import numpy as np
+import pytest
+
+import nbgen
+import oracle
+from util import check_parity, rel_err_scalar, rel_err_vec
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+N = 160000 + 77           # large enough for every rem <= 128 to take the tail (the rule needs N >= ~150000)
+
+
+@pytest.fixture(scope="module")
+def nbmod():
+    import __graft_entry__ as g
+    g.build()
+    import paper_1409_5474_b200 as nbm
+    return nbm
+
+
+@pytest.fixture(scope="module")
+def world(nbmod):
+    m, x, v = nbgen.plummer(N, 7300)
+    m = m * (0.5 + nbgen.Streams(7301, N).uniform())
+    a, j = nbgen.mean_field(x, v)
+    tj = 0.25 * nbgen.Streams(7302, N).uniform()
+    t = 0.2
+    flags = np.zeros(N, np.uint8)
+    flags[[40, 1100, 90000, N - 3]] = 1
+    xp, vp = oracle.predict(t, x, v, a, j, tj)
+    ctx = nbmod.Context(N, 4200)
+    ctx.set_j(m, x, v, a, j, tj)
+    fl = np.flatnonzero(flags).astype(np.int32)
+    ctx.set_flags(fl, np.ones(len(fl), np.uint8))
+    ctx.predict(t)
+    yield ctx, m, xp, vp, flags
+    ctx.close()
+
+
+def _i_list(ni, seed):
+    il = nbgen.permutation(seed, N)[:ni].astype(np.int32)
+    il[0], il[ni // 2], il[ni - 1], il[ni - 2] = 40, 1100, 90000, N - 3     # flagged ones in both segments
+    return il
+
+
+@pytest.mark.parametrize("ni,eps2", [(256 + 1, 2.0 ** -14), (256 + 8, 0.0), (256 + 40, 2.0 ** -14), (512 + 64, 1e-12),
+                                     (768 + 100, 2.0 ** -14), (1024 + 128, 2.0 ** -14), (2048 + 17, 0.0)])
+def test_tail_segment_by_index(nbmod, world, ni, eps2):
+    ctx, m, xp, vp, flags = world
+    il = _i_list(ni, 7310 + ni)
+    got = [q.cpu().numpy() for q in ctx.force(il, eps2)]
+    info = ctx.last_launch()
+    ctx.sync()
+    assert info["kernels"] == 3                      # full tiles + tail + one reduction
+    check_parity(got, oracle.force(m, xp, vp, il, eps2, flags))
+    again = [q.cpu().numpy() for q in ctx.force(il, eps2)]
+    assert all(np.array_equal(p, q) for p, q in zip(got, again))     # deterministic (R9)
+
+
+def test_tail_segment_by_value_and_kick(nbmod, world):
+    ctx, m, xp, vp, flags = world
+    ni, eps2 = 512 + 30, 2.0 ** -14
+    il = _i_list(ni, 7400)
+    ref = oracle.force(m, xp, vp, il, eps2, flags)
+    got = [q.cpu().numpy() for q in ctx.force_ext_ids(xp[:, il], vp[:, il], il, flags[il], eps2)]
+    assert ctx.last_launch()["kernels"] == 3
+    check_parity(got, ref)
+    # particles from outside the j-set; with jerk, and acc + pot only (the kick)
+    _, xo, vo = nbgen.plummer(ni, 7401)
+    xo, vo = np.ascontiguousarray(xo + 0.3), np.ascontiguousarray(vo)
+    ref = oracle.force(np.concatenate([m, np.zeros(ni)]), np.concatenate([xp, xo], 1), np.concatenate([vp, vo], 1),
+                       np.arange(N, N + ni, dtype=np.int32), eps2)
+    got = [q.cpu().numpy() for q in ctx.force_ext(xo, vo, eps2)]
+    assert ctx.last_launch()["kernels"] == 3
+    check_parity(got, ref)
+    acc, none, pot = ctx.force_ext(xo, None, eps2)
+    assert none is None and ctx.last_launch()["kernels"] == 3
+    assert rel_err_vec(acc.cpu().numpy(), ref[0]).max() <= 1e-5
+    assert rel_err_scalar(pot.cpu().numpy(), ref[2]).max() <= 1e-5
+    ctx.sync()
+
+
+def test_tail_segment_bad_index_in_either_segment(nbmod, world):
+    ctx, m, xp, vp, flags = world
+    nb = nbmod.binding
+    ni, eps2 = 256 + 20, 2.0 ** -14
+    il = _i_list(ni, 7500)
+    il[100], il[256 + 5] = -7, N                       # one in the full tile, one in the tail
+    got = [q.cpu().numpy() for q in ctx.force(il, eps2)]
+    with pytest.raises(nb.NBError) as e:
+        ctx.sync()
+    assert e.value.status == nb.NB_ERR_INDEX
+    bad = np.zeros(ni, bool)
+    bad[[100, 256 + 5]] = True
+    assert np.isnan(got[0][:, bad]).all() and np.isnan(got[2][bad]).all()
+    ok = ~bad
+    ref = oracle.force(m, xp, vp, il[ok], eps2, flags)
+    check_parity([got[0][:, ok], got[1][:, ok], got[2][ok]], ref)
+
+
+def test_calls_outside_the_rule_keep_one_segment(nbmod, world):
+    ctx, m, xp, vp, flags = world
+    for ni in (256, 512, 256 + 129, 1024 + 255, 130, 4096 + 20):
+        ctx.force(_i_list(ni, 7600 + ni), 1e-6)
+        assert ctx.last_launch()["kernels"] == 2, ni
+    ctx.tuning(3, 0)                                   # forced j-split: one segment
+    ctx.force(_i_list(300, 7601), 1e-6)
+    assert ctx.last_launch()["kernels"] == 2
+    ctx.tuning(0, 0)
+    ctx.sync()
+    # a small j-set: a launch costs more than the 256-slot pass
+    n = 5000
+    m2, x2, v2 = nbgen.plummer(n, 7602)
+    z = np.zeros((3, n))
+    with nbmod.Context(n, 512) as small:
+        small.set_j(m2, x2, v2, z, z, np.zeros(n))
+        small.predict(0.0)
+        il = nbgen.permutation(7603, n)[:300].astype(np.int32)
+        got = [q.cpu().numpy() for q in small.force(il, 1e-4)]
+        assert small.last_launch()["kernels"] == 2
+        small.sync()
+    check_parity(got, oracle.force(m2, x2, v2, il, 1e-4))
