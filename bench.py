@@ -80,7 +80,7 @@ def parse():
                     help="instead of the default line: the force call for a handful of active particles "
                          "(N_i = 1..64 of config 3, N = 2^20), nb_force and nb_force_fused, against the HBM roofline")
     ap.add_argument("--midsize", action="store_true",
-                    help="instead of the default line: nb_force for N_i = 256 ... 4128 active particles (full i-tiles, "
+                    help="instead of the default line: nb_force for N_i = 256 ... 16400 active particles (full i-tiles, "
                          "and i-tiles plus a few) at N = 2^16, 2^17, 2^20, against the FP32 roofline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target duration of the cpu_baseline sample")
@@ -741,12 +741,13 @@ def run_midsize(args):
     for n in (1 << 16, 1 << 17, 1 << 20):
         m, x, v = nbgen.plummer(n, 7)
         zero = np.zeros((3, n))
-        with nbm.Context(n, 8192) as ctx:
+        with nbm.Context(n, 16400) as ctx:
             ctx.set_j(m, x, v, zero, zero, np.zeros(n))
             ctx.predict(0.0)
             perm = torch.from_numpy(nbgen.permutation(8, n).astype(np.int32)).to(dev)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            for ni in (256, 257, 288, 320, 384, 512, 520, 640, 768, 800, 1024, 1056, 2048, 2080, 3100, 4096, 4128):
+            for ni in (256, 257, 288, 320, 384, 512, 520, 640, 768, 800, 1024, 1056, 2048, 2080, 3100, 4096, 4128, 8192, 8224,
+                       16384, 16400):
                 il = perm[:ni].contiguous()
                 reps = max(5, min(300, int(1e11 / (ni * n))))
                 for _ in range(max(args.warmup, 3)):

@@ -383,6 +383,18 @@ __global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_DYN_MINB : NB_DYN_MINB
 template <bool WARP>
 __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
 {
+    if (!WARP && R.warp_rows > 0) {
+        // the first CTAs take positions [0, ni - warp_rows) one per thread, the others the rest one per warp
+        const int first = R.ni - R.warp_rows, ctas_a = (first + 127) / 128;
+        if ((int)blockIdx.x >= ctas_a) {
+            const int k = first + ((int)blockIdx.x - ctas_a) * 4 + (int)(threadIdx.x >> 5);
+            if (k < R.ni) reduce_row<true, true>(R, k, threadIdx.x & 31);
+        } else {
+            const int k = blockIdx.x * blockDim.x + threadIdx.x;
+            if (k < first) reduce_row<false>(R, k, threadIdx.x & 31);
+        }
+        return;
+    }
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int k = WARP ? gt / 32 : gt;
     if (k >= R.ni) return;
@@ -531,6 +543,8 @@ cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s)
     const int most = a.splits > a.splits_b ? a.splits : a.splits_b;
     if (!a.atomic_mode && most > 8 && a.ni <= 4096)
         reduce_kernel<true><<<(a.ni + 3) / 4, 128, 0, s>>>(a);
+    else if (a.warp_rows > 0)
+        reduce_kernel<false><<<(a.ni - a.warp_rows + 127) / 128 + (a.warp_rows + 3) / 4, 128, 0, s>>>(a);
     else
         reduce_kernel<false><<<(a.ni + 127) / 128, 128, 0, s>>>(a);
     return cudaGetLastError();

@@ -373,12 +373,13 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // (2^jsh threads per i: 128 .. 8 slots per CTA), A = the q full tiles with j split by choose_splits --
     // when a 256-slot pass over j costs clearly more than the smaller one plus a launch (measured at
     // N = 131072: N_i = 288 / 320 went from 100 us to 74 / 82 us, at N = 2^20: N_i = 257 from 591 us to 325 us;
-    // at N = 32768 a launch costs what the pass costs, so small j-sets keep one segment).  Only up to 4096
-    // particles, where a warp per i sums the partials: the thread-per-i reduction of larger calls would add
-    // the tail's hundreds of j-subsets one dependent load at a time (measured: +130 us at N_i = 4128).
+    // at N = 32768 a launch costs what the pass costs, so small j-sets keep one segment).  Above 4096
+    // particles the reduction is one thread per i, which would add the tail's hundreds of j-subsets one
+    // dependent load at a time (measured: +130 us at N_i = 4128): the tail's positions are then summed by
+    // one warp each (ReduceArgs.warp_rows).  Beyond 16384 particles the tile is < 1.6 % of the call (measured at 16400 and 32800: -0.7 ... +2 %).
     int jsh_b = jsh, itile_b = itile, resident_b = resident;
     bool tail = false;
-    if (!f64 && !mode && jsh == 0 && tiles_a == 0 && c->tune_splits == 0 && NB_TAIL_SEGMENT && ni > ITILE && ni <= 4096 &&
+    if (!f64 && !mode && jsh == 0 && tiles_a == 0 && c->tune_splits == 0 && NB_TAIL_SEGMENT && ni > ITILE && ni <= 16384 &&
         a.ntiles > 0) {
         const int rem = (int)(ni % ITILE);
         if (rem >= 1 && rem <= ITILE / 2) {
@@ -454,6 +455,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
         const int most = splits_a > splits_b ? splits_a : splits_b;
         const bool warp_reduce = !r.atomic_mode && most > 8 && ni <= 4096;
         a.part_i_fastest = r.part_i_fastest = (!f64 && !reduce_here && !warp_reduce) ? 1 : 0;
+        r.warp_rows = (tail && !warp_reduce && splits_b > 8) ? (int)(ni - pad_a) : 0;
     }
     const bool xchg = c->xchg_call >= 0;
     const bool direct = (kmode == 0 || kmode == 1) && !f64 && !mode && c->tune_splits == 0 && ni <= DIRECT_NI_MAX &&

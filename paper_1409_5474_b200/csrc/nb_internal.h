@@ -133,6 +133,8 @@ struct ReduceArgs {
     int xchg_phase;           // ... 0: push, wait and sum inside the reducing CTA; 1: push only
     unsigned long long xchg_limit_ns;   // ... how long to wait for a peer
     int part_i_fastest;       // layout of part / part_b, as in ForceArgs
+    int warp_rows;            // thread-per-i reduction only: the LAST warp_rows positions (a tail segment with hundreds
+                              // of j-subsets) are summed by one warp each instead (0: none)
 };
 
 // kernel launchers (each returns the cudaError of the launch)

@@ -207,7 +207,10 @@ __device__ __forceinline__ void flush(Acc32& A, double* d)
 // unsoftened flagged-flagged pair terms in fp64 straight from the j-store (R7), NaN for a rejected
 // index, store SoA.  WARP: the 32 lanes of a warp stride over the partials (fixed butterfly) -- for
 // the few-i calls, whose many j-subsets would otherwise be summed by one thread; else one thread.
-template <bool WARP>
+// IFAST (with WARP): the partials are laid out [c][subset][i] (part_i_fastest) -- the tail rows of a call
+// whose other rows are summed one per thread; a compile-time choice, so that the in-kernel reductions of
+// the few-i, direct and fused kernels keep their code (a run-time select here cost them 2 - 10 us)
+template <bool WARP, bool IFAST = false>
 __device__ __forceinline__ void reduce_row(const ReduceArgs& R, int k, int lane)
 {
     double o[NOUT];
@@ -234,7 +237,9 @@ __device__ __forceinline__ void reduce_row(const ReduceArgs& R, int k, int lane)
                     const int s = s0 + q * 32 + lane;
 #pragma unroll
                     for (int c = 0; c < NOUT; ++c)
-                        v[q][c] = s < ns ? __ldcg(part + ((int64_t)c * stride + kl) * ns + s) : 0.0;
+                        v[q][c] = s < ns ? __ldcg(part + (IFAST ? ((int64_t)c * ns + s) * stride + kl
+                                                                : ((int64_t)c * stride + kl) * ns + s))
+                                         : 0.0;
                 }
 #pragma unroll
                 for (int q = 0; q < 4; ++q)

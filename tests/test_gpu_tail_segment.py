@@ -4,7 +4,7 @@ dispatcher hands that tile to the few-i kernel as a segment of its own (nb_api.c
 launches of DIFFERENT variants (thread per i; 2 .. 32 threads per i) write two partial buffers that one
 reduction reads.  Checked element by element against the oracle: by index (own pair, flagged pairs, a bad
 index in either segment), by value with ids, acc + pot only, eps2 = 0; and that calls just outside the
-rule (rem = 0, rem > 128, small N) keep one segment."""
+rule (rem = 0, rem > 128, more than 16384 particles, small N) keep one segment."""
 import numpy as np
 import pytest
 
@@ -37,7 +37,7 @@ def world(nbmod):
     flags = np.zeros(N, np.uint8)
     flags[[40, 1100, 90000, N - 3]] = 1
     xp, vp = oracle.predict(t, x, v, a, j, tj)
-    ctx = nbmod.Context(N, 4200)
+    ctx = nbmod.Context(N, 16500)
     ctx.set_j(m, x, v, a, j, tj)
     fl = np.flatnonzero(flags).astype(np.int32)
     ctx.set_flags(fl, np.ones(len(fl), np.uint8))
@@ -53,7 +53,10 @@ def _i_list(ni, seed):
 
 
 @pytest.mark.parametrize("ni,eps2", [(256 + 1, 2.0 ** -14), (256 + 8, 0.0), (256 + 40, 2.0 ** -14), (512 + 64, 1e-12),
-                                     (768 + 100, 2.0 ** -14), (1024 + 128, 2.0 ** -14), (2048 + 17, 0.0)])
+                                     (768 + 100, 2.0 ** -14), (1024 + 128, 2.0 ** -14), (2048 + 17, 0.0),
+                                     # above 4096 particles the reduction is one thread per i, but one warp per i
+                                     # of the tail (its hundreds of j-subsets)
+                                     (4096 + 20, 2.0 ** -14), (8192 + 100, 0.0)])
 def test_tail_segment_by_index(nbmod, world, ni, eps2):
     ctx, m, xp, vp, flags = world
     il = _i_list(ni, 7310 + ni)
@@ -109,7 +112,7 @@ def test_tail_segment_bad_index_in_either_segment(nbmod, world):
 
 def test_calls_outside_the_rule_keep_one_segment(nbmod, world):
     ctx, m, xp, vp, flags = world
-    for ni in (256, 512, 256 + 129, 1024 + 255, 130, 4096 + 20):
+    for ni in (256, 512, 256 + 129, 1024 + 255, 130, 4096 + 129, 16384 + 20):
         ctx.force(_i_list(ni, 7600 + ni), 1e-6)
         assert ctx.last_launch()["kernels"] == 2, ni
     ctx.tuning(3, 0)                                   # forced j-split: one segment
