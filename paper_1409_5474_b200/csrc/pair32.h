@@ -251,11 +251,27 @@ __device__ __forceinline__ void reduce_row(const ReduceArgs& R, int k, int lane)
 #pragma unroll
                 for (int w = 16; w >= 1; w >>= 1) o[c] += __shfl_xor_sync(0xffffffffu, o[c], w);
         } else {
-            for (int s = 0; s < ns; ++s) {
+            // element (c, s) of my row is at base + c * cs + s * ss in either layout.  Eight subsets are
+            // requested before the first is added (56 loads in flight; one subset at a time the loop is all
+            // load latency: 0.45 us per subset, 47 us of a 380 us call at N = 65536, N_i = 4352, S = 103);
+            // the additions keep their order (R9)
+            const int64_t cs = stride * ns, ss = R.part_i_fastest ? stride : 1;
+            const double* base = part + (R.part_i_fastest ? (int64_t)kl : (int64_t)kl * ns);
+            int s = 0;
+            for (; s + 8 <= ns; s += 8) {
+                double v[8][NOUT];
 #pragma unroll
-                for (int c = 0; c < NOUT; ++c)
-                    o[c] += __ldcg(part + (R.part_i_fastest ? ((int64_t)c * ns + s) * stride + kl
-                                                            : ((int64_t)c * stride + kl) * ns + s));
+                for (int q = 0; q < 8; ++q)
+#pragma unroll
+                    for (int c = 0; c < NOUT; ++c) v[q][c] = __ldcg(base + c * cs + (s + q) * ss);
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+#pragma unroll
+                    for (int c = 0; c < NOUT; ++c) o[c] += v[q][c];
+            }
+            for (; s < ns; ++s) {
+#pragma unroll
+                for (int c = 0; c < NOUT; ++c) o[c] += __ldcg(base + c * cs + s * ss);
             }
         }
     }
