@@ -357,14 +357,18 @@ force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __res
 template <bool FEW, bool GUARD>
 __global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_DYN_MINB : NB_DYN_MINB_ALL) force_dyn_kernel(DynPlan* __restrict__ plan)
 {
-    if (!plan->go || (plan->fa.jsh > 0) != FEW) return;
+    if (!plan->go) return;
+    // the plan's segment for this instantiation: the block itself (fa), or -- few-i form only -- its tail (fb)
+    const bool tail = FEW && plan->fa.jsh == 0 && plan->go_b;
+    if ((plan->fa.jsh > 0) != FEW && !tail) return;
     __shared__ ForceArgs sP;
     __shared__ ReduceArgs sR;
     __shared__ unsigned s_w;
     if (threadIdx.x == 0) {
-        sP = plan->fa;
+        sP = tail ? plan->fb : plan->fa;
         sR = plan->ra;
     }
+    unsigned* const next = tail ? &plan->next_b : &plan->next;
     __syncthreads();
     // the first item of a CTA is its place in the grid; further items are drawn from a counter (the
     // plan kernel zeroed it), so that a CTA whose items ran long does not hold up the launch's tail
@@ -372,7 +376,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_DYN_MINB : NB_DYN_MINB
     unsigned w = blockIdx.x;
     while (w < items) {
         force_body<false, FEW, 0, GUARD, true>(sP, sR, w, nullptr, nullptr, nullptr);   // ends with a CTA barrier
-        if (threadIdx.x == 0) s_w = gridDim.x + atomicAdd(&plan->next, 1u);
+        if (threadIdx.x == 0) s_w = gridDim.x + atomicAdd(next, 1u);
         __syncthreads();
         w = s_w;
         __syncthreads();
@@ -412,10 +416,14 @@ __global__ void __launch_bounds__(128) reduce_dyn_kernel(const DynPlan* __restri
     // a grid of fixed, modest size strides over the block (it was launched before the block's size was known)
     const int64_t gt = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t nthreads = (int64_t)gridDim.x * blockDim.x;
-    if (sR.splits > 8 && sR.ni <= 4096) {
+    const int most = sR.splits > sR.splits_b ? sR.splits : sR.splits_b;
+    if (most > 8 && sR.ni <= 4096) {
         for (int64_t k = gt / 32; k < sR.ni; k += nthreads / 32) reduce_row<true>(sR, (int)k, threadIdx.x & 31);
     } else {
-        for (int64_t k = gt; k < sR.ni; k += nthreads) reduce_row<false>(sR, (int)k, threadIdx.x & 31);
+        // the positions of a tail segment (its hundreds of j-subsets) one warp each, the others one thread each
+        const int64_t first = sR.ni - sR.warp_rows;
+        for (int64_t k = gt; k < first; k += nthreads) reduce_row<false>(sR, (int)k, threadIdx.x & 31);
+        for (int64_t k = first + gt / 32; k < sR.ni; k += nthreads / 32) reduce_row<true>(sR, (int)k, threadIdx.x & 31);
     }
 }
 

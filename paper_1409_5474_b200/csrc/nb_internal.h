@@ -230,6 +230,9 @@ struct DynPlan {
     long long ni;                 // its size
     ForceArgs fa;                 // launch shape and arguments of the pair kernel
     ReduceArgs ra;                // ... and of the reduction
+    int go_b;                     // 1: the block's last, at most half full i-tile is a segment of its own (fb) for the
+    unsigned next_b;              // few-i instantiation, with its own work counter (nb_api.cu force_impl: tail segment)
+    ForceArgs fb;
 };
 struct StepsProgress {            // where a batch of queued kernels stands (device memory)
     long long done;               // block steps completed since nb_steps was called

@@ -454,47 +454,95 @@ __device__ __forceinline__ bool plan_block(const StepsArgs& P, DynPlan* plan, Fo
     while (jsh < JSH_MAX && (ITILE >> (jsh + 1)) >= ni) ++jsh;
     const int itile = ITILE >> jsh;
     const int n_itiles = (int)((ni + itile - 1) / itile);
-    const int resident = jsh > 0 ? resident_few : resident_all;
-    long long smax = (long long)(part_bytes / (NOUT * sizeof(double) * (size_t)n_itiles * itile));
-    if (smax > fa.ntiles) smax = fa.ntiles;
-    if (smax > 4096) smax = 4096;
-    // j-subsets: the resident CTAs loop over n_itiles x S work items, so for every
-    // number of waves w the best S is the largest one that still fits w waves; of those the one with
-    // the best useful-tile fraction wins (each item also pays about two tiles of gather, pipeline fill
-    // and partial store -- the model nb_api.cu choose_splits uses on the host)
-    long long splits = 1;
-    double best = -1.0;
-    const long long w0 = (n_itiles + resident - 1) / resident;
-    for (long long w = w0; w < w0 + 12; ++w) {
-        long long sw = w * resident / n_itiles;
-        if (sw > smax) sw = smax;
-        if (sw < 1) sw = 1;
-        const long long items = (long long)n_itiles * sw;
-        const long long waves = (items + resident - 1) / resident;
-        const long long per = (fa.ntiles + sw - 1) / sw;
-        const double eff = (double)n_itiles * fa.ntiles / ((double)waves * resident * ((double)per + 0.5));
-        // (no term for the number of waves here, unlike choose_splits: the resident CTAs of force_dyn_kernel
-        // draw their items from a counter, which balances the SMs by itself)
-        if (eff > best * 1.004) {
-            best = eff;
-            splits = sw;
+    // a last i-tile that is at most half full becomes a segment of its own for the few-i instantiation
+    // (the rule of nb_api.cu force_impl)
+    int jsh_b = 0, itile_b = 0;
+    if (NB_TAIL_SEGMENT && jsh == 0 && ni > ITILE && ni <= 16384) {
+        const int rem = (int)(ni % ITILE);
+        if (rem >= 1 && rem <= ITILE / 2) {
+            int jb = 0;
+            while (jb < JSH_MAX && (ITILE >> (jb + 1)) >= rem) ++jb;
+            const int ib = ITILE >> jb;
+            if ((double)fa.n * ((double)ITILE - 1.3 * ib) / 0.9e12 >= 15e-6) {
+                jsh_b = jb;
+                itile_b = ib;
+            }
         }
-        if (sw == smax) break;
     }
+    const bool tail = itile_b > 0;
+    const int tiles_a = tail ? n_itiles - 1 : n_itiles;
+    const long long pad_a = (long long)tiles_a * itile;
+    // j-subsets: the resident CTAs loop over tiles x S work items, so for every
+    // number of waves w the best S is the largest one that still fits w waves; of those the one with
+    // the best useful-tile fraction wins (each item also pays about half a tile of gather, pipeline fill
+    // and partial store -- the model nb_api.cu choose_splits uses on the host)
+    auto best_splits = [&](int tiles, int resident, size_t bytes, long long slots) -> long long {
+        long long smax = (long long)(bytes / (NOUT * sizeof(double) * (size_t)slots));
+        if (smax > fa.ntiles) smax = fa.ntiles;
+        if (smax > 4096) smax = 4096;
+        long long splits = 1;
+        double best = -1.0;
+        const long long w0 = (tiles + resident - 1) / resident;
+        for (long long w = w0; w < w0 + 12; ++w) {
+            long long sw = w * resident / tiles;
+            if (sw > smax) sw = smax;
+            if (sw < 1) sw = 1;
+            const long long items = (long long)tiles * sw;
+            const long long waves = (items + resident - 1) / resident;
+            const long long per = (fa.ntiles + sw - 1) / sw;
+            const double eff = (double)tiles * fa.ntiles / ((double)waves * resident * ((double)per + 0.5));
+            // (no term for the number of waves here, unlike choose_splits: the resident CTAs of force_dyn_kernel
+            // draw their items from a counter, which balances the SMs by itself)
+            if (eff > best * 1.004) {
+                best = eff;
+                splits = sw;
+            }
+            if (sw == smax) break;
+        }
+        return splits;
+    };
+    // room for the tail's partials first: at most two waves of its CTAs
+    size_t keep = 0;
+    if (tail) {
+        const long long sb_max = fa.ntiles < 2 * resident_few ? fa.ntiles : 2 * resident_few;
+        keep = (size_t)NOUT * sizeof(double) * (size_t)itile_b * (size_t)sb_max;
+    }
+    const long long splits = best_splits(tiles_a, jsh > 0 ? resident_few : resident_all, part_bytes - keep, pad_a);
     fa.ni = (int)ni;
     fa.jsh = jsh;
     fa.k0 = 0;
-    fa.n_itiles = n_itiles;
-    fa.ni_pad = n_itiles * itile;
+    fa.n_itiles = tiles_a;
+    fa.ni_pad = (int)pad_a;
     fa.splits = (int)splits;
     fa.reduce_here = 0;
-    ra.kA = (int)ni;
+    ra.kA = tail ? (int)pad_a : (int)ni;
     ra.ni = (int)ni;
     ra.ni_pad = fa.ni_pad;
     ra.splits = (int)splits;
     ra.jrk = ra.acc + 3 * ni;                 // the context's block forces: [7][ni]
     ra.pot = ra.acc + 6 * ni;
     ra.t_pred = t1;
+    plan->go_b = 0;
+    if (tail) {
+        ForceArgs fb = fa;
+        double* part_b = fa.part + (size_t)NOUT * (size_t)pad_a * (size_t)splits;
+        const long long splits_b = best_splits(1, resident_few, part_bytes - (size_t)NOUT * sizeof(double) * (size_t)pad_a *
+                                                                                  (size_t)splits, itile_b);
+        fb.jsh = jsh_b;
+        fb.k0 = (int)pad_a;
+        fb.n_itiles = 1;
+        fb.ni_pad = itile_b;
+        fb.splits = (int)splits_b;
+        fb.part = part_b;
+        ra.part_b = part_b;
+        ra.ni_pad_b = itile_b;
+        ra.splits_b = (int)splits_b;
+        const long long most = splits > splits_b ? splits : splits_b;
+        ra.warp_rows = (most > 8 && ni <= 4096) ? 0 : (int)(ni - pad_a);      // force.cu reduce_dyn_kernel
+        plan->fb = fb;
+        plan->next_b = 0u;
+        plan->go_b = 1;
+    }
     plan->fa = fa;
     plan->ra = ra;
     plan->t1 = t1;

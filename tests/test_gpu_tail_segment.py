@@ -132,3 +132,42 @@ def test_calls_outside_the_rule_keep_one_segment(nbmod, world):
         assert small.last_launch()["kernels"] == 2
         small.sync()
     check_parity(got, oracle.force(m2, x2, v2, il, 1e-4))
+
+
+@pytest.mark.parametrize("queue", [2, 1, 0])
+def test_tail_segment_in_a_block_step(nbmod, queue):
+    """nb_steps: a block of 256 q + rem particles that the persistent kernel hands over is planned on the
+    device (steps.cu plan_block: queue modes 2 and 1) or goes through nb_step (mode 0); both cut the tail
+    off.  The steps are set by hand so that the first block is exactly the chosen particles; forces of the
+    block and the corrected state are checked against the oracle's step."""
+    from oracle import hermite as H
+    eps2, eta, lo, hi = 2.0 ** -14, 0.02, 2.0 ** -20, 2.0 ** -4
+    m, x, v = nbgen.plummer(N, 7700)
+    a, j = nbgen.mean_field(x, v)
+    view = nbmod.context._DeviceView
+    with nbmod.Context(N, 8192) as ctx:
+        ctx.steps_queue(queue)
+        for ni in (256 + 40, 1024 + 100, 4096 + 20):
+            idx = np.sort(nbgen.permutation(7701 + ni, N)[:ni]).astype(np.int32)
+            t = np.zeros(N)
+            dt = np.full(N, 2.0 ** -6)
+            dt[idx] = 2.0 ** -10
+            ctx.set_j(m, x, v, a, j, t)
+            ctx.set_dt(dt)
+            done, gt, gni = ctx.steps(1, eps2, eta, lo, hi)[:3]
+            assert done == 1 and gt[0] == 2.0 ** -10 and gni[0] == ni
+            xs, vs, as_, js, ts, dts = x.copy(), v.copy(), a.copy(), j.copy(), t.copy(), dt.copy()
+            t1, due = H.next_block(ts, dts)
+            assert np.array_equal(due, idx)
+            xp, vp = oracle.predict(t1, xs, vs, as_, js, ts)
+            a1, j1, p1 = oracle.force(m, xp, vp, idx, eps2)
+            pa, pj, pp = nbmod.binding.nb_block_forces(ctx.h)
+            ga = torch.as_tensor(view(pa, 3 * ni, "<f8"), device=ctx.device).cpu().numpy().reshape(3, ni)
+            gj = torch.as_tensor(view(pj, 3 * ni, "<f8"), device=ctx.device).cpu().numpy().reshape(3, ni)
+            gp = torch.as_tensor(view(pp, ni, "<f8"), device=ctx.device).cpu().numpy()
+            check_parity([ga, gj, gp], [a1, j1, p1])
+            H.corrector_step(xs, vs, as_, js, ts, dts, idx, t1, a1, j1, eta, lo, hi)
+            g = ctx.state().cpu().numpy()
+            assert np.abs(g[1:4] - xs).max() < 1e-9 and np.abs(g[4:7] - vs).max() < 1e-7
+            assert np.array_equal(g[13], ts) and (g[14] != dts).sum() <= max(2, ni // 100)
+        ctx.sync()
