@@ -546,7 +546,7 @@ def run_blockstep(args):
         with nbm.Context(n) as ctx:
             if args.steps_bound >= 0:
                 ctx.steps_bound(int(args.steps_bound))
-            ctx.steps_queue({"steps_host": 0, "steps_rounds": 1}.get(mode, 2))
+            ctx.steps_queue({"steps_host": 0, "steps_rounds": 1, "steps_graph": 2}.get(mode, -1))   # "steps": the default
             ctx.set_j(m, x, v)
             ctx.predict(0.0)
             ga, gj, gp = ctx.force(il, eps2)
@@ -576,7 +576,8 @@ def run_blockstep(args):
     # A/B inside one process, interleaved: numbers from different gpurun calls differ by +-20 % for a
     # latency-bound loop and must not be compared with each other
     times, times_host = [], []
-    runs = [(md, run(md)) for md in ("step", "steps_host", "steps_rounds", "steps") * 2]
+    runs = [(md, run(md)) for md in ("step", "steps_host", "steps_rounds", "steps_graph", "steps") * 2]
+    ms_graph, _, launches_graph, _, _ = min((r for md, r in runs if md == "steps_graph"), key=lambda r: r[0])
     ms_rounds, _, launches_rounds, _, _ = min((r for md, r in runs if md == "steps_rounds"), key=lambda r: r[0])
     ms_step, _, launches_step, _, _ = min((r for md, r in runs if md == "step"), key=lambda r: r[0])
     ms_host, _, launches_host, _, _ = min((r for md, r in runs if md == "steps_host"), key=lambda r: r[0])
@@ -593,9 +594,10 @@ def run_blockstep(args):
             "data": "synthetic",
             "config": {"workload": "blockstep_plummer_N%d" % n, "eta": eta, "eps2": eps2,
                        "step": "nb_steps: scheduler + predictor-in-pair-loop + reduce + corrector per block in "
-                               "one persistent kernel; blocks above 512 particles or 1.5e7 pairs: launch shape planned "
-                               "on the device, predictor + packed fp32 pair kernel + reduction + corrector queued "
-                               "ahead of time (no host round trip)"},
+                               "one persistent kernel; blocks above 512 particles or 1.5e7 pairs: " +
+                               ("launch shape planned on the device, predictor + packed fp32 pair kernel + reduction + "
+                                "corrector queued ahead of time (no host round trip)" if n < 262144 else
+                                "handed to nb_step's launches (one host synchronisation per such block)")},
             "block": {"mean_n_i": float(sizes.mean()), "median_n_i": float(np.median(sizes)),
                       "min_n_i": int(sizes.min()), "max_n_i": int(sizes.max()),
                       "in_persistent_kernel": in_kernel,
@@ -609,15 +611,18 @@ def run_blockstep(args):
             "ab": {"us_per_block_step_nb_step": ms_step / args.steps * 1e3,
                    "us_per_block_step_nb_steps_host_handover": ms_host / args.steps * 1e3,
                    "us_per_block_step_nb_steps_stream_rounds": ms_rounds / args.steps * 1e3,
+                   "us_per_block_step_nb_steps_graph": ms_graph / args.steps * 1e3,
                    "us_per_block_step_nb_steps": ms / args.steps * 1e3,
+                   "launches_per_block_nb_steps_graph": launches_graph / args.steps,
                    "launches_per_block_nb_steps_stream_rounds": launches_rounds / args.steps,
                    "launches_per_block_nb_step": launches_step / args.steps,
                    "launches_per_block_nb_steps_host_handover": launches_host / args.steps,
                    "launches_per_block_nb_steps": launches / args.steps,
                    "us_total_host_path_host_handover": float(np.minimum(times_host[0], times_host[1])[~small].sum()),
                    "note": "same process, same start and schedule, best of 2 each, interleaved; "
-                           "nb_steps = large blocks planned on the device, rounds in the WHILE node of one graph "
-                           "(nb_set_steps_queue 2, default), stream_rounds = the same rounds queued on the stream (1), "
+                           "nb_steps = the library's default (nb_set_steps_queue -1: graph below 262144 particles, "
+                           "host_handover from there on), graph = large blocks planned on the device, rounds in the "
+                           "WHILE node of one graph (queue 2), stream_rounds = the same rounds queued on the stream (1), "
                            "host_handover = one host synchronisation per large block (queue 0)"},
             "gpu_launches": int(launches)}
     if args.detail:

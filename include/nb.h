@@ -378,9 +378,9 @@ int nb_step(nb_ctx* c, double eps2, double eta, double dt_min, double dt_max, do
  * R18..R21 and the same decisions as nb_step).  It leaves a block to other kernels only when the block
  * is large -- more than 512 particles, or N_i x n above the bound of nb_set_steps_bound (default
  * 1.5e7 pairs: beyond it the packed fp32 pair kernel plus its launches beats the fp64 loop) -- and
- * how those kernels are issued is nb_set_steps_queue's choice: by default their launch shape is
- * planned on the device and they run as the body of a WHILE node of one CUDA graph, so that the host
- * synchronises once per nb_steps call; in mode 0 once per large block.
+ * how those kernels are issued is nb_set_steps_queue's choice: by default (fewer than 262144 particles)
+ * their launch shape is planned on the device and they run as the body of a WHILE node of one CUDA graph,
+ * so that the host synchronises once per nb_steps call; in mode 0 once per large block.
  * Stops after k steps, or before the first block whose time exceeds t_end (+inf: no limit; NaN is
  * NB_ERR_ARG).  HOST outputs: *done = steps taken; t_log[0..done), ni_log[0..done) and us_log[0..done)
  * = block time, block size and device time in microseconds (%globaltimer) of every step (each may be
@@ -395,7 +395,10 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
 int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs);
 
 /* How nb_steps takes a handed-over (large) block (the host link is the bottleneck).
- * mode 2 (default): the block's launch shape is planned ON THE DEVICE and one "round" -- persistent
+ * mode -1 (default): mode 2 while the j-set has fewer than 262144 particles, mode 0 from there on (large
+ *   blocks are then most of the run and nb_step's launches the faster way to take them; measured per block
+ *   step, mode 2 / mode 0: N = 131072: 131 / 134 us, 262144: 330 / 328, 524288: 491 / 478, 2^20: 1278 / 1248).
+ * mode 2: the block's launch shape is planned ON THE DEVICE and one "round" -- persistent
  *   kernel, plan, predictor, packed fp32 pair kernel (both thread mappings), reduction, corrector,
  *   each of which exits at once when it has nothing to do -- is the body of a WHILE node of a CUDA
  *   graph whose condition the plan kernel sets: one graph launch and one synchronisation per

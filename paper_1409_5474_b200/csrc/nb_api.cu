@@ -63,7 +63,8 @@ struct nb_ctx {
     int steps_ok = -1;                  // -1 unknown, 0 the cooperative kernel cannot be resident, 1 fine
     DynPlan* steps_plan = nullptr;      // the device-planned launch shape of a handed-over block
     StepsProgress* steps_prog = nullptr;   // where a queued batch of nb_steps stands
-    int steps_queue = 2;                // 0: host handover; 1: rounds queued ahead on the stream; 2: one graph with a WHILE node
+    int steps_queue = -1;               // 0: host handover; 1: rounds queued ahead on the stream; 2: one graph with a WHILE node;
+                                        // -1: by the size of the j-set (queue_mode)
     // the graph of mode 2 (built on first use, rebuilt when an argument baked into its kernels changes)
     cudaStream_t cap_stream = nullptr;
     cudaGraph_t steps_graph = nullptr;
@@ -1413,9 +1414,20 @@ int nb_set_steps_bound(nb_ctx* c, int64_t max_pairs)
 int nb_set_steps_queue(nb_ctx* c, int on)
 {
     if (!c) return NB_ERR_ARG;
-    if (on < 0 || on > 2) return NB_ERR_ARG;
+    if (on < -1 || on > 2) return NB_ERR_ARG;
     c->steps_queue = on;
     return NB_OK;
+}
+
+// The mode in force.  Automatic: rounds planned on the device in one graph while the j-set is small (no
+// host round trip per large block), the host's own launches from 262144 particles on, where the large
+// blocks are most of the time and nb_step's pair kernel (4 CTAs per SM; the device-planned form has 3) is
+// the faster one.  Measured per block step (bench.py --blockstep), mode 2 / mode 0, N = 131072: 130.9 /
+// 134.3 us, 262144: 329.5 / 327.6, 524288: 490.5 / 478.4, 2^20: 1278 / 1248.
+static int queue_mode(const nb_ctx* c)
+{
+    if (c->steps_queue >= 0) return c->steps_queue;
+    return c->n >= 262144 ? 0 : 2;
 }
 
 // nb_steps with handed-over blocks planned ON THE DEVICE (steps.cu plan_kernel): the host queues
@@ -1508,7 +1520,7 @@ static int steps_queued(nb_ctx* c, int64_t k, double eps2, double eta, double dt
     // Mode 2: the rounds are the body of a WHILE node of ONE graph (the plan kernel sets the loop
     // condition on the device), followed by a launch that closes the last time stamp: one graph launch
     // per nb_steps call, no empty rounds, nothing for the host to do until the end.
-    if (c->steps_queue == 2 && c->steps_graph_state >= 0) {
+    if (queue_mode(c) == 2 && c->steps_graph_state >= 0) {
         const double key[8] = {eps2, eta, dt_min, dt_max, t_end, (double)c->steps_max_pairs, (double)c->n,
                                (double)c->flagged.size()};
         const void* kp[3] = {c->steps_log_t, c->steps_log_ni, c->steps_log_ns};
@@ -1567,7 +1579,7 @@ static int steps_queued(nb_ctx* c, int64_t k, double eps2, double eta, double dt
     }
 
     int result = NB_OK;
-    if (c->steps_queue == 2 && c->steps_graph_state == 1) {
+    if (queue_mode(c) == 2 && c->steps_graph_state == 1) {
         if (cudaGraphLaunch(c->steps_exec, c->stream) != cudaSuccess) {
             cudaGetLastError();
             return NB_ERR_CUDA;
@@ -1609,7 +1621,7 @@ static int steps_queued(nb_ctx* c, int64_t k, double eps2, double eta, double dt
     if (p_out->pending_ni > 0) result = NB_ERR_ARG;            // a block above ni_max: the list was truncated
     else if (p_out->final && p_out->reason == STEPS_STUCK) result = NB_ERR_STATE;
     if (p_out->done > 0) c->blk_ni = (int64_t)meta_out[3];     // for nb_block_forces
-    if (want_us && !p_out->closed && p_out->pending_ni == 0 && !(c->steps_queue == 2 && c->steps_graph_state == 1)) {
+    if (want_us && !p_out->closed && p_out->pending_ni == 0 && !(queue_mode(c) == 2 && c->steps_graph_state == 1)) {
         // the batch ended with a device-planned block: one more (empty) launch stamps the closing time
         if (launch_steps(a, c->sm_count, c->stream) != cudaSuccess) {
             cudaGetLastError();
@@ -1660,7 +1672,7 @@ int nb_steps(nb_ctx* c, int64_t k, double eps2, double eta, double dt_min, doubl
     // handed-over blocks are planned on the device and queued, unless the mode was switched off, the
     // pair loop is the IEEE-double one (its launch shapes are not planned on the device) or the
     // reduction runs by atomics
-    const bool queued = c->steps_ok == 1 && c->steps_queue && c->precision == 0 && c->tune_reduce == 0 &&
+    const bool queued = c->steps_ok == 1 && queue_mode(c) != 0 && c->precision == 0 && c->tune_reduce == 0 &&
                         c->tune_splits == 0;
     std::vector<int64_t> host_idx;            // steps that went through the host path: (index, t, ni)
     std::vector<double> host_t;

@@ -173,6 +173,17 @@ def test_steps_host_path_and_mixed(nbmod, queue):
         ctx.sync()
 
 
+def test_steps_queue_modes_accepted(nbmod):
+    nb = nbmod.binding
+    with nbmod.Context(64) as ctx:
+        for mode in (-1, 0, 1, 2, -1):
+            ctx.steps_queue(mode)
+        for mode in (-2, 3):
+            with pytest.raises(nb.NBError) as e:
+                ctx.steps_queue(mode)
+            assert e.value.status == nb.NB_ERR_ARG
+
+
 def test_steps_queued_flags_eps0_t_end_and_overflow(nbmod):
     """The device-planned path for handed-over blocks (bound 0: every block): unsoftened flagged
     pairs, eps2 = 0 (the guarded pair kernels), t_end, k larger than what is left, and a block above
