@@ -171,3 +171,38 @@ def test_tail_segment_in_a_block_step(nbmod, queue):
             assert np.abs(g[1:4] - xs).max() < 1e-9 and np.abs(g[4:7] - vs).max() < 1e-7
             assert np.array_equal(g[13], ts) and (g[14] != dts).sum() <= max(2, ni // 100)
         ctx.sync()
+
+
+def test_random_midsize_shapes(nbmod):
+    """Seeded random (N, N_i) around the rule's edges -- rem = 1, 128, 129, 255, 0; N on both sides of the
+    threshold; by index and by value; eps2 = 0 now and then -- each against the oracle."""
+    rng = np.random.RandomState(7800)
+    rems = [1, 2, 7, 8, 9, 16, 17, 31, 32, 33, 63, 64, 65, 127, 128, 129, 200, 255, 0]
+    for case in range(19):
+        n = int(rng.choice([60000, 70001, 90000, 149000, 152000, 200003, 300000]))
+        q = int(rng.choice([1, 1, 2, 3, 5, 8, 15, 16, 17, 33]))
+        ni = 256 * q + rems[case]
+        eps2 = float(rng.choice([0.0, 2.0 ** -14, 1e-12]))
+        m, x, v = nbgen.plummer(n, 7801 + case)
+        zero = np.zeros((3, n))
+        flags = np.zeros(n, np.uint8)
+        il = nbgen.permutation(7900 + case, n)[:ni].astype(np.int32)
+        if case % 3 == 0:
+            flags[il[[0, ni - 1]]] = 1
+            flags[il[ni // 2]] = 1
+        with nbmod.Context(n, ni) as ctx:
+            ctx.set_j(m, x, v, zero, zero, np.zeros(n))
+            fl = np.flatnonzero(flags).astype(np.int32)
+            if len(fl):
+                ctx.set_flags(fl, np.ones(len(fl), np.uint8))
+            ctx.predict(0.0)
+            if case % 2 == 0:
+                got = [g.cpu().numpy() for g in ctx.force(il, eps2)]
+            else:
+                got = [g.cpu().numpy() for g in ctx.force_ext_ids(x[:, il], v[:, il], il, flags[il], eps2)]
+            kernels = ctx.last_launch()["kernels"]
+            ctx.sync()
+        rem = ni % 256
+        if rem == 0 or rem > 128 or ni > 16384:
+            assert kernels == 2, (case, n, ni)
+        check_parity(got, oracle.force(m, x, v, il, eps2, flags if flags.any() else None))
