@@ -374,7 +374,8 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
     // (2^jsh threads per i: 128 .. 8 slots per CTA), A = the q full tiles with j split by choose_splits --
     // when a 256-slot pass over j costs clearly more than the smaller one plus a launch (measured at
     // N = 131072: N_i = 288 / 320 went from 100 us to 74 / 82 us, at N = 2^20: N_i = 257 from 591 us to 325 us;
-    // at N = 32768 a launch costs what the pass costs, so small j-sets keep one segment).  Above 4096
+    // at N = 32768 a launch costs what the pass costs, so small j-sets keep one segment: the model's saving
+    // must reach NB_TAIL_MIN_GAIN, nb_internal.h).  Above 4096
     // particles the reduction is one thread per i, which would add the tail's hundreds of j-subsets one
     // dependent load at a time (measured: +130 us at N_i = 4128): the tail's positions are then summed by
     // one warp each (ReduceArgs.warp_rows).  Beyond 16384 particles the tile is < 1.6 % of the call (measured at 16400 and 32800: -0.7 ... +2 %).
@@ -388,7 +389,7 @@ int force_impl(nb_ctx* c, const int32_t* i_list, int64_t ni, double eps2, double
             while (jb < JSH_MAX && (ITILE >> (jb + 1)) >= rem) ++jb;
             const int ib = ITILE >> jb;
             const double saved_s = (double)n_launch * ((double)ITILE - 1.3 * ib) / 0.9e12;
-            if (saved_s >= 15e-6) {
+            if (saved_s >= NB_TAIL_GAIN_NEEDED(ib, ni)) {
                 tail = true;
                 jsh_b = jb;
                 itile_b = ib;

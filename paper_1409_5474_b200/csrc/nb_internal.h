@@ -39,6 +39,14 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 #define NB_TAIL_SEGMENT 1          // nb_force: a last i-tile that is at most half full goes to the few-i kernel as a
                                    // segment of its own (nb_api.cu force_impl); 0 = one all-i segment as before
 #endif
+#ifndef NB_TAIL_MIN_GAIN
+#define NB_TAIL_MIN_GAIN 9e-6      // ... when the model says it saves at least this many seconds (an extra launch costs ~5 us);
+#define NB_TAIL_MIN_GAIN_HALF 13e-6   // a 128-slot tail saves 0.42 of a pass at best and needs more (measured at N = 98304,
+                                      // N_i = 1152: 166 -> 180 us with 9e-6; at N = 131072: 207 -> 203 us)
+#endif
+// (and 20e-6 above 4096 particles, where the call's reduction is the thread-per-i one: N = 131072, N_i = 4224: 640 -> 652 us
+// with 13e-6; N = 262144: 1256 -> 1210 us)
+#define NB_TAIL_GAIN_NEEDED(slots, ni) ((slots) >= ITILE / 2 ? ((ni) > 4096 ? 20e-6 : NB_TAIL_MIN_GAIN_HALF) : NB_TAIL_MIN_GAIN)
 #ifndef NB_DYN_MINB
 #define NB_DYN_MINB 3
 #endif

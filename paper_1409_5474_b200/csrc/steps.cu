@@ -463,7 +463,7 @@ __device__ __forceinline__ bool plan_block(const StepsArgs& P, DynPlan* plan, Fo
             int jb = 0;
             while (jb < JSH_MAX && (ITILE >> (jb + 1)) >= rem) ++jb;
             const int ib = ITILE >> jb;
-            if ((double)fa.n * ((double)ITILE - 1.3 * ib) / 0.9e12 >= 15e-6) {
+            if ((double)fa.n * ((double)ITILE - 1.3 * ib) / 0.9e12 >= NB_TAIL_GAIN_NEEDED(ib, ni)) {
                 jsh_b = jb;
                 itile_b = ib;
             }

@@ -56,7 +56,7 @@ def _i_list(ni, seed):
                                      (768 + 100, 2.0 ** -14), (1024 + 128, 2.0 ** -14), (2048 + 17, 0.0),
                                      # above 4096 particles the reduction is one thread per i, but one warp per i
                                      # of the tail (its hundreds of j-subsets)
-                                     (4096 + 20, 2.0 ** -14), (8192 + 100, 0.0)])
+                                     (4096 + 20, 2.0 ** -14), (8192 + 60, 0.0)])
 def test_tail_segment_by_index(nbmod, world, ni, eps2):
     ctx, m, xp, vp, flags = world
     il = _i_list(ni, 7310 + ni)
