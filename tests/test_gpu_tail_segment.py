@@ -206,3 +206,22 @@ def test_random_midsize_shapes(nbmod):
         if rem == 0 or rem > 128 or ni > 16384:
             assert kernels == 2, (case, n, ni)
         check_parity(got, oracle.force(m, x, v, il, eps2, flags if flags.any() else None))
+
+
+def test_tail_segment_under_the_peer_exchange(nbmod, world):
+    """nb_xforce (world of one: the whole window / flag / sum path) on a call with a tail segment returns
+    nb_force_ext_ids' forces bit for bit: the exchange kernels run after the one reduction of both segments."""
+    ctx, m, xp, vp, flags = world
+    ctx.xchg_create(0, 1, 2048)
+    try:
+        for ni in (256 + 40, 1024 + 7):
+            il = _i_list(ni, 8000 + ni)
+            args = (xp[:, il], vp[:, il], il, flags[il], 2.0 ** -14)
+            want = [q.cpu().numpy() for q in ctx.force_ext_ids(*args)]
+            assert ctx.last_launch()["kernels"] == 3
+            got = [q.cpu().numpy() for q in ctx.xforce(*args)]
+            assert ctx.last_launch()["kernels"] == 5           # + push + sum
+            ctx.sync()
+            assert all(np.array_equal(g, w) for g, w in zip(got, want))
+    finally:
+        ctx.xchg_destroy()
