@@ -20,6 +20,7 @@
 #include "nb_internal.h"
 #include "pair32.h"
 #include "xchg.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -37,6 +38,7 @@ direct_kernel(ForceArgs P, ReduceArgs R)
     __shared__ double sred[DIRECT_THREADS / 32][NI][NOUT];
     __shared__ int s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();       // pdl.h
 
     // a3 starts here: the first UNR quads of this thread are requested before anything else -- they do
     // not depend on the i-particles, whose gather (two dependent loads) then runs under their latency
@@ -201,9 +203,8 @@ direct_kernel(ForceArgs P, ReduceArgs R)
 template <int NI>
 cudaError_t launch_ni(const ForceArgs& a, const ReduceArgs& r, int grid, cudaStream_t s)
 {
-    if (a.eps2 < EPS2_GUARD) direct_kernel<NI, true><<<grid, DIRECT_THREADS, 0, s>>>(a, r);
-    else direct_kernel<NI, false><<<grid, DIRECT_THREADS, 0, s>>>(a, r);
-    return cudaGetLastError();
+    if (a.eps2 < EPS2_GUARD) return pdl_launch(direct_kernel<NI, true>, grid, DIRECT_THREADS, 0, s, a, r);
+    return pdl_launch(direct_kernel<NI, false>, grid, DIRECT_THREADS, 0, s, a, r);
 }
 
 }  // namespace

@@ -16,6 +16,7 @@
 #include "pair32.h"
 #include "tma.h"
 #include "xchg.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -347,6 +348,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_MINB_FEW : NB_MINB)
 force_kernel(ForceArgs P, ReduceArgs R, double* __restrict__ oacc, double* __restrict__ ojrk,
              double* __restrict__ opot)
 {
+    pdl_wait();       // pdl.h: the pack and the partial buffers belong to earlier kernels until this returns
     force_body<ATOMIC, FEW, MODE, GUARD, false>(P, R, blockIdx.x, oacc, ojrk, opot);
 }
 
@@ -387,6 +389,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FEW ? NB_DYN_MINB : NB_DYN_MINB
 template <bool WARP>
 __global__ void __launch_bounds__(128) reduce_kernel(ReduceArgs R)
 {
+    pdl_wait();       // pdl.h
     if (!WARP && R.warp_rows > 0) {
         // the first CTAs take positions [0, ni - warp_rows) one per thread, the others the rest one per warp
         const int first = R.ni - R.warp_rows, ctas_a = (first + 127) / 128;
@@ -499,13 +502,13 @@ void launch_one(const ForceArgs& a, const ReduceArgs& r, int mode, int atomic_mo
 {
     const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
     if (mode == 1)
-        force_kernel<false, FEW, 1, GUARD><<<grid, FORCE_THREADS, force_smem(FEW), s>>>(a, r, acc, jrk, pot);
+        pdl_launch(force_kernel<false, FEW, 1, GUARD>, grid, FORCE_THREADS, force_smem(FEW), s, a, r, acc, jrk, pot);
     else if (mode == 2)
-        force_kernel<false, FEW, 2, GUARD><<<grid, FORCE_THREADS, force_smem(FEW), s>>>(a, r, acc, jrk, pot);
+        pdl_launch(force_kernel<false, FEW, 2, GUARD>, grid, FORCE_THREADS, force_smem(FEW), s, a, r, acc, jrk, pot);
     else if (atomic_mode)
-        force_kernel<true, FEW, 0, GUARD><<<grid, FORCE_THREADS, force_smem(FEW), s>>>(a, r, acc, jrk, pot);
+        pdl_launch(force_kernel<true, FEW, 0, GUARD>, grid, FORCE_THREADS, force_smem(FEW), s, a, r, acc, jrk, pot);
     else
-        force_kernel<false, FEW, 0, GUARD><<<grid, FORCE_THREADS, force_smem(FEW), s>>>(a, r, acc, jrk, pot);
+        pdl_launch(force_kernel<false, FEW, 0, GUARD>, grid, FORCE_THREADS, force_smem(FEW), s, a, r, acc, jrk, pot);
 }
 
 // a.jsh > 0 selects the few-i kernel, which also reduces (unless atomic_mode): r must then be complete
@@ -549,13 +552,11 @@ cudaError_t launch_reduce_dyn(const DynPlan* plan, int64_t ni_max, cudaStream_t 
 cudaError_t launch_reduce(const ReduceArgs& a, cudaStream_t s)
 {
     const int most = a.splits > a.splits_b ? a.splits : a.splits_b;
-    if (!a.atomic_mode && most > 8 && a.ni <= 4096)
-        reduce_kernel<true><<<(a.ni + 3) / 4, 128, 0, s>>>(a);
-    else if (a.warp_rows > 0)
-        reduce_kernel<false><<<(a.ni - a.warp_rows + 127) / 128 + (a.warp_rows + 3) / 4, 128, 0, s>>>(a);
-    else
-        reduce_kernel<false><<<(a.ni + 127) / 128, 128, 0, s>>>(a);
-    return cudaGetLastError();
+    const bool warp = !a.atomic_mode && most > 8 && a.ni <= 4096;
+    const unsigned grid = warp ? (a.ni + 3) / 4
+                               : (a.warp_rows > 0 ? (a.ni - a.warp_rows + 127) / 128 + (a.warp_rows + 3) / 4
+                                                  : (a.ni + 127) / 128);
+    return warp ? pdl_launch(reduce_kernel<true>, grid, 128, 0, s, a) : pdl_launch(reduce_kernel<false>, grid, 128, 0, s, a);
 }
 
 cudaError_t launch_zero_out(double* acc, double* jrk, double* pot, int64_t ni, cudaStream_t s)

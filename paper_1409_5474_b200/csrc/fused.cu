@@ -15,6 +15,7 @@
 // eps2 = 0 in the loop (R5, R7).
 #include "nb_internal.h"
 #include "pair64.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -38,6 +39,7 @@ fused_kernel(StorePtrs st, const uint8_t* __restrict__ flags, const int32_t* __r
     __shared__ int sflag[NI];
     __shared__ double sred[FUSED_THREADS / 32][NI][NOUT];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();       // pdl.h
 
     // the active particles, predicted to t (R8: i and j alike are taken at their predicted state)
     if (tid < NI) {
@@ -130,16 +132,16 @@ cudaError_t launch_fused(const StorePtrs& st, const uint8_t* flags, const int32_
     *grid_out = grid;
     if (ni <= 1) {
         *ni_pad_out = 1;
-        fused_kernel<1><<<grid, FUSED_THREADS, 0, s>>>(st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
+        return pdl_launch(fused_kernel<1>, grid, FUSED_THREADS, 0, s, st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
     } else if (ni <= 2) {
         *ni_pad_out = 2;
-        fused_kernel<2><<<grid, FUSED_THREADS, 0, s>>>(st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
+        return pdl_launch(fused_kernel<2>, grid, FUSED_THREADS, 0, s, st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
     } else if (ni <= 4) {
         *ni_pad_out = 4;
-        fused_kernel<4><<<grid, FUSED_THREADS, 0, s>>>(st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
+        return pdl_launch(fused_kernel<4>, grid, FUSED_THREADS, 0, s, st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
     } else {
         *ni_pad_out = 8;
-        fused_kernel<8><<<grid, FUSED_THREADS, 0, s>>>(st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
+        return pdl_launch(fused_kernel<8>, grid, FUSED_THREADS, 0, s, st, flags, i_list, ni, n, n_pad, t, eps2, any_flagged, part, err);
     }
     return cudaGetLastError();
 }

@@ -9,6 +9,7 @@
 
 #include "nb_internal.h"
 #include "hermite_dev.h"
+#include "pdl.h"
 
 namespace cg = cooperative_groups;
 
@@ -127,6 +128,7 @@ correct_kernel(StorePtrs st, double* __restrict__ dts, const int32_t* __restrict
                int64_t n, double t1, const double* __restrict__ acc, const double* __restrict__ jrk,
                double eta, double dt_min, double dt_max, int* err)
 {
+    pdl_wait();       // pdl.h
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= ni) return;
     const int64_t i = list[k];
@@ -202,9 +204,8 @@ cudaError_t launch_correct(const StorePtrs& st, double* dts, const int32_t* list
                            double dt_max, int* err, cudaStream_t s)
 {
     if (ni == 0) return cudaSuccess;
-    correct_kernel<<<(unsigned)((ni + 127) / 128), 128, 0, s>>>(st, dts, list, ni, n, t1, acc, jrk, eta,
-                                                                dt_min, dt_max, err);
-    return cudaGetLastError();
+    return pdl_launch(correct_kernel, (unsigned)((ni + 127) / 128), 128, 0, s, st, dts, list, ni, n, t1, acc, jrk, eta, dt_min,
+                      dt_max, err);
 }
 
 cudaError_t launch_init_steps(const StorePtrs& st, double* dts, const int32_t* list, int64_t ni, int64_t n,

@@ -35,6 +35,10 @@ enum Field { F_M = 0, F_X, F_Y, F_Z, F_VX, F_VY, F_VZ, F_AX, F_AY, F_AZ, F_JX, F
 #ifndef NB_MINB_FEW
 #define NB_MINB_FEW 3
 #endif
+#ifndef NB_PDL
+#define NB_PDL 1                   // force_kernel and reduce_kernel are launched with programmatic stream serialization
+                                   // and wait for the kernel before them with griddepcontrol.wait (force.cu pdl_launch)
+#endif
 #ifndef NB_TAIL_SEGMENT
 #define NB_TAIL_SEGMENT 1          // nb_force: a last i-tile that is at most half full goes to the few-i kernel as a
                                    // segment of its own (nb_api.cu force_impl); 0 = one all-i segment as before

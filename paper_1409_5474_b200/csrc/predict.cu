@@ -6,6 +6,7 @@
 // flag word) into the tiled pack the pair kernel streams.  All accesses are unit-stride across
 // the warp; each thread handles two particles so that loads are 128-bit and stores 64-bit.
 #include "nb_internal.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -26,6 +27,7 @@ __global__ void __launch_bounds__(256) update_j_kernel(StorePtrs dst, SrcPtrs sr
                                                        const int32_t* __restrict__ idx,
                                                        int64_t count, int64_t n, int* err)
 {
+    pdl_wait();       // pdl.h
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < count; p += stride) {
         const int64_t q = idx[p];
@@ -73,6 +75,7 @@ __global__ void __launch_bounds__(128) predict_kernel(StorePtrs st, const uint8_
                                                       int64_t n, int64_t n_pad, double t,
                                                       const DynPlan* __restrict__ plan)
 {
+    pdl_wait();       // pdl.h (a no-op in the rounds nb_steps queues: those are launched without the attribute)
     if (plan) {                   // a block planned on the device (nb_steps): its time, or nothing to do
         if (!plan->go) return;
         t = plan->t1;
@@ -182,8 +185,7 @@ cudaError_t launch_update_j(const StorePtrs& dst, const SrcPtrs& src, const int3
                             int64_t count, int64_t n, int* err, cudaStream_t s)
 {
     if (count == 0) return cudaSuccess;
-    update_j_kernel<<<grid_for(count, 256, 148 * 16), 256, 0, s>>>(dst, src, idx, count, n, err);
-    return cudaGetLastError();
+    return pdl_launch(update_j_kernel, grid_for(count, 256, 148 * 16), 256, 0, s, dst, src, idx, count, n, err);
 }
 
 cudaError_t launch_set_flags(uint8_t* flags, const int32_t* idx_then_val, int count, cudaStream_t s)
@@ -202,7 +204,10 @@ cudaError_t launch_predict(const StorePtrs& store, const uint8_t* flags, float* 
     if (pack64 && pack6) predict_kernel<true, true><<<grid, 128, 0, s>>>(store, flags, pack, pack64, pack6, n, n_pad, t, plan);
     else if (pack64) predict_kernel<true, false><<<grid, 128, 0, s>>>(store, flags, pack, pack64, nullptr, n, n_pad, t, plan);
     else if (pack6) predict_kernel<false, true><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, pack6, n, n_pad, t, plan);
-    else predict_kernel<false, false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, nullptr, n, n_pad, t, plan);
+    else if (plan) predict_kernel<false, false><<<grid, 128, 0, s>>>(store, flags, pack, nullptr, nullptr, n, n_pad, t, plan);
+    else   // the default mode outside nb_steps' queued rounds: may be set up while the kernel before it drains
+        return pdl_launch(predict_kernel<false, false>, grid, 128, 0, s, store, flags, pack, (double*)nullptr, (float*)nullptr, n,
+                          n_pad, t, plan);
     return cudaGetLastError();
 }
 
