@@ -3,6 +3,7 @@
 // For a handful of active particles the same steps run inside the pair kernel's last CTA (force.cu), so
 // that pair loop, reduction, exchange and cross-rank sum are ONE launch.
 #include "xchg.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -16,6 +17,7 @@ __global__ void __launch_bounds__(XT) xchg_push_kernel(const Xchg* __restrict__ 
                                                         double* pot, long long ni, unsigned* ticket)
 {
     __shared__ int s_last;
+    pdl_wait();       // pdl.h: the reduction before this kernel has written acc / jrk / pot
     const int world = X->world, rank = X->rank;
     const long long total = (long long)NOUT * ni;
     for (long long q = (long long)blockIdx.x * XT + threadIdx.x; q < total; q += (long long)gridDim.x * XT) {
@@ -41,6 +43,7 @@ __global__ void __launch_bounds__(XT) xchg_push_kernel(const Xchg* __restrict__ 
 __global__ void __launch_bounds__(XT) xchg_sum_kernel(const Xchg* __restrict__ X, unsigned epoch, double* acc, double* jrk,
                                                        double* pot, long long ni, int* err, unsigned long long limit_ns)
 {
+    pdl_wait();       // pdl.h: my own push (the kernel before this one) is complete
     xchg_wait(X, epoch, threadIdx.x, err, limit_ns);
     const long long total = (long long)NOUT * ni;
     for (long long q = (long long)blockIdx.x * XT + threadIdx.x; q < total; q += (long long)gridDim.x * XT) {
@@ -62,15 +65,13 @@ unsigned grid_for(long long ni)
 cudaError_t launch_xchg_push(const Xchg* X, unsigned epoch, double* acc, double* jrk, double* pot, long long ni,
                              unsigned* ticket, cudaStream_t s)
 {
-    xchg_push_kernel<<<grid_for(ni), XT, 0, s>>>(X, epoch, acc, jrk, pot, ni, ticket);
-    return cudaGetLastError();
+    return pdl_launch(xchg_push_kernel, grid_for(ni), XT, 0, s, X, epoch, acc, jrk, pot, ni, ticket);
 }
 
 cudaError_t launch_xchg_sum(const Xchg* X, unsigned epoch, double* acc, double* jrk, double* pot, long long ni, int* err,
                             unsigned long long limit_ns, cudaStream_t s)
 {
-    xchg_sum_kernel<<<grid_for(ni), XT, 0, s>>>(X, epoch, acc, jrk, pot, ni, err, limit_ns);
-    return cudaGetLastError();
+    return pdl_launch(xchg_sum_kernel, grid_for(ni), XT, 0, s, X, epoch, acc, jrk, pot, ni, err, limit_ns);
 }
 
 }  // namespace nb
