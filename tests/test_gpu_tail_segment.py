@@ -225,3 +225,30 @@ def test_tail_segment_under_the_peer_exchange(nbmod, world):
             assert all(np.array_equal(g, w) for g, w in zip(got, want))
     finally:
         ctx.xchg_destroy()
+
+
+def test_predict_and_force_captured_into_a_cuda_graph(nbmod):
+    """nb_predict + nb_force recorded into a CUDA graph on the context's stream and replayed: the chains of
+    dependent launches (csrc/pdl.h), the one-launch kernels, the few-i kernel and a call with a tail segment
+    all give the bits of the eager call."""
+    n = 150000
+    m, x, v = nbgen.plummer(n, 8100)
+    zero = np.zeros((3, n))
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        with nbmod.Context(n, 4096, stream=s.cuda_stream) as ctx:
+            ctx.set_j(m, x, v, zero, zero, np.zeros(n))
+            ctx.predict(0.0)
+            for ni in (1, 12, 100, 300, 1024):
+                il = torch.as_tensor(nbgen.permutation(8101, n)[:ni].astype(np.int32)).to(ctx.device)
+                eager = [q.clone() for q in ctx.force(il, 1e-6)]
+                s.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=s):
+                    ctx.predict(0.0)
+                    out = ctx.force(il, 1e-6)
+                for _ in range(3):
+                    graph.replay()
+                torch.cuda.synchronize()
+                assert all(torch.equal(a, b) for a, b in zip(eager, out)), ni
+            ctx.sync()
