@@ -20,6 +20,7 @@
 // reduction, straight from the j-store).
 #include "nb_internal.h"
 #include "tma.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -89,6 +90,7 @@ __device__ __forceinline__ void pair6(const I6& I, A6& A, const float2* f, float
 
 __global__ void __launch_bounds__(FORCE_THREADS, 2) force6_kernel(Force6Args P)
 {
+    pdl_wait();       // pdl.h
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STG6 * TILE6_BYTES);
@@ -210,6 +212,7 @@ __global__ void __launch_bounds__(128) reduce6_kernel(Force6Args P, StorePtrs st
                                                       double t_pred, double* acc, double* jrk, double* snp,
                                                       double* pot)
 {
+    pdl_wait();       // pdl.h
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= P.ni) return;
     double o[NOUT6];
@@ -286,14 +289,12 @@ cudaError_t launch_force6(const Force6Args& a, const StorePtrs& st, const int32_
                           double* acc, double* jrk, double* snp, double* pot, cudaStream_t s)
 {
     if (a.ntiles > 0) {
-        force6_kernel<<<(unsigned)a.n_itiles * (unsigned)a.splits, FORCE_THREADS, F6_SMEM, s>>>(a);
-        cudaError_t e = cudaGetLastError();
+        cudaError_t e = pdl_launch(force6_kernel, (unsigned)a.n_itiles * (unsigned)a.splits, FORCE_THREADS, F6_SMEM, s, a);
         if (e != cudaSuccess) return e;
     }
     Force6Args r = a;
     if (a.ntiles == 0) r.splits = 0;
-    reduce6_kernel<<<(unsigned)((a.ni + 127) / 128), 128, 0, s>>>(r, st, flag_list, nflag, t_pred, acc, jrk, snp, pot);
-    return cudaGetLastError();
+    return pdl_launch(reduce6_kernel, (unsigned)((a.ni + 127) / 128), 128, 0, s, r, st, flag_list, nflag, t_pred, acc, jrk, snp, pot);
 }
 
 }  // namespace nb

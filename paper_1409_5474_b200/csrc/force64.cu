@@ -17,6 +17,7 @@
 #include "nb_internal.h"
 #include "pair64.h"
 #include "tma.h"
+#include "pdl.h"
 
 namespace nb {
 
@@ -31,6 +32,7 @@ template <bool FLAGS, int MODE>
 __global__ void __launch_bounds__(FORCE_THREADS, 3) force64_kernel(ForceArgs P)
 {
     constexpr bool JERK = (MODE != 2);
+    pdl_wait();       // pdl.h
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* tiles = reinterpret_cast<double*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + STAGES64 * TILE64_BYTES);
@@ -164,11 +166,10 @@ cudaError_t force64_kernel_setup(int* blocks_per_sm)
 cudaError_t launch_force64(const ForceArgs& a, int mode, cudaStream_t s)
 {
     const unsigned grid = (unsigned)a.n_itiles * (unsigned)a.splits;
-    if (mode == 1) force64_kernel<false, 1><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
-    else if (mode == 2) force64_kernel<false, 2><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
-    else if (a.any_flagged) force64_kernel<true, 0><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
-    else force64_kernel<false, 0><<<grid, FORCE_THREADS, F64_SMEM, s>>>(a);
-    return cudaGetLastError();
+    if (mode == 1) return pdl_launch(force64_kernel<false, 1>, grid, FORCE_THREADS, F64_SMEM, s, a);
+    if (mode == 2) return pdl_launch(force64_kernel<false, 2>, grid, FORCE_THREADS, F64_SMEM, s, a);
+    if (a.any_flagged) return pdl_launch(force64_kernel<true, 0>, grid, FORCE_THREADS, F64_SMEM, s, a);
+    return pdl_launch(force64_kernel<false, 0>, grid, FORCE_THREADS, F64_SMEM, s, a);
 }
 
 }  // namespace nb
